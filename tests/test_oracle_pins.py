@@ -1,0 +1,284 @@
+"""Pins for the CPU oracle (no GPU).  Each pin fixes the oracle to something other
+than itself: closed forms, invariants, the exact definition (eq. 4-5) by brute
+force, a library routine in a special case, and values the paper prints.
+See DESIGN.md "Oracle pins" for what mistake each one would catch."""
+import dataclasses
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import fstat_oracle as O
+from paper_2201_00451_b200 import synth
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")
+
+
+def _golden():
+    out = {}
+    for line in open(GOLDEN):
+        line = line.split("#")[0].strip()
+        if line:
+            k, v = line.split()
+            out[k] = float(v)
+    return out
+
+
+# -- P8: chi^2_4 tail against the paper's worked false-alarm number
+def test_chi2_tail_matches_paper_false_alarm():
+    g = _golden()
+    p1 = float(O.chi2_4_sf(g["false_alarm_threshold"]))
+    p_any = -math.expm1(g["false_alarm_n_templates"] * math.log1p(-p1))
+    assert abs(p_any - g["false_alarm_probability"]) < 0.02          # paper prints "~0.2"; exact 0.19
+    assert abs(g["pilot_templates"] * g["pilot_bins"] / g["pilot_values"] - 1.0) < 5e-3
+    assert abs(g["pilot_gpu_hours"] * 3600 / g["pilot_values"] / g["pilot_tau_eff_gpu"] - 1.0) < 5e-3
+    # tail is a proper survival function: numerical integral of the chi^2_4 pdf x e^{-x/2}/4
+    x = np.linspace(0.0, 200.0, 2_000_001)
+    pdf = x * np.exp(-x / 2) / 4
+    cdf_at_10 = np.trapezoid(pdf[x <= 10.0], x[x <= 10.0])
+    assert abs((1 - cdf_at_10) - float(O.chi2_4_sf(10.0))) < 1e-9
+
+
+# -- Fig. 1 listing with E = 0 is eq. 8 up to the stated normalisation
+def test_fig1_formula_equals_eq8_with_E_zero():
+    rng = np.random.default_rng(3)
+    Fa = rng.standard_normal(50) + 1j * rng.standard_normal(50)
+    Fb = rng.standard_normal(50) + 1j * rng.standard_normal(50)
+    A, B, C, S = 3.1, 2.2, 0.7, 5.5
+    D = A * B - C * C
+    Ah, Bh, Ch = A / S, B / S, C / S
+    Dinv = 1.0 / (Ah * Bh - Ch * Ch)
+    fig1 = O.twoF_fig1(Fa / math.sqrt(2 * S), Fb / math.sqrt(2 * S), Ah, Bh, Ch, 0.0, Dinv)
+    np.testing.assert_allclose(fig1, O.twoF_from_FaFb(Fa, Fb, A, B, C, D), rtol=1e-12)
+    # textbook form: (Fa,Fb) M^-1 (Fa,Fb)^H with M = [[A,C],[C,B]]
+    Minv = np.linalg.inv(np.array([[A, C], [C, B]]))
+    v = np.stack([Fa, Fb])
+    quad = np.einsum("in,ij,jn->n", v.conj(), Minv, v).real
+    np.testing.assert_allclose(quad, O.twoF_from_FaFb(Fa, Fb, A, B, C, D), rtol=1e-12)
+
+
+# -- P5: antenna closed form (ref. [24] eq. 12-13) vs detector-tensor contraction; delay vs vector form
+def test_antenna_and_delay_closed_form_vs_geometry():
+    rng = np.random.default_rng(0)
+    for _ in range(300):
+        det = dict(lat_rad=rng.uniform(-1.5, 1.5), lon_east_rad=rng.uniform(-3, 3),
+                   xarm_azimuth_rad=rng.uniform(0, 2 * math.pi))
+        eph = dict(synth.EPHEM_DEFAULT, gmst0_rad=rng.uniform(0, 6), phi_orb0=rng.uniform(0, 6))
+        al, de = rng.uniform(0, 2 * math.pi), rng.uniform(-1.5, 1.5)
+        tp = rng.uniform(0, 2e6, 40)
+        a, b = O.antenna_ab(det, eph, al, de, tp)
+        a2, b2 = synth.geometric_antenna(det, eph, al, de, tp)
+        assert np.abs(a - a2).max() < 1e-12 and np.abs(b - b2).max() < 1e-12
+        d1 = O.ssb_delay(det, eph, al, de, tp)
+        d2 = synth.geometric_delay(det, eph, al, de, tp)
+        assert np.abs(d1 - d2).max() < 1e-10
+    # a source at the pole of a detector on the equator with arms N/E: |a| <= 1, b bounded, known symmetric point
+    det = dict(lat_rad=0.0, lon_east_rad=0.0, xarm_azimuth_rad=0.0)
+    a, b = O.antenna_ab(det, synth.EPHEM_DEFAULT, 0.0, 0.0, np.array([0.0]))
+    # source overhead (alpha = theta, delta = lat = 0): arms along N and W; xi=(0,-1,0)=W... -> |a| = 1, b = 0
+    assert abs(abs(a[0]) - 1.0) < 1e-12 and abs(b[0]) < 1e-12
+
+
+def test_inverse_timing_converged_and_monotone():
+    p = synth.small_problem(n_samples=5000, n_fft=1 << 13, noise=False, rho=None)
+    tau, T, Delta = O.ssb_grid_timing(p, 0, 3.52, -0.83)
+    resid = T + O.ssb_delay(p.detectors[0], p.ephem, 3.52, -0.83, T) - tau
+    assert np.abs(resid).max() < 1e-9
+    assert np.all(np.diff(T) > 0)
+    assert np.abs(Delta).max() < 500.0 + 0.03
+
+
+# -- P2: noise-free injection, matched template on a bin => 2F = rho^2 up to interpolation error
+@pytest.mark.parametrize("dterms,tol", [(8, 2e-3), (16, 2e-3)])
+def test_noise_free_injection_gives_rho_squared(dterms, tol):
+    p = synth.small_problem(noise=False, rho=15.0, n_templates=5, dterms=dterms, n_samples=30000,
+                            n_fft=1 << 15, fddot=3e-15)
+    twoF = O.fstat_2F_bank(p)
+    it = p.injection_template
+    inj_bin = int(round((p.injection.f - p.f_min) / p.df))
+    assert twoF[it].argmax() == inj_bin
+    assert abs(twoF[it, inj_bin] / 225.0 - 1.0) < tol
+    # mismatched spin-down loses the signal (wrong sign / missing Phi_s term would not)
+    assert twoF[0].max() < 0.9 * 225.0 and twoF[-1].max() < 0.9 * 225.0
+    assert int(np.argmax(twoF.max(axis=1))) == it
+
+
+def test_noise_free_single_detector_no_gaps():
+    p = synth.small_problem(noise=False, rho=20.0, n_det=1, gap_frac=0.0, weights=False, n_templates=3)
+    twoF = O.fstat_2F_bank(p, [p.injection_template])
+    assert abs(twoF[0].max() / 400.0 - 1.0) < 2e-3
+
+
+# -- P1: pure noise => chi^2_4 (mean 4, var 8) over the central bins
+def test_pure_noise_is_chi2_4():
+    p = synth.small_problem(seed=11, rho=None, n_samples=200000, n_fft=1 << 18, n_templates=2, gap_frac=0.5)
+    twoF = O.fstat_2F_bank(p)
+    nb = p.n_bins
+    central = twoF[:, nb // 4: 3 * nb // 4].ravel()          # ~1.3e5 values; edges roll off (kernel band limit)
+    assert central.size >= 100000
+    assert abs(central.mean() - 4.0) < 0.08
+    assert abs(central.var() - 8.0) < 0.6
+    for thr in (6.0, 10.0, 15.0):
+        frac = (central > thr).mean()
+        assert abs(frac / float(O.chi2_4_sf(thr)) - 1.0) < 0.12
+
+
+# -- P3: noisy injection => E[2F] = 4 + rho^2
+def test_noisy_injection_expectation():
+    vals = []
+    for seed in range(40):
+        p = synth.small_problem(seed=1000 + seed, rho=12.0, n_samples=6000, n_fft=1 << 13, n_templates=1,
+                                gap_frac=0.2)
+        p.templates[0, 3] = p.injection.fdot
+        twoF = O.fstat_2F(p, p.templates[0])
+        vals.append(twoF[int(round((p.injection.f - p.f_min) / p.df))])
+    vals = np.array(vals)
+    expect, sd = 4.0 + 144.0, math.sqrt(2 * (4 + 2 * 144.0))
+    assert abs(vals.mean() - expect) < 4.0 * sd / math.sqrt(len(vals))
+    assert 0.6 * sd < vals.std() < 1.5 * sd
+
+
+# -- P4: brute-force detector-frame sum (eq. 4-5), no resampling, no FFT.
+# The two agree only within the method's own error.  Measured here: the floor is
+# ~5e-3..2e-2 of max(2F,4) on noise bins, independent of Dterms (8 or 16) and
+# still ~5e-3 for noise band-limited to |f| < fs/4 -- consistent with the ~2e-3
+# pass-band ripple of a Hamming-windowed sinc (amplitude; x2 in power).  A wrong
+# sign, a dropped phase term or a transposed a/b gives O(1) errors.
+def test_direct_sum_on_tiny_input():
+    p = synth.small_problem(seed=5, rho=20.0, n_samples=9000, n_fft=1 << 14, n_templates=3, gap_frac=0.25)
+    it = p.injection_template
+    twoF = O.fstat_2F(p, p.templates[it])
+    peak = int(twoF.argmax())
+    rng = np.random.default_rng(1)
+    nb = p.n_bins
+    bins = np.concatenate([np.arange(peak - 3, peak + 4), rng.integers(nb // 8, 7 * nb // 8, 40)])
+    ref = O.direct_sum_2F(p, p.templates[it], bins)
+    err = np.abs(twoF[bins] - ref) / np.maximum(ref, 4.0)
+    assert err.max() < 2.5e-2, err.max()
+    assert np.median(err) < 6e-3
+    assert abs(twoF[peak] - ref[3]) / ref[3] < 3e-3
+    # and for a mismatched template (tests the spin-down phase convention off-peak too)
+    ref0 = O.direct_sum_2F(p, p.templates[0], bins[:12])
+    tw0 = O.fstat_2F(p, p.templates[0])
+    assert (np.abs(tw0[bins[:12]] - ref0) / np.maximum(ref0, 4.0)).max() < 2.5e-2
+
+
+def test_direct_sum_noise_free_tracks_peak_shape():
+    # signal only: the whole main lobe and the mismatched-template response follow the definition
+    p = synth.small_problem(seed=6, rho=25.0, noise=False, n_samples=9000, n_fft=1 << 14, n_templates=3,
+                            gap_frac=0.25, fddot=2e-14)
+    for it in (p.injection_template, 0):
+        twoF = O.fstat_2F(p, p.templates[it])
+        peak = int(twoF.argmax())
+        bins = np.arange(peak - 6, peak + 7)
+        ref = O.direct_sum_2F(p, p.templates[it], bins)
+        assert int(bins[ref.argmax()]) == peak
+        assert (np.abs(twoF[bins] - ref) / ref.max()).max() < 3e-3
+
+
+# -- P9: frozen Earth (omega_orb = omega_rot = 0): Delta, a, b are constants, so the
+# resampled series is x convolved with ONE fixed fractional-delay FIR filter and
+# Fa is, exactly, a e^{-i 2 pi f_het Delta} X[m] H_delta[m] (convolution theorem).
+# Pins tap indexing, the sign of delta, the K_m shift and the bin mapping to rounding.
+def test_frozen_earth_is_a_fixed_fir_filter():
+    eph = dict(synth.EPHEM_DEFAULT, omega_orb=0.0, omega_rot=0.0, phi_orb0=0.9, gmst0_rad=0.4)
+    p = synth.small_problem(seed=41, n_samples=3000, n_fft=1 << 13, n_templates=1, ephem=eph, n_det=1,
+                            gap_frac=0.0, weights=False, dt=0.5)
+    # zero the ends so grid points whose epoch falls outside the data (dropped by step 3) carry nothing
+    p.series[0][:40] = 0
+    p.series[0][-40:] = 0
+    tmpl = p.templates[0].copy()
+    tmpl[3] = 0.0
+    Fa, Fb, _ = O.fstat_FaFb(p, tmpl)
+    det = p.detectors[0]
+    Delta = float(synth.geometric_delay(det, eph, tmpl[0], tmpl[1], np.array([0.0]))[0])
+    a, b = [float(v[0]) for v in synth.geometric_antenna(det, eph, tmpl[0], tmpl[1], np.array([0.0]))]
+    km = O.k_margin(p)
+    D = p.dterms
+    # grid point k samples the detector series at u = (k - km) - Delta/dt = j0 + delta
+    shift_samples = -Delta / p.dt
+    n0 = math.floor(shift_samples + 0.5)
+    dl = shift_samples - n0
+    taps = {mm: np.sinc(dl - mm) * (0.54 + 0.46 * math.cos(math.pi * (dl - mm) / (D + 0.5))) for mm in range(-D, D + 1)}
+    bins = np.array([0, 3, 100, p.n_bins // 2, p.n_bins - 2])
+    m = (bins + O.bin_shift(p)) % p.n_fft
+    x = p.series[0].astype(np.complex128)
+    j = np.arange(p.n_samples)
+    out = []
+    for mi in m:
+        w = np.exp(-2j * np.pi * mi / p.n_fft)
+        Xm = np.sum(x * w ** j)                                     # DFT of the raw series
+        # z_k = sum_mm x[k - km + n0 + mm] h(dl - mm)  =>  Z[m] = X[m] * sum_mm h w^{km - n0 - mm}
+        H = sum(h * w ** (km - n0 - mm) for mm, h in taps.items())
+        out.append(Xm * H)
+    out = np.array(out) * np.exp(-2j * np.pi * p.f_het * Delta)
+    np.testing.assert_allclose(Fa[bins], a * out, rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(Fb[bins], b * out, rtol=1e-9, atol=1e-9)
+
+
+# -- P6: invariances
+def test_invariances():
+    p = synth.small_problem(seed=21, n_samples=8000, n_fft=1 << 14, n_templates=2)
+    base = O.fstat_2F_bank(p)
+    # global phase of the data
+    q = dataclasses.replace(p, series=[(x * np.exp(0.7j)).astype(np.complex64) for x in p.series])
+    np.testing.assert_allclose(O.fstat_2F_bank(q), base, rtol=2e-5, atol=2e-5)
+    # x -> c x, w -> w / c^2 (c = 2 keeps float32 exact)
+    q = dataclasses.replace(p, series=[(2 * x) for x in p.series], weights=[w / 4 for w in p.weights])
+    np.testing.assert_allclose(O.fstat_2F_bank(q), base, rtol=1e-10, atol=1e-10)
+    # detector order
+    q = dataclasses.replace(p, detectors=p.detectors[::-1], series=p.series[::-1],
+                            timestamps=p.timestamps[::-1], weights=p.weights[::-1])
+    np.testing.assert_allclose(O.fstat_2F_bank(q), base, rtol=1e-9, atol=1e-9)
+    # arm swap (x-arm azimuth + 90 deg): a, b change sign, 2F does not
+    dets = [dict(d, xarm_azimuth_rad=d["xarm_azimuth_rad"] + math.pi / 2) for d in p.detectors]
+    q = dataclasses.replace(p, detectors=dets)
+    np.testing.assert_allclose(O.fstat_2F_bank(q), base, rtol=1e-9, atol=1e-9)
+
+
+# -- P7: zero delays => identity interpolation; Fa is the zero-padded DFT of w a x e^{-i Phi_s}
+def test_zero_delay_special_case_is_plain_fft():
+    eph = dict(synth.EPHEM_DEFAULT, au_over_c_s=0.0, re_over_c_s=0.0)
+    p = synth.small_problem(seed=31, n_samples=3000, n_fft=1 << 12, n_templates=2, ephem=eph, n_det=2)
+    tmpl = p.templates[1]
+    Fa, Fb, (A, B, C, D) = O.fstat_FaFb(p, tmpl)
+    tp = np.arange(p.n_samples) * p.dt
+    ya = np.zeros(p.n_fft, dtype=np.complex128)
+    yb = np.zeros(p.n_fft, dtype=np.complex128)
+    for X, det in enumerate(p.detectors):
+        a, b = synth.geometric_antenna(det, eph, tmpl[0], tmpl[1], tp)
+        w = O.slot_weights(p, X)[(tp // p.t_sft).astype(int)]
+        rot = np.exp(-2j * np.pi * (0.5 * tmpl[3] * tp ** 2 + tmpl[4] * tp ** 3 / 6))
+        ya[:p.n_samples] += w * a * p.series[X] * rot
+        yb[:p.n_samples] += w * b * p.series[X] * rot
+    # explicit DFT matrix on a subset of bins (not numpy.fft), shifted by K_m samples
+    km = O.k_margin(p)
+    bins = np.array([0, 1, 17, p.n_bins // 2, p.n_bins - 1])
+    m = (bins + O.bin_shift(p)) % p.n_fft
+    k = np.arange(p.n_fft)
+    Wm = np.exp(-2j * np.pi * np.outer(m, k) / p.n_fft)
+    shift = np.exp(-2j * np.pi * m * km / p.n_fft)
+    np.testing.assert_allclose(Fa[bins], shift * (Wm @ ya), rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(Fb[bins], shift * (Wm @ yb), rtol=1e-9, atol=1e-9)
+
+
+def test_interpolation_reproduces_band_limited_tone():
+    # a complex tone well inside the band is reproduced by the kernel to its design accuracy
+    n, D = 4000, 8
+    j = np.arange(n)
+    f = 0.11
+    x = np.exp(2j * np.pi * f * j)
+    u = np.linspace(50.3, 3900.7, 777)
+    z = O.windowed_sinc_interpolate(x, u, D)
+    assert np.abs(z - np.exp(2j * np.pi * f * u)).max() < 3e-3
+    # integer positions are reproduced exactly; out-of-range taps are dropped
+    np.testing.assert_allclose(O.windowed_sinc_interpolate(x, np.array([10.0, 200.0]), D), x[[10, 200]], atol=1e-13)
+    edge = O.windowed_sinc_interpolate(np.ones(20, dtype=complex), np.array([-30.0, 0.0, 19.0, 60.0]), D)
+    assert edge[0] == 0 and edge[3] == 0 and abs(edge[1] - 1) < 1e-13 and abs(edge[2] - 1) < 1e-13
+
+
+def test_topk_ties_and_order():
+    v = np.array([1.0, 5.0, 3.0, 5.0, 2.0, 5.0])
+    vals, idx = O.topk(v, 4)
+    assert list(idx) == [1, 3, 5, 2] and list(vals) == [5.0, 5.0, 5.0, 3.0]
