@@ -1,0 +1,218 @@
+"""Thin Python binding over the C ABI of include/fstat.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind
+`libfstat_b200.so`.  torch is used for device memory and streams (tensor.data_ptr(),
+torch.cuda.current_stream().cuda_stream) and nothing else.  There is no fallback:
+if the library is missing or no GPU is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+from . import build as _build
+
+FSTAT_OK, FSTAT_EINVAL, FSTAT_ESIZE, FSTAT_EDOM, FSTAT_ECUDA, FSTAT_ENOMEM = 0, -1, -2, -3, -4, -5
+
+EXPORTS = [
+    "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_host",
+    "fstat_compute_topk_host", "fstat_resample_sky", "fstat_sync", "fstat_launch_count",
+    "fstat_set_inflight", "fstat_destroy", "fstat_strerror", "fstat_last_error",
+]
+
+
+class Detector(C.Structure):
+    _fields_ = [("lat_rad", C.c_double), ("lon_east_rad", C.c_double), ("xarm_azimuth_rad", C.c_double)]
+
+
+class Ephem(C.Structure):
+    _fields_ = [("au_over_c_s", C.c_double), ("omega_orb", C.c_double), ("phi_orb0", C.c_double),
+                ("obliquity_rad", C.c_double), ("re_over_c_s", C.c_double), ("omega_rot", C.c_double),
+                ("gmst0_rad", C.c_double)]
+
+
+class FstatError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"fstat error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True) -> C.CDLL:
+    """dlopen the in-tree library; build it with nvcc first if it is missing or stale."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if build_if_missing and _build.is_stale():
+        try:
+            _build.build_library()
+        except Exception:
+            if not os.path.exists(path):
+                raise
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not built: run `python -m paper_2201_00451_b200.build`")
+    lib = C.CDLL(path)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.fstat_setup.restype = C.c_int
+    lib.fstat_setup.argtypes = [C.POINTER(vp), i32, C.POINTER(Detector), C.POINTER(vp), i64, dbl, dbl, dbl,
+                                C.POINTER(vp), C.POINTER(vp), C.POINTER(i32), dbl, C.POINTER(Ephem),
+                                i32, dbl, dbl, i64, vp]
+    lib.fstat_get_layout.restype = C.c_int
+    lib.fstat_get_layout.argtypes = [vp, C.POINTER(i64), C.POINTER(dbl)]
+    lib.fstat_compute.restype = C.c_int
+    lib.fstat_compute.argtypes = [vp, vp, i32, vp]
+    lib.fstat_compute_topk.restype = C.c_int
+    lib.fstat_compute_topk.argtypes = [vp, vp, i32, i32, vp, vp]
+    lib.fstat_compute_host.restype = C.c_int
+    lib.fstat_compute_host.argtypes = [vp, vp, i32, vp]
+    lib.fstat_compute_topk_host.restype = C.c_int
+    lib.fstat_compute_topk_host.argtypes = [vp, vp, i32, i32, vp, vp]
+    lib.fstat_resample_sky.restype = C.c_int
+    lib.fstat_resample_sky.argtypes = [vp, dbl, dbl, vp, C.POINTER(dbl)]
+    lib.fstat_sync.restype = C.c_int
+    lib.fstat_sync.argtypes = [vp]
+    lib.fstat_launch_count.restype = C.c_int
+    lib.fstat_launch_count.argtypes = [vp, C.POINTER(i64)]
+    lib.fstat_set_inflight.restype = C.c_int
+    lib.fstat_set_inflight.argtypes = [vp, i32]
+    lib.fstat_destroy.restype = None
+    lib.fstat_destroy.argtypes = [vp]
+    lib.fstat_strerror.restype = C.c_char_p
+    lib.fstat_strerror.argtypes = [C.c_int]
+    lib.fstat_last_error.restype = C.c_char_p
+    lib.fstat_last_error.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def _templates_array(templates) -> np.ndarray:
+    t = np.ascontiguousarray(np.asarray(templates, dtype=np.float64))
+    if t.ndim != 2 or t.shape[1] != 5:
+        raise ValueError("templates must be [n, 5]: alpha, delta, f0, fdot, fddot")
+    return t
+
+
+class FstatPlan:
+    """fstat_setup / fstat_compute* / fstat_destroy for one `synth.Problem`-like object."""
+
+    def __init__(self, prob, stream=None, series_on_device: bool = False):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2201_00451_b200 needs a CUDA device; there is no CPU fallback")
+        self._torch = torch
+        self.lib = load_library()
+        self.prob = prob
+        self.stream = torch.cuda.current_stream() if stream is None else stream
+        n_det = prob.n_det
+        dets = (Detector * n_det)(*[Detector(d["lat_rad"], d["lon_east_rad"], d["xarm_azimuth_rad"])
+                                    for d in prob.detectors])
+        eph = Ephem(**{k: prob.ephem[k] for k, _ in Ephem._fields_})
+        keep = []
+        if series_on_device:
+            dev = [torch.from_numpy(x.view(np.float32)).cuda() for x in prob.series]
+            keep.append(dev)
+            sptr = (C.c_void_p * n_det)(*[t.data_ptr() for t in dev])
+        else:
+            host = [np.ascontiguousarray(x, dtype=np.complex64) for x in prob.series]
+            keep.append(host)
+            sptr = (C.c_void_p * n_det)(*[x.ctypes.data for x in host])
+        ts = [np.ascontiguousarray(t, dtype=np.float64) for t in prob.timestamps]
+        ws = [np.ascontiguousarray(w, dtype=np.float32) for w in prob.weights]
+        tptr = (C.c_void_p * n_det)(*[t.ctypes.data for t in ts])
+        wptr = (C.c_void_p * n_det)(*[w.ctypes.data for w in ws])
+        nseg = (C.c_int32 * n_det)(*[len(t) for t in ts])
+        handle = C.c_void_p()
+        rc = self.lib.fstat_setup(C.byref(handle), n_det, dets, sptr, prob.n_samples, prob.t_start, prob.dt,
+                                  prob.f_het, tptr, wptr, nseg, prob.t_sft, C.byref(eph), prob.dterms,
+                                  prob.f_min, prob.band, prob.n_fft, C.c_void_p(self.stream.cuda_stream))
+        if rc != 0:
+            raise FstatError(rc, (self.lib.fstat_last_error(None) or b"").decode())
+        self.handle = handle
+        nb, df = C.c_int64(), C.c_double()
+        self._check(self.lib.fstat_get_layout(self.handle, C.byref(nb), C.byref(df)))
+        self.n_bins, self.df = int(nb.value), float(df.value)
+        self.n_fft = int(prob.n_fft)
+
+    # -- helpers ----------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise FstatError(rc, (self.lib.fstat_last_error(self.handle) or self.lib.fstat_strerror(rc)).decode())
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.fstat_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the C-ABI calls -----------------------------------------------------------
+    def compute(self, templates, out=None):
+        """fstat_compute: 2F[n_tmpl][n_bins] in device memory (a torch tensor)."""
+        t = _templates_array(templates)
+        torch = self._torch
+        if out is None:
+            out = torch.empty((t.shape[0], self.n_bins), dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.numel() == t.shape[0] * self.n_bins
+        self._check(self.lib.fstat_compute(self.handle, t.ctypes.data, t.shape[0], out.data_ptr()))
+        return out
+
+    def compute_topk(self, templates, k: int, out: Optional[Tuple] = None):
+        t = _templates_array(templates)
+        torch = self._torch
+        if out is None:
+            out = (torch.empty((t.shape[0], k), dtype=torch.float32, device="cuda"),
+                   torch.empty((t.shape[0], k), dtype=torch.int32, device="cuda"))
+        val, idx = out
+        self._check(self.lib.fstat_compute_topk(self.handle, t.ctypes.data, t.shape[0], k, val.data_ptr(), idx.data_ptr()))
+        return val, idx
+
+    def compute_host(self, templates, out=None):
+        """fstat_compute_host: 2F rows land in HOST memory (pinned torch tensor by default)."""
+        t = _templates_array(templates)
+        torch = self._torch
+        if out is None:
+            out = torch.empty((t.shape[0], self.n_bins), dtype=torch.float32, pin_memory=True)
+        assert (not out.is_cuda) and out.dtype == torch.float32 and out.is_contiguous()
+        self._check(self.lib.fstat_compute_host(self.handle, t.ctypes.data, t.shape[0], out.data_ptr()))
+        return out
+
+    def compute_topk_host(self, templates, k: int):
+        t = _templates_array(templates)
+        val = np.empty((t.shape[0], k), dtype=np.float32)
+        idx = np.empty((t.shape[0], k), dtype=np.int32)
+        self._check(self.lib.fstat_compute_topk_host(self.handle, t.ctypes.data, t.shape[0], k, val.ctypes.data, idx.ctypes.data))
+        return val, idx
+
+    def resample_sky(self, alpha: float, delta: float):
+        torch = self._torch
+        S = torch.empty((self.n_fft, 4), dtype=torch.float32, device="cuda")
+        abcd = (C.c_double * 4)()
+        self._check(self.lib.fstat_resample_sky(self.handle, alpha, delta, S.data_ptr(), abcd))
+        return S, np.array(list(abcd))
+
+    def sync(self):
+        self._check(self.lib.fstat_sync(self.handle))
+
+    def launch_count(self) -> int:
+        n = C.c_int64()
+        self._check(self.lib.fstat_launch_count(self.handle, C.byref(n)))
+        return int(n.value)
+
+    def set_inflight(self, n: int):
+        self._check(self.lib.fstat_set_inflight(self.handle, n))

@@ -1,0 +1,600 @@
+// C-ABI of the B200 resampling F-statistic path (include/fstat.h): plan management and
+// kernel orchestration.  All arithmetic of the path runs in the kernels of sky_kernels.cuh,
+// fft_kernels.cuh and topk_kernels.cuh; the host only derives O(n_det) per-sky constants.
+#include "../../include/fstat.h"
+#include "fstat_common.cuh"
+#include "sky_kernels.cuh"
+#include "fft_kernels.cuh"
+#include "topk_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+thread_local std::string g_setup_error;
+
+struct SkyGroup { double alpha, delta; int first, count; };
+
+struct HostRing {            // device row buffers for the *_host variants
+    float *buf[2] = {nullptr, nullptr};
+    cudaEvent_t done[2] = {nullptr, nullptr};   // D2H of that buffer finished
+    int64_t rows = 0;
+};
+
+}  // namespace
+
+struct fstat_plan {
+    PlanGeom g{};
+    WinTable win{};
+    cudaStream_t stream = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    fstat_detector_t det[FSTAT_MAX_DET];
+    fstat_ephem_t eph{};
+    double f_min = 0, band = 0, df = 0;
+    int device = 0;
+    // device memory
+    float2 *d_series = nullptr;
+    float *d_wslot = nullptr;
+    float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
+    float4 *d_S = nullptr;   int n_sky_slots = 0;
+    float4 *d_T = nullptr;   int n_inflight = 0;
+    SkyConst *d_sky = nullptr; size_t sky_cap = 0;
+    SkyABCD *d_abcd = nullptr;
+    double *d_abc_partial = nullptr; int abc_nblk = 0;
+    TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
+    int *d_err = nullptr;
+    float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
+    float *d_cand_v = nullptr; int *d_cand_i = nullptr; size_t cand_cap = 0;
+    HostRing ring;
+    float *d_topk_v = nullptr; int *d_topk_i = nullptr; size_t topk_cap = 0;
+    // pinned staging
+    SkyConst *h_sky = nullptr; TmplDesc *h_tmpl = nullptr;
+    cudaEvent_t staging_ev = nullptr; cudaEvent_t chunk_ev = nullptr;
+    int *h_err = nullptr;
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+#define CUDA_TRY(plan, expr)                                                                          \
+    do {                                                                                              \
+        cudaError_t e__ = (expr);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            (plan)->err = std::string(#expr) + ": " + cudaGetErrorString(e__);                        \
+            return FSTAT_ECUDA;                                                                       \
+        }                                                                                             \
+    } while (0)
+
+int fail(fstat_plan *p, int code, const std::string &msg) {
+    if (p) p->err = msg; else g_setup_error = msg;
+    return code;
+}
+
+int ilog2(int64_t v) { int l = 0; while ((int64_t(1) << l) < v) ++l; return l; }
+
+// radix list of fft_kernels.cuh RadixPlan<LOGN>
+std::vector<int> radix_list(int logn) {
+    switch (logn) {
+        case 6: return {8, 8};
+        case 7: return {16, 8};
+        case 8: return {16, 16};
+        case 9: return {8, 8, 8};
+        case 10: return {16, 16, 4};
+        case 11: return {16, 16, 8};
+        default: return {16, 16, 16};
+    }
+}
+
+// Twiddles of passes s >= 1: entry [(r-1)*P + k] = exp(-2 pi i r k / (P R)).
+std::vector<float2> make_twiddles(int logn) {
+    std::vector<float2> tw;
+    const std::vector<int> rl = radix_list(logn);
+    int P = rl[0];
+    for (size_t s = 1; s < rl.size(); ++s) {
+        const int R = rl[s];
+        for (int r = 1; r < R; ++r)
+            for (int k = 0; k < P; ++k) {
+                const double ang = -2.0 * M_PI * (double)r * (double)k / ((double)P * (double)R);
+                tw.push_back(make_float2((float)cos(ang), (float)sin(ang)));
+            }
+        P *= R;
+    }
+    return tw;
+}
+
+void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *sc) {
+    const fstat_ephem_t &e = p->eph;
+    const double nx = cos(delta) * cos(alpha), ny = cos(delta) * sin(alpha), nz = sin(delta);
+    sc->Pc = e.au_over_c_s * nx;
+    sc->Ps = e.au_over_c_s * (ny * cos(e.obliquity_rad) + nz * sin(e.obliquity_rad));
+    for (int X = 0; X < p->g.n_det; ++X) {
+        const fstat_detector_t &d = p->det[X];
+        const double lam = d.lat_rad, L = d.lon_east_rad, gam = d.xarm_azimuth_rad + 0.75 * M_PI;
+        sc->Qc[X] = e.re_over_c_s * cos(lam) * (nx * cos(L) + ny * sin(L));
+        sc->Qs[X] = e.re_over_c_s * cos(lam) * (ny * cos(L) - nx * sin(L));
+        sc->Q0[X] = e.re_over_c_s * nz * sin(lam);
+        sc->cal[X] = (float)cos(alpha - L);
+        sc->sal[X] = (float)sin(alpha - L);
+        const double s2g = sin(2 * gam), c2g = cos(2 * gam);
+        sc->ac[X][0] = (float)(0.75 * s2g * cos(lam) * cos(lam) * cos(delta) * cos(delta));
+        sc->ac[X][1] = (float)(s2g * (3.0 - cos(2 * lam)) * (3.0 - cos(2 * delta)) / 16.0);
+        sc->ac[X][2] = (float)(-0.25 * c2g * sin(lam) * (3.0 - cos(2 * delta)));
+        sc->ac[X][3] = (float)(0.25 * s2g * sin(2 * lam) * sin(2 * delta));
+        sc->ac[X][4] = (float)(-0.5 * c2g * cos(lam) * sin(2 * delta));
+        sc->bc[X][0] = (float)(c2g * sin(lam) * sin(delta));
+        sc->bc[X][1] = (float)(0.25 * s2g * (3.0 - cos(2 * lam)) * sin(delta));
+        sc->bc[X][2] = (float)(c2g * cos(lam) * cos(delta));
+        sc->bc[X][3] = (float)(0.5 * s2g * sin(2 * lam) * cos(delta));
+    }
+}
+
+template <int LOGN> int launch_pass1(fstat_plan *p, const FftArgs &a, int n_cols_blocks, int n_t) {
+    using C = FftCfg<LOGN>;
+    static thread_local int configured_dev = -1;
+    if (configured_dev != p->device) {
+        CUDA_TRY(p, cudaFuncSetAttribute(fft_pass1_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured_dev = p->device;
+    }
+    fft_pass1_kernel<LOGN><<<dim3(n_cols_blocks, n_t), C::NT, C::SMEM_BYTES, p->stream>>>(a);
+    ++p->launches;
+    return FSTAT_OK;
+}
+template <int LOGN> int launch_pass2(fstat_plan *p, const FftArgs &a, int n_row_blocks, int n_t) {
+    using C = FftCfg<LOGN>;
+    static thread_local int configured_dev = -1;
+    if (configured_dev != p->device) {
+        CUDA_TRY(p, cudaFuncSetAttribute(fft_pass2_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured_dev = p->device;
+    }
+    fft_pass2_kernel<LOGN><<<dim3(n_row_blocks, n_t), C::NT, C::SMEM_BYTES, p->stream>>>(a);
+    ++p->launches;
+    return FSTAT_OK;
+}
+
+#define DISPATCH_LOGN(logn, fn, ...)                         \
+    switch (logn) {                                          \
+        case 6: rc = fn<6>(__VA_ARGS__); break;              \
+        case 7: rc = fn<7>(__VA_ARGS__); break;              \
+        case 8: rc = fn<8>(__VA_ARGS__); break;              \
+        case 9: rc = fn<9>(__VA_ARGS__); break;              \
+        case 10: rc = fn<10>(__VA_ARGS__); break;            \
+        case 11: rc = fn<11>(__VA_ARGS__); break;            \
+        default: rc = fn<12>(__VA_ARGS__); break;            \
+    }
+
+int tile_w(int logn) { return logn == 12 ? 2 : (1 << (12 - logn)); }
+
+// FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
+int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_stride) {
+    FftArgs a{};
+    a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd;
+    a.twoF = rows; a.twoF_stride = row_stride;
+    a.n_fft = p->g.n_fft; a.n_src = p->g.n_src; a.n_bins = p->g.n_bins; a.k_margin = p->g.k_margin;
+    a.dt = p->g.dt;
+    int rc = FSTAT_OK;
+    const int l1 = p->g.log_n1, l2 = p->g.log_n2;
+    a.tw = p->d_tw1; a.log_other = l2;
+    DISPATCH_LOGN(l1, launch_pass1, p, a, (1 << l2) / tile_w(l1), nt);
+    if (rc) return rc;
+    a.tw = p->d_tw2; a.log_other = l1;
+    DISPATCH_LOGN(l2, launch_pass2, p, a, (1 << l1) / tile_w(l2), nt);
+    if (rc) return rc;
+    CUDA_TRY(p, cudaGetLastError());
+    return FSTAT_OK;
+}
+
+// Sky-dependent kernels for sky groups [g0, g0+ng) -> S slots 0..ng-1, abcd slots 0..ng-1.
+int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst) {
+    const PlanGeom &g = p->g;
+    dim3 grid((unsigned)((g.n_src + 255) / 256), ng);
+    sky_resample_kernel<<<grid, 256, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst);
+    dim3 grid2(p->abc_nblk, ng);
+    sky_abc_partial_kernel<<<grid2, ABC_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_wslot, p->d_abc_partial);
+    sky_abc_finalize_kernel<<<ng, 256, 0, p->stream>>>(p->d_abc_partial, p->abc_nblk, p->d_abcd, p->d_err);
+    p->launches += 3;
+    CUDA_TRY(p, cudaGetLastError());
+    return FSTAT_OK;
+}
+
+int ensure_tmpl_capacity(fstat_plan *p, size_t n_tmpl, size_t n_groups) {
+    if (n_tmpl > p->tmpl_cap) {
+        if (p->d_tmpl) cudaFree(p->d_tmpl);
+        if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
+        p->d_tmpl = nullptr; p->h_tmpl = nullptr; p->tmpl_cap = 0;
+        const size_t cap = n_tmpl + n_tmpl / 2 + 16;
+        CUDA_TRY(p, cudaMalloc(&p->d_tmpl, cap * sizeof(TmplDesc)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_tmpl, cap * sizeof(TmplDesc)));
+        p->tmpl_cap = cap;
+    }
+    if (n_groups > p->sky_cap) {
+        if (p->d_sky) cudaFree(p->d_sky);
+        if (p->h_sky) cudaFreeHost(p->h_sky);
+        p->d_sky = nullptr; p->h_sky = nullptr; p->sky_cap = 0;
+        const size_t cap = n_groups + n_groups / 2 + 16;
+        CUDA_TRY(p, cudaMalloc(&p->d_sky, cap * sizeof(SkyConst)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_sky, cap * sizeof(SkyConst)));
+        p->sky_cap = cap;
+    }
+    return FSTAT_OK;
+}
+
+enum OutMode { OUT_DEV_ROWS, OUT_HOST_ROWS, OUT_TOPK };
+
+struct OutSpec {
+    OutMode mode;
+    float *rows = nullptr;       // device (OUT_DEV_ROWS) or host (OUT_HOST_ROWS) [n_tmpl][n_bins]
+    int k = 0;
+    float *val = nullptr;        // device [n_tmpl][k]
+    int32_t *bin = nullptr;
+};
+
+int ensure_topk_scratch(fstat_plan *p, int k) {
+    const int64_t nb = p->g.n_bins;
+    const int nblk = (int)((nb + TOPK_SLICE - 1) / TOPK_SLICE);
+    if (!p->d_rows) CUDA_TRY(p, cudaMalloc(&p->d_rows, (size_t)p->n_inflight * nb * sizeof(float)));
+    const size_t need = (size_t)p->n_inflight * nblk * k;
+    if (need > p->cand_cap) {
+        if (p->d_cand_v) cudaFree(p->d_cand_v);
+        if (p->d_cand_i) cudaFree(p->d_cand_i);
+        p->d_cand_v = nullptr; p->d_cand_i = nullptr; p->cand_cap = 0;
+        CUDA_TRY(p, cudaMalloc(&p->d_cand_v, need * sizeof(float)));
+        CUDA_TRY(p, cudaMalloc(&p->d_cand_i, need * sizeof(int)));
+        p->cand_cap = need;
+    }
+    return FSTAT_OK;
+}
+
+int ensure_host_ring(fstat_plan *p) {
+    if (p->ring.rows) return FSTAT_OK;
+    const int64_t nb = p->g.n_bins;
+    int64_t rows = (int64_t)(64ll << 20) / (nb * 4);
+    if (rows < p->n_inflight) rows = p->n_inflight;
+    rows = (rows / p->n_inflight) * p->n_inflight;
+    for (int i = 0; i < 2; ++i) {
+        CUDA_TRY(p, cudaMalloc(&p->ring.buf[i], (size_t)rows * nb * sizeof(float)));
+        CUDA_TRY(p, cudaEventCreateWithFlags(&p->ring.done[i], cudaEventDisableTiming));
+    }
+    p->ring.rows = rows;
+    return FSTAT_OK;
+}
+
+int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, const OutSpec &out) {
+    if (!p) return FSTAT_EINVAL;
+    if (n_tmpl < 0 || (n_tmpl > 0 && !tm)) return fail(p, FSTAT_EINVAL, "null template array");
+    if (n_tmpl == 0) return FSTAT_OK;
+    if (out.mode == OUT_TOPK) {
+        if (out.k < 1 || out.k > FSTAT_MAX_TOPK || out.k > p->g.n_bins) return fail(p, FSTAT_EINVAL, "k outside [1, min(64, n_bins)]");
+        if (!out.val || !out.bin) return fail(p, FSTAT_EINVAL, "null top-k output");
+    } else if (!out.rows) return fail(p, FSTAT_EINVAL, "null 2F output");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    const double ftol = 1e-9 * fmax(1.0, fabs(p->f_min));
+    std::vector<SkyGroup> groups;
+    for (int t = 0; t < n_tmpl; ++t) {
+        if (!(fabs(tm[t].f0 - p->f_min) <= ftol)) return fail(p, FSTAT_EDOM, "template f0 differs from the plan's f_min");
+        if (!std::isfinite(tm[t].alpha) || !std::isfinite(tm[t].delta) || !std::isfinite(tm[t].fdot) || !std::isfinite(tm[t].fddot))
+            return fail(p, FSTAT_EINVAL, "non-finite template parameter");
+        if (groups.empty() || groups.back().alpha != tm[t].alpha || groups.back().delta != tm[t].delta)
+            groups.push_back({tm[t].alpha, tm[t].delta, t, 0});
+        ++groups.back().count;
+    }
+    int rc = ensure_tmpl_capacity(p, n_tmpl, groups.size());
+    if (rc) return rc;
+    // staging buffers are reused between calls: wait until the previous upload has been consumed
+    CUDA_TRY(p, cudaEventSynchronize(p->staging_ev));
+    for (size_t gi = 0; gi < groups.size(); ++gi) {
+        fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &p->h_sky[gi]);
+        for (int t = groups[gi].first; t < groups[gi].first + groups[gi].count; ++t) {
+            p->h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
+            p->h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
+            p->h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
+            p->h_tmpl[t].pad = 0;
+        }
+    }
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, p->h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaEventRecord(p->staging_ev, p->stream));
+
+    if (out.mode == OUT_TOPK) { rc = ensure_topk_scratch(p, out.k); if (rc) return rc; }
+    if (out.mode == OUT_HOST_ROWS) { rc = ensure_host_ring(p); if (rc) return rc; }
+
+    const int64_t nb = p->g.n_bins;
+    const int TB = p->n_inflight;
+    int ring_i = 0; int64_t ring_fill = 0; int64_t ring_row0 = 0;   // host-ring state
+    auto flush_ring = [&](void) -> int {
+        if (ring_fill == 0) return FSTAT_OK;
+        CUDA_TRY(p, cudaEventRecord(p->chunk_ev, p->stream));
+        CUDA_TRY(p, cudaStreamWaitEvent(p->copy_stream, p->chunk_ev, 0));
+        CUDA_TRY(p, cudaMemcpyAsync(out.rows + ring_row0 * nb, p->ring.buf[ring_i], (size_t)ring_fill * nb * sizeof(float),
+                                    cudaMemcpyDeviceToHost, p->copy_stream));
+        CUDA_TRY(p, cudaEventRecord(p->ring.done[ring_i], p->copy_stream));
+        ring_i ^= 1; ring_row0 += ring_fill; ring_fill = 0;
+        // the buffer we are about to fill must have been drained
+        CUDA_TRY(p, cudaStreamWaitEvent(p->stream, p->ring.done[ring_i], 0));
+        return FSTAT_OK;
+    };
+
+    for (size_t gb = 0; gb < groups.size(); gb += p->n_sky_slots) {
+        const int ng = (int)std::min<size_t>(p->n_sky_slots, groups.size() - gb);
+        rc = launch_sky_batch(p, (int)gb, ng, p->d_S);
+        if (rc) return rc;
+        const int t_begin = groups[gb].first;
+        const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
+        for (int t0 = t_begin; t0 < t_end; t0 += TB) {
+            const int nt = std::min(TB, t_end - t0);
+            if (out.mode == OUT_DEV_ROWS) {
+                rc = launch_fft_chunk(p, t0, nt, out.rows + (int64_t)t0 * nb, nb);
+                if (rc) return rc;
+            } else if (out.mode == OUT_HOST_ROWS) {
+                if (ring_fill + nt > p->ring.rows) { rc = flush_ring(); if (rc) return rc; }
+                rc = launch_fft_chunk(p, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb);
+                if (rc) return rc;
+                ring_fill += nt;
+            } else {
+                rc = launch_fft_chunk(p, t0, nt, p->d_rows, nb);
+                if (rc) return rc;
+                const int nblk = (int)((nb + TOPK_SLICE - 1) / TOPK_SLICE);
+                topk_stage1_kernel<<<dim3(nblk, nt), TOPK_THREADS, 0, p->stream>>>(p->d_rows, nb, nb, out.k, p->d_cand_v, p->d_cand_i);
+                topk_stage2_kernel<<<nt, TOPK_THREADS, 0, p->stream>>>(p->d_cand_v, p->d_cand_i, nblk * out.k, out.k,
+                                                                       out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k);
+                p->launches += 2;
+                CUDA_TRY(p, cudaGetLastError());
+            }
+        }
+    }
+    if (out.mode == OUT_HOST_ROWS) {
+        rc = flush_ring();
+        if (rc) return rc;
+        CUDA_TRY(p, cudaStreamSynchronize(p->copy_stream));
+    }
+    return FSTAT_OK;
+}
+
+void destroy_impl(fstat_plan *p) {
+    if (!p) return;
+    cudaSetDevice(p->device);
+    if (p->stream) cudaStreamSynchronize(p->stream);
+    cudaFree(p->d_series); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
+    cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd); cudaFree(p->d_abc_partial);
+    cudaFree(p->d_tmpl); cudaFree(p->d_err); cudaFree(p->d_rows); cudaFree(p->d_cand_v); cudaFree(p->d_cand_i);
+    cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
+    for (int i = 0; i < 2; ++i) { cudaFree(p->ring.buf[i]); if (p->ring.done[i]) cudaEventDestroy(p->ring.done[i]); }
+    if (p->h_sky) cudaFreeHost(p->h_sky);
+    if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
+    if (p->h_err) cudaFreeHost(p->h_err);
+    if (p->staging_ev) cudaEventDestroy(p->staging_ev);
+    if (p->chunk_ev) cudaEventDestroy(p->chunk_ev);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    delete p;
+}
+
+int default_inflight(int64_t n_fft) {
+    // keep the four-step intermediates of one launch within ~32 MB (L2-resident beside the source)
+    int64_t tb = (32ll << 20) / (n_fft * 16);
+    if (tb < 1) tb = 1;
+    if (tb > 64) tb = 64;
+    return (int)tb;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *fstat_strerror(int code) {
+    switch (code) {
+        case FSTAT_OK: return "ok";
+        case FSTAT_EINVAL: return "invalid argument";
+        case FSTAT_ESIZE: return "size constraint violated";
+        case FSTAT_EDOM: return "outside the domain of the plan (f0 != f_min or D <= 0)";
+        case FSTAT_ECUDA: return "CUDA error";
+        case FSTAT_ENOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+
+const char *fstat_last_error(const fstat_plan_t *plan) { return plan ? plan->err.c_str() : g_setup_error.c_str(); }
+
+int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, const void *const *series_c64,
+                int64_t n_samples, double t_start, double dt, double f_het, const double *const *timestamps,
+                const float *const *weights, const int32_t *n_seg, double t_sft, const fstat_ephem_t *eph,
+                int32_t dterms, double f_min, double band, int64_t n_fft, void *cuda_stream) {
+    if (!out) return fail(nullptr, FSTAT_EINVAL, "out is null");
+    *out = nullptr;
+    if (n_det < 1 || n_det > FSTAT_MAX_DET) return fail(nullptr, FSTAT_EINVAL, "n_det outside [1, 8]");
+    if (!det || !series_c64 || !timestamps || !weights || !n_seg || !eph) return fail(nullptr, FSTAT_EINVAL, "null argument");
+    if (!(dt > 0) || !(t_sft > 0) || n_samples < 1 || !(band > 0) || !std::isfinite(f_min) || !std::isfinite(f_het) || !std::isfinite(t_start))
+        return fail(nullptr, FSTAT_EINVAL, "dt, t_sft, n_samples, band must be positive and finite");
+    if (dterms < 1 || dterms > FSTAT_MAX_DTERMS) return fail(nullptr, FSTAT_ESIZE, "dterms outside [1, 32]");
+    if (n_fft < (1 << 12) || n_fft > (1 << 24) || (n_fft & (n_fft - 1))) return fail(nullptr, FSTAT_ESIZE, "n_fft must be a power of two in [2^12, 2^24]");
+    const int64_t km = (int64_t)ceil(512.0 / dt);
+    if (n_samples + 2 * km > n_fft) return fail(nullptr, FSTAT_ESIZE, "n_samples + 2*ceil(512 s/dt) exceeds n_fft");
+    if (band > (1.0 / dt) * (1.0 + 1e-12)) return fail(nullptr, FSTAT_ESIZE, "band wider than the sample rate 1/dt");
+    const double reach = fabs(eph->au_over_c_s) + fabs(eph->re_over_c_s);
+    if (fabs(eph->omega_rot) * reach > 0.05 || fabs(eph->omega_orb) * reach > 0.05)
+        return fail(nullptr, FSTAT_EINVAL, "ephemeris outside the small-delay regime (omega * delay must be < 0.05 rad)");
+    const int64_t n_bins = llround(band * (double)n_fft * dt);
+    if (n_bins < 1 || n_bins > n_fft) return fail(nullptr, FSTAT_ESIZE, "band gives no bins");
+    const int n_slots = (int)ceil((double)n_samples * dt / t_sft - 1e-9);
+
+    // timestamps -> dense slot weights
+    std::vector<float> wslot((size_t)n_det * n_slots, 0.f);
+    for (int X = 0; X < n_det; ++X) {
+        if (n_seg[X] < 0 || (n_seg[X] > 0 && (!timestamps[X] || !weights[X]))) return fail(nullptr, FSTAT_EINVAL, "null timestamps/weights");
+        if (!series_c64[X]) return fail(nullptr, FSTAT_EINVAL, "null series pointer");
+        long long prev = -1;
+        for (int s = 0; s < n_seg[X]; ++s) {
+            const double q = (timestamps[X][s] - t_start) / t_sft;
+            const long long idx = llround(q);
+            if (fabs(q - (double)idx) > 1e-6 || idx < 0 || idx >= n_slots) return fail(nullptr, FSTAT_EINVAL, "timestamp not on the t_start + n*t_sft grid of the series");
+            if (idx <= prev) return fail(nullptr, FSTAT_EINVAL, "timestamps unsorted or overlapping");
+            if (!(weights[X][s] >= 0.f) || !std::isfinite(weights[X][s])) return fail(nullptr, FSTAT_EINVAL, "negative or non-finite weight");
+            wslot[(size_t)X * n_slots + idx] = weights[X][s];
+            prev = idx;
+        }
+    }
+
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, FSTAT_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(ce));
+    }
+    fstat_plan *p = new (std::nothrow) fstat_plan();
+    if (!p) return fail(nullptr, FSTAT_ENOMEM, "host allocation failed");
+    auto bail = [&](int code) { g_setup_error = p->err; destroy_impl(p); return code; };
+#define SETUP_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { p->err = std::string(#expr) + ": " + cudaGetErrorString(e__); return bail(e__ == cudaErrorMemoryAllocation ? FSTAT_ENOMEM : FSTAT_ECUDA); } } while (0)
+    SETUP_TRY(cudaGetDevice(&p->device));
+    p->stream = (cudaStream_t)cuda_stream;
+    PlanGeom &g = p->g;
+    g.n_det = n_det; g.dterms = dterms; g.n_samples = n_samples; g.k_margin = km; g.n_src = n_samples + 2 * km;
+    g.n_fft = n_fft; g.n_bins = n_bins; g.series_stride = n_samples + 2 * SERIES_PAD; g.n_slots = n_slots;
+    g.dt = dt; g.inv_dt = 1.0 / dt; g.t_sft = t_sft; g.inv_t_sft = 1.0 / t_sft; g.span = (double)n_samples * dt;
+    g.f_het = f_het; g.omega_orb = eph->omega_orb; g.phi_orb0 = eph->phi_orb0; g.omega_rot = eph->omega_rot; g.gmst0 = eph->gmst0_rad;
+    const long long shift = llround((f_min - f_het) * (double)n_fft * dt);
+    g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
+    const int L = ilog2(n_fft);
+    g.log_n1 = L / 2; g.log_n2 = L - g.log_n1;
+    p->eph = *eph; p->f_min = f_min; p->band = band; p->df = 1.0 / ((double)n_fft * dt);
+    for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
+    for (int m = -dterms; m <= dterms; ++m) {
+        p->win.c[m + dterms] = (float)cos(M_PI * m / (dterms + 0.5));
+        p->win.s[m + dterms] = (float)sin(M_PI * m / (dterms + 0.5));
+    }
+
+    SETUP_TRY(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    SETUP_TRY(cudaEventCreateWithFlags(&p->staging_ev, cudaEventDisableTiming));
+    SETUP_TRY(cudaEventCreateWithFlags(&p->chunk_ev, cudaEventDisableTiming));
+    SETUP_TRY(cudaMalloc(&p->d_series, (size_t)n_det * g.series_stride * sizeof(float2)));
+    SETUP_TRY(cudaMemsetAsync(p->d_series, 0, (size_t)n_det * g.series_stride * sizeof(float2), p->stream));
+    for (int X = 0; X < n_det; ++X)
+        SETUP_TRY(cudaMemcpyAsync(p->d_series + (size_t)X * g.series_stride + SERIES_PAD, series_c64[X], (size_t)n_samples * sizeof(float2),
+                                  cudaMemcpyDefault, p->stream));
+    SETUP_TRY(cudaMalloc(&p->d_wslot, wslot.size() * sizeof(float)));
+    SETUP_TRY(cudaMemcpyAsync(p->d_wslot, wslot.data(), wslot.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
+    const std::vector<float2> tw1 = make_twiddles(g.log_n1), tw2 = make_twiddles(g.log_n2);
+    SETUP_TRY(cudaMalloc(&p->d_tw1, tw1.size() * sizeof(float2)));
+    SETUP_TRY(cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
+    SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    SETUP_TRY(cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    p->n_inflight = default_inflight(n_fft);
+    p->n_sky_slots = default_inflight(n_fft);
+    SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
+    SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
+    SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
+    SETUP_TRY(cudaMalloc(&p->d_abcd, (size_t)p->n_sky_slots * sizeof(SkyABCD)));
+    p->abc_nblk = (int)((n_samples * n_det + ABC_THREADS * ABC_PER_THREAD - 1) / (ABC_THREADS * ABC_PER_THREAD));
+    SETUP_TRY(cudaMalloc(&p->d_abc_partial, (size_t)p->n_sky_slots * p->abc_nblk * 3 * sizeof(double)));
+    SETUP_TRY(cudaMalloc(&p->d_err, sizeof(int)));
+    SETUP_TRY(cudaMemsetAsync(p->d_err, 0, sizeof(int), p->stream));
+    SETUP_TRY(cudaMallocHost(&p->h_err, sizeof(int)));
+    SETUP_TRY(cudaEventRecord(p->staging_ev, p->stream));
+    // the caller may free its buffers when we return
+    SETUP_TRY(cudaStreamSynchronize(p->stream));
+#undef SETUP_TRY
+    *out = p;
+    return FSTAT_OK;
+}
+
+int fstat_get_layout(const fstat_plan_t *plan, int64_t *n_bins, double *df) {
+    if (!plan) return FSTAT_EINVAL;
+    if (n_bins) *n_bins = plan->g.n_bins;
+    if (df) *df = plan->df;
+    return FSTAT_OK;
+}
+
+int fstat_compute(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_dev) {
+    OutSpec o; o.mode = OUT_DEV_ROWS; o.rows = twoF_dev;
+    return compute_impl(plan, tmpl_host, n_tmpl, o);
+}
+
+int fstat_compute_topk(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, int32_t k, float *val_dev, int32_t *bin_dev) {
+    OutSpec o; o.mode = OUT_TOPK; o.k = k; o.val = val_dev; o.bin = bin_dev;
+    return compute_impl(plan, tmpl_host, n_tmpl, o);
+}
+
+int fstat_compute_host(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_host) {
+    OutSpec o; o.mode = OUT_HOST_ROWS; o.rows = twoF_host;
+    int rc = compute_impl(plan, tmpl_host, n_tmpl, o);
+    if (rc) return rc;
+    return fstat_sync(plan);
+}
+
+int fstat_compute_topk_host(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, int32_t k, float *val_host, int32_t *bin_host) {
+    if (!plan) return FSTAT_EINVAL;
+    if (n_tmpl <= 0) return n_tmpl == 0 ? FSTAT_OK : FSTAT_EINVAL;
+    if (!val_host || !bin_host) return fail(plan, FSTAT_EINVAL, "null top-k output");
+    if (k < 1 || k > FSTAT_MAX_TOPK) return fail(plan, FSTAT_EINVAL, "k outside [1, 64]");
+    const size_t need = (size_t)n_tmpl * k;
+    if (need > plan->topk_cap) {
+        cudaFree(plan->d_topk_v); cudaFree(plan->d_topk_i);
+        plan->d_topk_v = nullptr; plan->d_topk_i = nullptr; plan->topk_cap = 0;
+        CUDA_TRY(plan, cudaMalloc(&plan->d_topk_v, need * sizeof(float)));
+        CUDA_TRY(plan, cudaMalloc(&plan->d_topk_i, need * sizeof(int)));
+        plan->topk_cap = need;
+    }
+    OutSpec o; o.mode = OUT_TOPK; o.k = k; o.val = plan->d_topk_v; o.bin = plan->d_topk_i;
+    int rc = compute_impl(plan, tmpl_host, n_tmpl, o);
+    if (rc) return rc;
+    CUDA_TRY(plan, cudaMemcpyAsync(val_host, plan->d_topk_v, need * sizeof(float), cudaMemcpyDeviceToHost, plan->stream));
+    CUDA_TRY(plan, cudaMemcpyAsync(bin_host, plan->d_topk_i, need * sizeof(int), cudaMemcpyDeviceToHost, plan->stream));
+    return fstat_sync(plan);
+}
+
+int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta, float *S_dev, double *abcd_host) {
+    if (!plan || !S_dev || !abcd_host) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaSetDevice(plan->device));
+    int rc = ensure_tmpl_capacity(plan, 1, 1);
+    if (rc) return rc;
+    CUDA_TRY(plan, cudaEventSynchronize(plan->staging_ev));
+    fill_sky_const(plan, alpha, delta, &plan->h_sky[0]);
+    CUDA_TRY(plan, cudaMemcpyAsync(plan->d_sky, plan->h_sky, sizeof(SkyConst), cudaMemcpyHostToDevice, plan->stream));
+    CUDA_TRY(plan, cudaEventRecord(plan->staging_ev, plan->stream));
+    CUDA_TRY(plan, cudaMemsetAsync(S_dev, 0, (size_t)plan->g.n_fft * sizeof(float4), plan->stream));
+    rc = launch_sky_batch(plan, 0, 1, (float4 *)S_dev);
+    if (rc) return rc;
+    SkyABCD r;
+    CUDA_TRY(plan, cudaMemcpyAsync(&r, plan->d_abcd, sizeof(SkyABCD), cudaMemcpyDeviceToHost, plan->stream));
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    abcd_host[0] = r.A; abcd_host[1] = r.B; abcd_host[2] = r.C; abcd_host[3] = r.D;
+    return FSTAT_OK;
+}
+
+int fstat_sync(fstat_plan_t *plan) {
+    if (!plan) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaMemcpyAsync(plan->h_err, plan->d_err, sizeof(int), cudaMemcpyDeviceToHost, plan->stream));
+    CUDA_TRY(plan, cudaMemsetAsync(plan->d_err, 0, sizeof(int), plan->stream));
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    if (*plan->h_err) return fail(plan, FSTAT_EDOM, "antenna determinant D <= 0 for at least one template (outputs are NaN)");
+    return FSTAT_OK;
+}
+
+int fstat_launch_count(const fstat_plan_t *plan, int64_t *count) {
+    if (!plan || !count) return FSTAT_EINVAL;
+    *count = plan->launches;
+    return FSTAT_OK;
+}
+
+int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight) {
+    if (!plan || n_inflight < 0 || n_inflight > 4096) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaSetDevice(plan->device));
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    const int tb = n_inflight == 0 ? default_inflight(plan->g.n_fft) : n_inflight;
+    if (tb == plan->n_inflight) return FSTAT_OK;
+    cudaFree(plan->d_T); plan->d_T = nullptr;
+    cudaFree(plan->d_rows); plan->d_rows = nullptr;
+    cudaFree(plan->d_cand_v); cudaFree(plan->d_cand_i); plan->d_cand_v = nullptr; plan->d_cand_i = nullptr; plan->cand_cap = 0;
+    for (int i = 0; i < 2; ++i) { cudaFree(plan->ring.buf[i]); plan->ring.buf[i] = nullptr; if (plan->ring.done[i]) cudaEventDestroy(plan->ring.done[i]); plan->ring.done[i] = nullptr; }
+    plan->ring.rows = 0;
+    plan->n_inflight = tb;
+    CUDA_TRY(plan, cudaMalloc(&plan->d_T, (size_t)tb * plan->g.n_fft * sizeof(float4)));
+    return FSTAT_OK;
+}
+
+void fstat_destroy(fstat_plan_t *plan) { destroy_impl(plan); }
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads without a GPU and
+exports every symbol include/fstat.h declares; argument validation that needs no device."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2201_00451_b200 import binding, build, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "fstat.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(fstat_[a-z_]+)\s*\(", text)))
+
+
+def test_library_builds_loads_and_exports_header_symbols():
+    build.build_library()
+    lib = C.CDLL(build.LIB_PATH)
+    syms = _declared_symbols()
+    assert set(syms) == set(binding.EXPORTS), (syms, binding.EXPORTS)
+    for s in syms:
+        assert hasattr(lib, s), s
+
+
+def test_strerror_and_codes():
+    lib = binding.load_library()
+    assert lib.fstat_strerror(0) == b"ok"
+    for code in (-1, -2, -3, -4, -5):
+        assert len(lib.fstat_strerror(code)) > 0
+
+
+def _setup_raw(lib, prob, **over):
+    n_det = prob.n_det
+    dets = (binding.Detector * n_det)(*[binding.Detector(d["lat_rad"], d["lon_east_rad"], d["xarm_azimuth_rad"]) for d in prob.detectors])
+    eph = binding.Ephem(**{k: prob.ephem[k] for k, _ in binding.Ephem._fields_})
+    ser = [np.ascontiguousarray(x) for x in prob.series]
+    ts = [np.ascontiguousarray(over.get("timestamps", prob.timestamps)[X], dtype=np.float64) for X in range(n_det)]
+    ws = [np.ascontiguousarray(w, dtype=np.float32) for w in prob.weights]
+    sptr = (C.c_void_p * n_det)(*[x.ctypes.data for x in ser])
+    tptr = (C.c_void_p * n_det)(*[t.ctypes.data for t in ts])
+    wptr = (C.c_void_p * n_det)(*[w.ctypes.data for w in ws])
+    nseg = (C.c_int32 * n_det)(*[len(t) for t in ts])
+    h = C.c_void_p()
+    rc = lib.fstat_setup(C.byref(h), n_det, dets, sptr, prob.n_samples, prob.t_start, prob.dt, prob.f_het, tptr, wptr, nseg,
+                         prob.t_sft, C.byref(eph), over.get("dterms", prob.dterms), prob.f_min, over.get("band", prob.band),
+                         over.get("n_fft", prob.n_fft), None)
+    return rc, h
+
+
+def test_setup_argument_validation_without_gpu():
+    """Validation runs before any CUDA call, so these codes are observable on a CPU box."""
+    lib = binding.load_library()
+    p = synth.small_problem(n_samples=5000, n_fft=1 << 13, rho=None)
+    assert _setup_raw(lib, p, n_fft=(1 << 13) + 2)[0] == binding.FSTAT_ESIZE          # not a power of two
+    assert _setup_raw(lib, p, n_fft=1 << 12)[0] == binding.FSTAT_ESIZE                # n_samples + 2 K_m > n_fft
+    assert _setup_raw(lib, p, band=1.5 / p.dt)[0] == binding.FSTAT_ESIZE              # band > sample rate
+    assert _setup_raw(lib, p, dterms=0)[0] == binding.FSTAT_ESIZE
+    assert _setup_raw(lib, p, dterms=33)[0] == binding.FSTAT_ESIZE
+    bad = [t.copy() for t in p.timestamps]
+    bad[0][0] += 7.0                                                                   # off the slot grid
+    assert _setup_raw(lib, p, timestamps=bad)[0] == binding.FSTAT_EINVAL
+    bad = [t[::-1].copy() for t in p.timestamps]                                       # unsorted
+    assert _setup_raw(lib, p, timestamps=bad)[0] == binding.FSTAT_EINVAL
+    assert len(lib.fstat_last_error(None)) > 0
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    lib = binding.load_library()
+    p = synth.small_problem(n_samples=5000, n_fft=1 << 13, rho=None)
+    rc, _ = _setup_raw(lib, p)
+    assert rc == binding.FSTAT_ECUDA                      # valid arguments, but no device: fails loudly
+    with pytest.raises(RuntimeError):
+        binding.FstatPlan(p)
