@@ -1,0 +1,166 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the resampling F-statistic hot path on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one pass of the whole hot path (sky-dependent kernels, fused FFT passes, 2F) over
+one batch of synthetic input: `fstat_compute` on the full template bank of the workload
+(default: BASELINE.json configs[1] -- 2 detectors, 10 d at 2 Hz, 30 % gaps, 1024 fdot templates,
+FFT 2^21).  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2201_00451_b200 import synth  # noqa: E402
+
+METRIC = "2F_bins_per_s"
+UNIT = "2F-bins/s"
+
+
+def make_workload(name: str, rank: int = 0):
+    if name == "config2":
+        p = synth.config2()
+    elif name == "config1":
+        p = synth.config1()
+    elif name.startswith("config3"):          # config3:<days>:<band>
+        _, d, b = name.split(":")
+        p = synth.config3(float(d) if "." in d else int(d), float(b))
+    elif name.startswith("config4"):          # config4:<target>[:n_fdot]
+        parts = name.split(":")
+        p = synth.config4(int(parts[1]), n_fdot=int(parts[2]) if len(parts) > 2 else 256)
+    elif name.startswith("config5"):          # config5[:n_sky]
+        parts = name.split(":")
+        p = synth.config5(n_sky=int(parts[1]) if len(parts) > 1 else 512)
+    elif name == "small":
+        p = synth.small_problem(n_samples=20000, n_fft=1 << 15, n_templates=64)
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if rank > 0:                              # replicas: every rank searches its own fdot sub-bank
+        span = float(np.ptp(p.templates[:, 3])) or 1e-9
+        p.templates[:, 3] -= rank * span
+    return p
+
+
+def algorithmic_bytes(p):
+    """Per-template algorithmic bytes of the two FFT passes:
+    pass 1 reads the detector-summed resampled series (16 B x n_src) and writes the four-step
+    intermediate (16 B x n_fft); pass 2 reads it back and writes 2F (4 B x n_bins).  Their sum is
+    SURVEY.md 8(d)'s B_2pass."""
+    n_src = p.n_samples + 2 * int(np.ceil(512.0 / p.dt))
+    b1 = 16 * n_src + 16 * p.n_fft
+    b2 = 16 * p.n_fft + 4 * p.n_bins
+    return b1, b2
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15 and len(r) >= 7] or [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "power_w_max": max(float(r[2]) for r in rows),
+                "samples": len(rows), "reasons": reasons}
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py touches oracle/)
+# ------------------------------------------------------------------------------------------
+def oracle_step(p, n_templates: int):
+    """One bounded oracle sample: the sky-dependent work once, then n_templates templates."""
+    from oracle import fstat_oracle as O
+    t0 = time.perf_counter()
+    sky = O.per_sky(p, float(p.templates[0, 0]), float(p.templates[0, 1]))
+    t1 = time.perf_counter()
+    for i in range(n_templates):
+        O.fstat_2F(p, p.templates[i], sky)
+    t2 = time.perf_counter()
+    return t1 - t0, (t2 - t1) / n_templates
+
+
+def cpu_baseline(p, n_templates: int = 8):
+    t_sky, t_tmpl = oracle_step(p, n_templates)
+    n_groups = len({(float(a), float(d)) for a, d in p.templates[:, :2]})
+    n_t = len(p.templates)
+    full = n_groups * t_sky + n_t * t_tmpl             # extrapolated to the whole bank
+    return {"value": n_t * p.n_bins / full, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "templates_per_s": n_t / full,
+            "sample": f"numpy fp64 oracle, 1 sky preparation ({t_sky:.2f} s) + {n_templates} of {n_t} templates "
+                      f"({t_tmpl:.3f} s each), extrapolated to the bank ({n_groups} sky position(s))"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    p = make_workload(args.workload)
+    n_per_step = 2
+    times = []
+    for s in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle_step(p, n_per_step)
+        dt = time.perf_counter() - t0
+        if s >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = n_per_step * p.n_bins / (ms * 1e-3)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "n_det": p.n_det, "n_samples": p.n_samples, "n_fft": p.n_fft,
+                       "n_bins": p.n_bins, "templates_per_step": n_per_step,
+                       "note": "CPU oracle (numpy fp64) on a bounded sample: one sky preparation + 2 templates per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": f"{n_per_step} templates + 1 sky preparation per step"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))

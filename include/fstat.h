@@ -152,6 +152,15 @@ FSTAT_API int fstat_launch_count(const fstat_plan_t *plan, int64_t *count);
  * kept in flight; bounds the L2 / HBM footprint of the four-step FFT. */
 FSTAT_API int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight);
 
+/* Per-kernel-class device timing with CUDA events on the plan's stream (for the roofline
+ * report).  While enabled, every group of launches of one class is bracketed by two events.
+ * fstat_get_profile waits for the stream, writes the summed elapsed milliseconds and launch
+ * counts since the last call into HOST ms[4], launches[4], and resets the record.
+ * Classes: 0 = sky-dependent kernels (timing, resampling, antenna sums), 1 = FFT pass 1
+ * (spin-down prologue + column FFTs), 2 = FFT pass 2 (row FFTs + 2F epilogue), 3 = top-k. */
+FSTAT_API int fstat_set_profile(fstat_plan_t *plan, int32_t enable);
+FSTAT_API int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launches);
+
 FSTAT_API void fstat_destroy(fstat_plan_t *plan);
 
 FSTAT_API const char *fstat_strerror(int code);

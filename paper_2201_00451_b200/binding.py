@@ -20,7 +20,7 @@ FSTAT_OK, FSTAT_EINVAL, FSTAT_ESIZE, FSTAT_EDOM, FSTAT_ECUDA, FSTAT_ENOMEM = 0, 
 EXPORTS = [
     "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_host",
     "fstat_compute_topk_host", "fstat_resample_sky", "fstat_sync", "fstat_launch_count",
-    "fstat_set_inflight", "fstat_destroy", "fstat_strerror", "fstat_last_error",
+    "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile", "fstat_destroy", "fstat_strerror", "fstat_last_error",
 ]
 
 
@@ -81,6 +81,10 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.fstat_set_inflight.restype = C.c_int
     lib.fstat_set_inflight.argtypes = [vp, i32]
+    lib.fstat_set_profile.restype = C.c_int
+    lib.fstat_set_profile.argtypes = [vp, i32]
+    lib.fstat_get_profile.restype = C.c_int
+    lib.fstat_get_profile.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     lib.fstat_destroy.restype = None
     lib.fstat_destroy.argtypes = [vp]
     lib.fstat_strerror.restype = C.c_char_p
@@ -213,6 +217,18 @@ class FstatPlan:
         n = C.c_int64()
         self._check(self.lib.fstat_launch_count(self.handle, C.byref(n)))
         return int(n.value)
+
+    PROFILE_CLASSES = ("sky", "fft_pass1", "fft_pass2", "topk")
+
+    def set_profile(self, enable: bool):
+        self._check(self.lib.fstat_set_profile(self.handle, 1 if enable else 0))
+
+    def get_profile(self):
+        """{class: (milliseconds, launches)} since the last call."""
+        ms = (C.c_double * 4)()
+        n = (C.c_int64 * 4)()
+        self._check(self.lib.fstat_get_profile(self.handle, ms, n))
+        return {c: (float(ms[i]), int(n[i])) for i, c in enumerate(self.PROFILE_CLASSES)}
 
     def set_inflight(self, n: int):
         self._check(self.lib.fstat_set_inflight(self.handle, n))

@@ -58,6 +58,11 @@ struct fstat_plan {
     int *h_err = nullptr;
     int64_t launches = 0;
     std::string err;
+    // optional per-kernel-class timing (fstat_set_profile)
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
+    struct Seg { int cls; size_t e0, e1; int launches; };
+    std::vector<Seg> segs;
 };
 
 namespace {
@@ -75,6 +80,20 @@ int fail(fstat_plan *p, int code, const std::string &msg) {
     if (p) p->err = msg; else g_setup_error = msg;
     return code;
 }
+
+// profiling: bracket a group of launches of one class with two events on the plan's stream
+size_t prof_mark(fstat_plan *p) {
+    if (p->ev_used == p->ev_pool.size()) {
+        cudaEvent_t e; cudaEventCreate(&e); p->ev_pool.push_back(e);
+    }
+    cudaEventRecord(p->ev_pool[p->ev_used], p->stream);
+    return p->ev_used++;
+}
+struct ProfScope {
+    fstat_plan *p; int cls; size_t e0; int64_t l0;
+    ProfScope(fstat_plan *pl, int c) : p(pl), cls(c), e0(0), l0(pl->launches) { if (p->profile) e0 = prof_mark(p); }
+    ~ProfScope() { if (p->profile) { size_t e1 = prof_mark(p); p->segs.push_back({cls, e0, e1, (int)(p->launches - l0)}); } }
+};
 
 int ilog2(int64_t v) { int l = 0; while ((int64_t(1) << l) < v) ++l; return l; }
 
@@ -180,10 +199,10 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
     int rc = FSTAT_OK;
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
     a.tw = p->d_tw1; a.log_other = l2;
-    DISPATCH_LOGN(l1, launch_pass1, p, a, (1 << l2) / tile_w(l1), nt);
+    { ProfScope ps(p, 1); DISPATCH_LOGN(l1, launch_pass1, p, a, (1 << l2) / tile_w(l1), nt); }
     if (rc) return rc;
     a.tw = p->d_tw2; a.log_other = l1;
-    DISPATCH_LOGN(l2, launch_pass2, p, a, (1 << l1) / tile_w(l2), nt);
+    { ProfScope ps(p, 2); DISPATCH_LOGN(l2, launch_pass2, p, a, (1 << l1) / tile_w(l2), nt); }
     if (rc) return rc;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -192,6 +211,7 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
 // Sky-dependent kernels for sky groups [g0, g0+ng) -> S slots 0..ng-1, abcd slots 0..ng-1.
 int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst) {
     const PlanGeom &g = p->g;
+    ProfScope ps(p, 0);
     dim3 grid((unsigned)((g.n_src + 255) / 256), ng);
     sky_resample_kernel<<<grid, 256, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst);
     dim3 grid2(p->abc_nblk, ng);
@@ -339,6 +359,7 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
                 rc = launch_fft_chunk(p, t0, nt, p->d_rows, nb);
                 if (rc) return rc;
                 const int nblk = (int)((nb + TOPK_SLICE - 1) / TOPK_SLICE);
+                ProfScope ps(p, 3);
                 topk_stage1_kernel<<<dim3(nblk, nt), TOPK_THREADS, 0, p->stream>>>(p->d_rows, nb, nb, out.k, p->d_cand_v, p->d_cand_i);
                 topk_stage2_kernel<<<nt, TOPK_THREADS, 0, p->stream>>>(p->d_cand_v, p->d_cand_i, nblk * out.k, out.k,
                                                                        out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k);
@@ -370,6 +391,7 @@ void destroy_impl(fstat_plan *p) {
     if (p->staging_ev) cudaEventDestroy(p->staging_ev);
     if (p->chunk_ev) cudaEventDestroy(p->chunk_ev);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
     delete p;
 }
 
@@ -592,6 +614,27 @@ int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight) {
     plan->ring.rows = 0;
     plan->n_inflight = tb;
     CUDA_TRY(plan, cudaMalloc(&plan->d_T, (size_t)tb * plan->g.n_fft * sizeof(float4)));
+    return FSTAT_OK;
+}
+
+int fstat_set_profile(fstat_plan_t *plan, int32_t enable) {
+    if (!plan) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    plan->profile = enable != 0;
+    plan->segs.clear(); plan->ev_used = 0;
+    return FSTAT_OK;
+}
+
+int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launches) {
+    if (!plan || !ms || !launches) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    for (int c = 0; c < 4; ++c) { ms[c] = 0.0; launches[c] = 0; }
+    for (const fstat_plan::Seg &sg : plan->segs) {
+        float t = 0.f;
+        CUDA_TRY(plan, cudaEventElapsedTime(&t, plan->ev_pool[sg.e0], plan->ev_pool[sg.e1]));
+        ms[sg.cls] += t; launches[sg.cls] += sg.launches;
+    }
+    plan->segs.clear(); plan->ev_used = 0;
     return FSTAT_OK;
 }
 

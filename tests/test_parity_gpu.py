@@ -1,0 +1,172 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerance (BASELINE.json north_star):
+|2F_gpu - 2F_cpu| <= 1e-3 * max(2F_cpu, 4) per bin; loudest template identical."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import fstat_oracle as O
+from paper_2201_00451_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-3
+
+
+def _plan(prob, **kw):
+    from paper_2201_00451_b200.binding import FstatPlan
+    return FstatPlan(prob, **kw)
+
+
+def _rel_err(gpu, cpu):
+    return np.abs(gpu.astype(np.float64) - cpu) / np.maximum(cpu, 4.0)
+
+
+def _check_bank(prob, idxs=None, tol=TOL):
+    idxs = list(range(len(prob.templates))) if idxs is None else list(idxs)
+    cpu = O.fstat_2F_bank(prob, idxs)
+    with _plan(prob) as plan:
+        gpu = plan.compute(prob.templates[idxs])
+        plan.sync()
+        gpu = gpu.cpu().numpy()
+    assert gpu.shape == cpu.shape
+    err = _rel_err(gpu, cpu)
+    assert np.isfinite(gpu).all()
+    assert err.max() <= tol, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    return gpu, cpu
+
+
+# every sub-FFT length 2^6 .. 2^12 appears in one of these (n_fft = 2^12 .. 2^24 splits as L/2, L-L/2)
+@pytest.mark.parametrize("log_nfft,n_samples,dt", [
+    (12, 1500, 1.0), (13, 5000, 1.0), (14, 11000, 1.0), (15, 20000, 1.0), (16, 50001, 1.0),
+    (17, 100003, 1.0), (18, 250000, 0.5), (19, 400001, 0.5),
+])
+def test_parity_small_all_bins(log_nfft, n_samples, dt):
+    p = synth.small_problem(seed=log_nfft, n_samples=n_samples, dt=dt, n_fft=1 << log_nfft, n_templates=3,
+                            gap_frac=0.3, rho=12.0, fddot=1e-16)
+    gpu, cpu = _check_bank(p)
+    assert int(np.argmax(gpu.max(axis=1))) == int(np.argmax(cpu.max(axis=1)))
+    if n_samples * dt >= 50000:       # shorter spans cannot tell the fdot templates apart
+        assert int(np.argmax(gpu.max(axis=1))) == p.injection_template
+
+
+@pytest.mark.parametrize("log_nfft", [20, 21, 22])
+def test_parity_large_fft_one_template(log_nfft):
+    n = int(0.8 * (1 << log_nfft))
+    p = synth.small_problem(seed=100 + log_nfft, n_samples=n, dt=0.5, n_fft=1 << log_nfft, n_templates=2,
+                            gap_frac=0.4, rho=15.0)
+    _check_bank(p, [p.injection_template])
+
+
+def test_parity_fs_equals_band_full_output():
+    # config-4 shape: band = sample rate, every FFT output is a bin, f_het at band centre
+    p = synth.small_problem(seed=3, n_samples=30000, dt=0.5, n_fft=1 << 16, n_templates=2, band=2.0, rho=10.0)
+    assert p.n_bins == p.n_fft
+    _check_bank(p)
+
+
+def test_parity_dterms16_single_detector_no_gaps():
+    p = synth.small_problem(seed=4, n_det=1, n_samples=40000, n_fft=1 << 16, dterms=16, gap_frac=0.0,
+                            weights=False, n_templates=2, rho=20.0)
+    _check_bank(p)
+
+
+def test_resampled_series_and_antenna_sums_match_oracle():
+    p = synth.small_problem(seed=9, n_samples=30000, n_fft=1 << 15, n_templates=1)
+    al, de = synth.SKY0
+    sky = O.per_sky(p, al, de)
+    n_src = p.n_samples + 2 * O.k_margin(p)
+    ya = np.zeros(n_src, dtype=np.complex128)
+    yb = np.zeros(n_src, dtype=np.complex128)
+    k = np.arange(n_src)
+    for X in range(p.n_det):
+        s = sky["det"][X]
+        rot = np.exp(-2j * np.pi * np.mod(p.f_het * s["Delta"], 1.0))
+        ya += s["wk"] * s["a"] * s["z"] * rot
+        yb += s["wk"] * s["b"] * s["z"] * rot
+    shift = np.exp(-2j * np.pi * np.mod(O.bin_shift(p) * k, p.n_fft) / p.n_fft)
+    ya *= shift
+    yb *= shift
+    with _plan(p) as plan:
+        S, abcd = plan.resample_sky(al, de)
+        S = S.cpu().numpy().astype(np.float64)
+    scale = np.abs(np.concatenate([ya, yb])).max()
+    assert np.abs(S[:n_src, 0] + 1j * S[:n_src, 1] - ya).max() <= 2e-5 * scale
+    assert np.abs(S[:n_src, 2] + 1j * S[:n_src, 3] - yb).max() <= 2e-5 * scale
+    assert np.all(S[n_src:] == 0)
+    np.testing.assert_allclose(abcd, np.array(sky["ABCD"]), rtol=2e-6)
+
+
+def test_multiple_sky_positions_in_one_call():
+    # config-5 shape: sky-major template order, sky-dependent work redone per sky position
+    p = synth.small_problem(seed=12, n_samples=20000, n_fft=1 << 15, n_templates=2, rho=None)
+    sky = synth.disc_sky_points(5, seed=1)
+    rows = [(a, d, p.f_min, fd, 0.0) for (a, d) in sky for fd in (-3e-9, 0.0)]
+    p.templates = np.array(rows)
+    _check_bank(p)
+
+
+def test_topk_matches_oracle_topk():
+    p = synth.small_problem(seed=13, n_samples=30000, n_fft=1 << 15, n_templates=4, rho=14.0)
+    k = 10
+    cpu = O.fstat_2F_bank(p)
+    with _plan(p) as plan:
+        val, idx = plan.compute_topk(p.templates, k)
+        full = plan.compute(p.templates)
+        plan.sync()
+        val, idx, full = val.cpu().numpy(), idx.cpu().numpy(), full.cpu().numpy()
+        hv, hi = plan.compute_topk_host(p.templates, k)
+    np.testing.assert_array_equal(hv, val)
+    np.testing.assert_array_equal(hi, idx)
+    for t in range(len(p.templates)):
+        # bit-exact against the same selection rule applied to the GPU's own 2F row
+        ev, ei = O.topk(full[t], k)
+        np.testing.assert_array_equal(idx[t], ei)
+        np.testing.assert_array_equal(val[t], ev)
+        # and against the oracle: same loudest bin, values within tolerance
+        cv, ci = O.topk(cpu[t], k)
+        assert idx[t, 0] == ci[0]
+        assert abs(val[t, 0] - cv[0]) <= TOL * max(cv[0], 4.0)
+        assert np.all(np.diff(val[t]) <= 0)
+
+
+def test_host_variant_equals_device_variant():
+    p = synth.small_problem(seed=14, n_samples=20000, n_fft=1 << 15, n_templates=7)
+    with _plan(p) as plan:
+        dev = plan.compute(p.templates)
+        plan.sync()
+        host = plan.compute_host(p.templates)
+        np.testing.assert_array_equal(host.numpy(), dev.cpu().numpy())
+        plan.set_inflight(2)
+        host2 = plan.compute_host(p.templates)
+        np.testing.assert_array_equal(host2.numpy(), dev.cpu().numpy())
+        assert plan.launch_count() > 0
+
+
+def test_series_on_device_and_error_codes():
+    from paper_2201_00451_b200.binding import FstatError, FSTAT_EDOM
+    p = synth.small_problem(seed=15, n_samples=8000, n_fft=1 << 14, n_templates=2)
+    with _plan(p) as a, _plan(p, series_on_device=True) as b:
+        ra, rb = a.compute(p.templates), b.compute(p.templates)
+        a.sync(); b.sync()
+        np.testing.assert_array_equal(ra.cpu().numpy(), rb.cpu().numpy())
+        bad = p.templates.copy()
+        bad[0, 2] += 0.1
+        with pytest.raises(FstatError) as ei:
+            a.compute(bad)
+        assert ei.value.code == FSTAT_EDOM
+        a.compute(p.templates[:0])            # empty batch is a no-op
+
+
+def test_empty_detector_gives_edom():
+    from paper_2201_00451_b200.binding import FstatError, FSTAT_EDOM
+    p = synth.small_problem(seed=16, n_det=1, n_samples=8000, n_fft=1 << 14, n_templates=1)
+    p.timestamps = [p.timestamps[0][:0]]
+    p.weights = [p.weights[0][:0]]
+    with _plan(p) as plan:
+        out = plan.compute(p.templates)
+        with pytest.raises(FstatError) as ei:
+            plan.sync()
+        assert ei.value.code == FSTAT_EDOM
+        assert np.isnan(out.cpu().numpy()).all()
