@@ -31,8 +31,9 @@ UNIT = "2F-bins/s"
 
 
 def make_workload(name: str, rank: int = 0):
-    if name == "config2":
-        p = synth.config2()
+    if name.startswith("config2"):            # config2[:n_templates]
+        parts = name.split(":")
+        p = synth.config2(n_templates=int(parts[1])) if len(parts) > 1 else synth.config2()
     elif name == "config1":
         p = synth.config1()
     elif name.startswith("config3"):          # config3:<days>:<band>
@@ -164,3 +165,159 @@ def run_reference(args):
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------
+# Our arm
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2201_00451_b200.binding import FstatPlan
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p = make_workload(args.workload, rank)
+    plan = FstatPlan(p)
+    if args.inflight:
+        plan.set_inflight(args.inflight)
+    n_t, nb = len(p.templates), plan.n_bins
+    out = torch.empty((n_t, nb), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.compute(p.templates, out=out)
+
+    for _ in range(args.warmup):
+        step()
+    plan.sync()
+    # ---- timed region: K steps, per-step CUDA events on the plan's stream, L2 flushed between steps
+    plan.set_profile(not args.no_kernel_events)
+    l0 = plan.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    t_wall0 = time.time()
+    for s in range(args.steps):
+        flush.zero_()
+        ev[s][0].record(stream)
+        step()
+        ev[s][1].record(stream)
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1)
+    prof = plan.get_profile() if not args.no_kernel_events else None
+    plan.set_profile(False)
+    launches = plan.launch_count() - l0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n_t * nb / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel class (CUDA events inside the library, same timed steps)
+    roofline = None
+    kernels = None
+    if prof is not None:
+        b1, b2 = algorithmic_bytes(p)
+        peak, peak_src = measured_peaks()
+        per_launch_t = plan_inflight = None
+        kernels = {}
+        for cls, bytes_per_t in (("fft_pass1", b1), ("fft_pass2", b2)):
+            ms, n = prof[cls]
+            tot_bytes = bytes_per_t * n_t * args.steps
+            kernels[cls] = {"ms_total": ms, "launches": n, "avg_launch_us": 1e3 * ms / max(n, 1),
+                            "algorithmic_bytes_per_template": bytes_per_t,
+                            "achieved_gbs": tot_bytes / (ms * 1e-3) / 1e9 if ms > 0 else None}
+        kernels["sky"] = {"ms_total": prof["sky"][0], "launches": prof["sky"][1]}
+        dom = max(("fft_pass1", "fft_pass2"), key=lambda c: prof[c][0])
+        ach = kernels[dom]["achieved_gbs"]
+        both = (b1 + b2) * n_t * args.steps / ((prof["fft_pass1"][0] + prof["fft_pass2"][0]) * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": None, "peak_source": peak_src,
+                    "fft_pair_achieved": both, "fft_pair_frac": both / peak,
+                    "share_of_step": prof[dom][0] / total_ms if world == 1 else None}
+
+    # ---- end to end through the host-buffer entry point (pinned host 2F, D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        host_out = torch.empty((n_t, nb), dtype=torch.float32, pin_memory=True)
+        plan.compute_host(p.templates, out=host_out)                  # warm-up (allocates the device ring)
+        n_e2e = max(1, min(args.steps, 3))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            plan.compute_host(p.templates, out=host_out)              # blocks until the rows have landed
+        torch.cuda.synchronize()
+        e_ms = 1e3 * (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([e_ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": world * n_t * nb / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": n_e2e,
+               "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(n_t * nb * 4),
+               "api": "fstat_compute_host (host templates in, pinned host 2F[n_tmpl][n_bins] out); the series is uploaded once "
+                      "by fstat_setup (PAPER.md:93) and is not part of a step"}
+        del host_out
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(p, args.cpu_templates)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "templates_per_s": world * n_t / (ms_per_step * 1e-3),
+                "tau_eff_s_per_bin_per_detector": ms_per_step * 1e-3 / (n_t * nb * p.n_det),
+                "config": {"workload": args.workload, "n_det": p.n_det, "n_samples": p.n_samples, "dt": p.dt, "n_fft": p.n_fft,
+                           "n_bins": nb, "n_templates": n_t, "dterms": p.dterms, "multi_gpu": "independent replicas, no collective",
+                           "l2": "256 MiB flush buffer written between timed steps; each step also writes "
+                                 f"{n_t * nb * 4 / 1e9:.2f} GB of 2F (> L2)"},
+                "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
+                "cpu_baseline": cpu}
+        print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--cpu-templates", type=int, default=8)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-events", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
