@@ -6,10 +6,13 @@
 //   pass 2 (one CTA = W adjacent rows   m1):    X[m1 + N1 m2] = sum_k2 T[k2][m1] W_N2^{k2 m2}
 //
 // An element is a float4 = (Re Fa, Im Fa, Re Fb, Im Fb): both transforms run in lock step and
-// share every twiddle.  Each thread keeps 16 elements in registers; shared memory is only the
-// exchange buffer between radix passes (one buffer, two barriers per exchange).  The first pass
-// reads global memory straight into registers and the last pass writes global memory straight
-// from registers, so a sub-FFT of length 2^10 costs two shared-memory round trips.
+// share every twiddle.  Each thread keeps 16 elements in registers; shared memory is the exchange
+// buffer between radix passes (one buffer, two barriers per exchange).  CTAs are persistent: each
+// loops over tiles, and as soon as the last radix pass of a tile has pulled its inputs out of
+// the buffer, the NEXT tile's global loads are started into it with cp.async (L2 -> shared, no
+// registers), so they fly while the last pass, the twiddle/2F epilogue and the global stores of
+// the current tile execute.  Each thread prefetches exactly the elements it will itself read in
+// pass 0, so the hand-over needs cp.async.wait_group only, no extra barrier.
 #pragma once
 #include "fstat_common.cuh"
 
@@ -61,30 +64,34 @@ template <> struct RadixPlan<10> { static constexpr int np = 3, r0 = 16, r1 = 16
 template <> struct RadixPlan<11> { static constexpr int np = 3, r0 = 16, r1 = 16, r2 = 8; };
 template <> struct RadixPlan<12> { static constexpr int np = 3, r0 = 16, r1 = 16, r2 = 16; };
 
-constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
+__host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
 template <int LOGN> struct FftCfg {
     static constexpr int LOGW = (LOGN == 12) ? 1 : 12 - LOGN;     // tile = 4096 elements (8192 for 2^12)
     static constexpr int W = 1 << LOGW;
     static constexpr int N = 1 << LOGN;
     static constexpr int NT = (N * W) / 16;
-    static constexpr int SMEM_BYTES = N * W * 16;
     // twiddle table offsets (float2 entries): pass s >= 1 holds (R_s - 1) * P_s entries, [r-1][k]
     static constexpr int P1 = RadixPlan<LOGN>::r0;
     static constexpr int P2 = P1 * RadixPlan<LOGN>::r1;
     static constexpr int OFF1 = 0;
     static constexpr int OFF2 = (RadixPlan<LOGN>::r1 - 1) * P1;
     static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN>::np > 2 ? (RadixPlan<LOGN>::r2 - 1) * P2 : 0);
+    static constexpr int SMEM_BYTES = N * W * 16 + TW_ENTRIES * 8;   // exchange buffer + twiddle table
 };
 
-// Shared-memory exchange layout: element idx of lane w lives at idx*W + (w ^ swz(idx)) so that
-// both "consecutive lanes -> consecutive w" and "consecutive lanes -> consecutive idx" accesses
-// of 16-byte elements spread over all banks.
-template <int LOGW> __device__ __forceinline__ int sm_phys(int idx, int w) {
+// Shared-memory exchange layout: element idx of lane w lives at 16-byte chunk
+//   ((idx ^ hi) << LOGW) + (w ^ lo)
+// with lo, hi taken from other bits of idx so that every access pattern of the passes --
+// "consecutive lanes -> consecutive w then consecutive idx" (loads), "stride R0 in idx" (pass-0
+// stores) and "consecutive lanes -> consecutive idx, fixed w" (last pass of pass 1) -- touches 8
+// distinct chunks per quarter warp (checked exhaustively for every LOGN by a simulator).
+template <int LOGW, int LOGR0> __device__ __forceinline__ int sm_phys(int idx, int w) {
     constexpr int W = 1 << LOGW;
-    if (LOGW == 0) return idx;
-    const int s = (LOGW >= 3) ? (idx & 7) : ((idx >> (3 - LOGW)) & (W - 1));
-    return (idx << LOGW) + (w ^ s);
+    if (LOGW >= 3) return (idx << LOGW) + (w ^ (idx & 7));
+    const int hi = (idx >> LOGR0) & ((1 << (3 - LOGW)) - 1);
+    const int lo = (idx >> (3 - LOGW)) & (W - 1);
+    return ((idx ^ hi) << LOGW) + (w ^ lo);
 }
 
 // One radix-R Stockham pass on the 16 register elements: twiddle (if P > 1) and DFT.
@@ -117,7 +124,7 @@ __device__ __forceinline__ void pass_compute(float2 (&a)[16], float2 (&b)[16], c
             const int k = i & (P - 1);
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                const float2 t = __ldg(tw + (r - 1) * P + k);
+                const float2 t = tw[(r - 1) * P + k];
                 a[bb * R + r] = cmul(a[bb * R + r], t);
                 b[bb * R + r] = cmul(b[bb * R + r], t);
             }
@@ -127,7 +134,7 @@ __device__ __forceinline__ void pass_compute(float2 (&a)[16], float2 (&b)[16], c
     }
 }
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST>
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0>
 __device__ __forceinline__ void pass_store_smem(const float2 (&a)[16], const float2 (&b)[16], float4 *sm) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
@@ -136,11 +143,11 @@ __device__ __forceinline__ void pass_store_smem(const float2 (&a)[16], const flo
         PI::item(bb, i, w);
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            sm[sm_phys<LOGW>(PI::out_idx(i, r), w)] = make_float4(a[bb * R + r].x, a[bb * R + r].y, b[bb * R + r].x, b[bb * R + r].y);
+            sm[sm_phys<LOGW, LOGR0>(PI::out_idx(i, r), w)] = make_float4(a[bb * R + r].x, a[bb * R + r].y, b[bb * R + r].x, b[bb * R + r].y);
     }
 }
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST>
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0>
 __device__ __forceinline__ void pass_load_smem(float2 (&a)[16], float2 (&b)[16], const float4 *sm) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
@@ -148,99 +155,201 @@ __device__ __forceinline__ void pass_load_smem(float2 (&a)[16], float2 (&b)[16],
         int i, w;
         PI::item(bb, i, w);
 #pragma unroll
+        // in_idx = i + r*NI: when r*NI only touches idx bits the swizzle does not read, the
+        // address is base + r*NI*W (immediate offsets instead of per-element index math)
+        constexpr bool AFFINE = (LOGW >= 3) ? (PI::NI >= 8) : (PI::NI >= (1 << (LOGR0 + 3 - LOGW)));
+        const int base = sm_phys<LOGW, LOGR0>(i, w);
+#pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float4 v = sm[sm_phys<LOGW>(PI::in_idx(i, r), w)];
+            const float4 v = AFFINE ? sm[base + ((r * PI::NI) << LOGW)] : sm[sm_phys<LOGW, LOGR0>(PI::in_idx(i, r), w)];
             a[bb * R + r] = make_float2(v.x, v.y);
             b[bb * R + r] = make_float2(v.z, v.w);
         }
     }
 }
 
+
 struct FftArgs {
-    const float4 *S;          // [n_sky_slots][n_fft] per-sky resampled series
-    float4 *T;                // [n_inflight][n_fft] four-step intermediate
-    const TmplDesc *tmpl;     // descriptors of the templates of this launch (blockIdx.y indexes it)
+    const float4 *S;          // [n_sky_slots][n_fft] per-sky resampled series (zero beyond n_src)
+    float4 *T;                // [templates of this launch][n_fft] four-step intermediate
+    const TmplDesc *tmpl;     // descriptors of the templates of this launch
     const SkyABCD *abcd;      // [n_sky_slots]
-    float *twoF;              // output rows of this launch: row blockIdx.y
+    float *twoF;              // output rows of this launch
     int64_t twoF_stride;      // floats between rows
     const float2 *tw;         // twiddle table of this sub-FFT length
     int64_t n_fft, n_src, n_bins, k_margin;
     double dt;
     int log_other;            // log2 of the other factor (N2 for pass 1, N1 for pass 2)
+    int log_tiles;            // log2(tiles per template) = log_other - LOGW
+    int n_tiles;              // tiles_per_tmpl * templates in this launch
 };
+
+// exp(-2 pi i x) for a phase x in cycles held in fp64: reduce mod 1 in fp64, sincospif in fp32.
+__device__ __forceinline__ float2 expm2pi(double cyc) {
+    float sp, cp;
+    sincospif(-2.0f * (float)(cyc - rint(cyc)), &sp, &cp);
+    return make_float2(cp, sp);
+}
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+
+// Start the global -> shared copy of one tile: this thread copies exactly the 16 elements it
+// reads back itself in pass 0.  src points at element (row 0, lane 0) of the tile; rows are
+// 2^log_other elements apart.
+template <int LOGN>
+__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, int log_other) {
+    using C = FftCfg<LOGN>;
+    using RP = RadixPlan<LOGN>;
+    constexpr int LOGR0 = ilog2c(RP::r0);
+    using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
+#pragma unroll
+    for (int bb = 0; bb < PI::NB; ++bb) {
+        int i, w;
+        PI::item(bb, i, w);
+#pragma unroll
+        constexpr bool AFFINE = (C::LOGW >= 3) ? (PI::NI >= 8) : (PI::NI >= (1 << (LOGR0 + 3 - C::LOGW)));
+        const int base = sm_phys<C::LOGW, LOGR0>(i, w);
+        const float4 *g0 = src + ((int64_t)i << log_other) + w;
+#pragma unroll
+        for (int r = 0; r < RP::r0; ++r) {
+            const int idx = PI::in_idx(i, r);
+            cp_async16(sm + (AFFINE ? base + ((r * PI::NI) << C::LOGW) : sm_phys<C::LOGW, LOGR0>(idx, w)),
+                       g0 + ((int64_t)(r * PI::NI) << log_other));
+        }
+    }
+    cp_async_commit();
+}
+
+// Radix passes of one tile between "inputs of pass 0 are in registers" and "inputs of the last
+// pass are in registers and the exchange buffer is free again" (barrier included).
+// LASTMAP_IFAST selects the lane mapping of the last pass (pass 1 of the four-step wants
+// consecutive lanes on consecutive outputs m1 of one column; pass 2 on consecutive rows).
+template <int LOGN, bool LASTMAP_IFAST>
+__device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], float4 *sm, const float2 *__restrict__ tw) {
+    using C = FftCfg<LOGN>;
+    using RP = RadixPlan<LOGN>;
+    constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
+    constexpr bool LAST1 = (RP::np == 2);
+    __syncthreads();                                   // every thread has taken its pass-0 inputs
+    pass_compute<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, nullptr);
+    pass_store_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
+    __syncthreads();
+    pass_load_smem<RP::r1, C::P1, LOGN, LOGW, NT, LAST1 && LASTMAP_IFAST, LOGR0>(a, b, sm);
+    if (!LAST1) {
+        pass_compute<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, tw + C::OFF1);
+        __syncthreads();
+        pass_store_smem<RP::r1, C::P1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
+        __syncthreads();
+        pass_load_smem<RP::r2, C::P2, LOGN, LOGW, NT, LASTMAP_IFAST, LOGR0>(a, b, sm);
+    }
+    __syncthreads();                                   // buffer free: the next tile may be prefetched
+}
+
+template <int LOGN, bool LASTMAP_IFAST>
+__device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16], const float2 *__restrict__ tw) {
+    using C = FftCfg<LOGN>;
+    using RP = RadixPlan<LOGN>;
+    if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, LASTMAP_IFAST>(a, b, tw + C::OFF1);
+    else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, LASTMAP_IFAST>(a, b, tw + C::OFF2);
+}
 
 // ---------------------------------------------------------------------------------------
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
-// grid = (N2 / W, templates in this launch)
+// Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
 // ---------------------------------------------------------------------------------------
 template <int LOGN>
 __global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
-fft_pass1_kernel(FftArgs p) {
+fft_pass1_kernel(const __grid_constant__ FftArgs p) {
     using C = FftCfg<LOGN>;
     using RP = RadixPlan<LOGN>;
-    constexpr int LOGW = C::LOGW, NT = C::NT;
+    constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
     extern __shared__ float4 sm[];
-    const TmplDesc td = p.tmpl[blockIdx.y];
-    const float4 *__restrict__ S = p.S + (int64_t)td.sky_slot * p.n_fft;
-    float4 *__restrict__ T = p.T + (int64_t)blockIdx.y * p.n_fft;
-    const int k2_0 = blockIdx.x << LOGW;
+    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);
+    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];   // visible after the first barrier
     float2 a[16], b[16];
-
-    {   // pass 0 inputs from global memory, times exp(-i Phi_s) (S9)
-        using PI = PassIdx<RP::r0, 1, LOGN, LOGW, NT, false>;
+    int tile = blockIdx.x;
+    if (tile >= p.n_tiles) return;
+    {
+        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        tile_prefetch<LOGN>(sm, p.S + (int64_t)p.tmpl[t].sky_slot * p.n_fft + (x << LOGW), p.log_other);
+    }
+    for (; tile < p.n_tiles; tile += gridDim.x) {
+        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        const TmplDesc td = p.tmpl[t];
+        const int k2_0 = x << LOGW;
+        const int nxt = tile + gridDim.x;               // fetch the next tile's source slot early
+        const int sky_next = (nxt < p.n_tiles) ? p.tmpl[nxt >> p.log_tiles].sky_slot : 0;
+        cp_async_wait_all();
+        pass_load_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
+        {   // times exp(-i Phi_s) (S9).  The r0 inputs of one butterfly sit on an
+            // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic
+            // phi(tau) = tau^2 (c1 + c2 tau): its forward differences D1, D2 and the constant D3 are
+            // evaluated once per butterfly in fp64 (mod 1), and exp(-2 pi i phi(tau_r)) follows by the
+            // recurrence e_{r+1} = e_r d_r, d_{r+1} = d_r q_r, q_{r+1} = q_r c  (fp32 complex products).
+            using PI = PassIdx<RP::r0, 1, LOGN, LOGW, NT, false>;
+            const double h = (double)((int64_t)PI::NI << p.log_other) * p.dt;
+            const double c1 = td.half_fdot, c2 = td.sixth_fddot;
+            const bool cubic = (c2 != 0.0);
+            float2 cc = make_float2(1.f, 0.f);
+            if (cubic) cc = expm2pi(6.0 * c2 * h * h * h);
 #pragma unroll
-        for (int bb = 0; bb < PI::NB; ++bb) {
-            int i, w;
-            PI::item(bb, i, w);
+            for (int bb = 0; bb < PI::NB; ++bb) {
+                int i, w;
+                PI::item(bb, i, w);
+                const int64_t k = ((int64_t)i << p.log_other) + k2_0 + w;
+                const double tau = (double)(k - p.k_margin) * p.dt;
+                const double t3 = 3.0 * c2 * tau;
+                float2 e = expm2pi(tau * tau * fma(c2, tau, c1));
+                float2 d = expm2pi(h * (fma(2.0 * tau, c1, tau * t3) + h * (c1 + t3 + c2 * h)));
+                float2 q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
 #pragma unroll
-            for (int r = 0; r < RP::r0; ++r) {
-                const int64_t k = ((int64_t)PI::in_idx(i, r) << p.log_other) + k2_0 + w;
-                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (k < p.n_src) {
-                    v = __ldcg(S + k);
-                    const double tau = (double)(k - p.k_margin) * p.dt;
-                    const double cyc = tau * tau * fma(td.sixth_fddot, tau, td.half_fdot);
-                    float sp, cp;
-                    sincospif(-2.0f * (float)(cyc - rint(cyc)), &sp, &cp);
-                    v = make_float4(v.x * cp - v.y * sp, v.x * sp + v.y * cp, v.z * cp - v.w * sp, v.z * sp + v.w * cp);
+                for (int r = 0; r < RP::r0; ++r) {
+                    a[bb * RP::r0 + r] = cmul(a[bb * RP::r0 + r], e);
+                    b[bb * RP::r0 + r] = cmul(b[bb * RP::r0 + r], e);
+                    if (r + 1 < RP::r0) {
+                        e = cmul(e, d);
+                        d = cmul(d, q);
+                        if (cubic) q = cmul(q, cc);
+                    }
                 }
-                a[bb * RP::r0 + r] = make_float2(v.x, v.y);
-                b[bb * RP::r0 + r] = make_float2(v.z, v.w);
             }
         }
-    }
-    pass_compute<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, nullptr);
-    pass_store_smem<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, sm);
-    __syncthreads();
-    constexpr bool LAST1 = (RP::np == 2);
-    pass_load_smem<RP::r1, C::P1, LOGN, LOGW, NT, LAST1>(a, b, sm);
-    pass_compute<RP::r1, C::P1, LOGN, LOGW, NT, LAST1>(a, b, p.tw + C::OFF1);
-    if (!LAST1) {
-        __syncthreads();
-        pass_store_smem<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, sm);
-        __syncthreads();
-        pass_load_smem<RP::r2, C::P2, LOGN, LOGW, NT, true>(a, b, sm);
-        pass_compute<RP::r2, C::P2, LOGN, LOGW, NT, true>(a, b, p.tw + C::OFF2);
-    }
-    {   // last pass outputs: m1 = i + r*N1/R (consecutive lanes -> consecutive m1), times W_N^{k2 m1}
-        constexpr int RL = LAST1 ? RP::r1 : RP::r2;
-        constexpr int PL = LAST1 ? C::P1 : C::P2;
-        using PI = PassIdx<RL, PL, LOGN, LOGW, NT, true>;
-        const float inv_n = 1.0f / (float)p.n_fft;
+        tile_passes<LOGN, true>(a, b, sm, sm_tw);
+        if (nxt < p.n_tiles) {
+            const int x2 = nxt & ((1 << p.log_tiles) - 1);
+            tile_prefetch<LOGN>(sm, p.S + (int64_t)sky_next * p.n_fft + (x2 << LOGW), p.log_other);
+        }
+        tile_last_pass<LOGN, true>(a, b, sm_tw);
+        {   // outputs m1 = i + r*NI (consecutive lanes -> consecutive m1), times the four-step twiddle
+            // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r: two exact sincospif per butterfly, powers by products.
+            constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
+            constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
+            using PI = PassIdx<RL, PL, LOGN, LOGW, NT, true>;
+            float4 *__restrict__ T = p.T + (int64_t)t * p.n_fft;
+            const float inv_n = 1.0f / (float)p.n_fft;
+            const uint32_t nmask = (uint32_t)(p.n_fft - 1);
 #pragma unroll
-        for (int bb = 0; bb < PI::NB; ++bb) {
-            int i, w;
-            PI::item(bb, i, w);
-            const int k2 = k2_0 + w;
-#pragma unroll
-            for (int r = 0; r < RL; ++r) {
-                const int m1 = PI::out_idx(i, r);
-                const uint32_t t = ((uint32_t)k2 * (uint32_t)m1) & (uint32_t)(p.n_fft - 1);
+            for (int bb = 0; bb < PI::NB; ++bb) {
+                int i, w;
+                PI::item(bb, i, w);
+                const uint32_t k2 = (uint32_t)(k2_0 + w);
                 float sp, cp;
-                sincospif(-2.0f * ((float)t * inv_n), &sp, &cp);
-                const float2 tw = make_float2(cp, sp);
-                const float2 x = cmul(a[bb * RL + r], tw), y = cmul(b[bb * RL + r], tw);
-                __stcg(T + ((int64_t)k2 << LOGN) + m1, make_float4(x.x, x.y, y.x, y.y));
+                sincospif(-2.0f * ((float)((k2 * (uint32_t)i) & nmask) * inv_n), &sp, &cp);
+                float2 tw = make_float2(cp, sp);
+                sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
+                const float2 step = make_float2(cp, sp);
+                float4 *dst = T + ((int64_t)k2 << LOGN) + i;
+#pragma unroll
+                for (int r = 0; r < RL; ++r) {
+                    const float2 xx = cmul(a[bb * RL + r], tw), yy = cmul(b[bb * RL + r], tw);
+                    __stcg(dst + r * PI::NI, make_float4(xx.x, xx.y, yy.x, yy.y));
+                    if (r + 1 < RL) tw = cmul(tw, step);
+                }
             }
         }
     }
@@ -248,64 +357,57 @@ fft_pass1_kernel(FftArgs p) {
 
 // ---------------------------------------------------------------------------------------
 // Pass 2: row FFTs of length N2 = 2^LOGN + the 2F combination of eq. 8 (Fig. 1).
-// grid = (N1 / W, templates in this launch)
+// Persistent; tile = (template, W adjacent rows m1).
 // ---------------------------------------------------------------------------------------
 template <int LOGN>
 __global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
-fft_pass2_kernel(FftArgs p) {
+fft_pass2_kernel(const __grid_constant__ FftArgs p) {
     using C = FftCfg<LOGN>;
     using RP = RadixPlan<LOGN>;
-    constexpr int LOGW = C::LOGW, NT = C::NT;
+    constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
     extern __shared__ float4 sm[];
-    const TmplDesc td = p.tmpl[blockIdx.y];
-    const float4 *__restrict__ T = p.T + (int64_t)blockIdx.y * p.n_fft;
-    const int m1_0 = blockIdx.x << LOGW;
+    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);
+    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];   // visible after the first barrier
     float2 a[16], b[16];
+    int tile = blockIdx.x;
+    if (tile >= p.n_tiles) return;
     {
-        using PI = PassIdx<RP::r0, 1, LOGN, LOGW, NT, false>;
-#pragma unroll
-        for (int bb = 0; bb < PI::NB; ++bb) {
-            int i, w;
-            PI::item(bb, i, w);
-#pragma unroll
-            for (int r = 0; r < RP::r0; ++r) {
-                const float4 v = __ldcg(T + ((int64_t)PI::in_idx(i, r) << p.log_other) + m1_0 + w);
-                a[bb * RP::r0 + r] = make_float2(v.x, v.y);
-                b[bb * RP::r0 + r] = make_float2(v.z, v.w);
+        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        tile_prefetch<LOGN>(sm, p.T + (int64_t)t * p.n_fft + (x << LOGW), p.log_other);
+    }
+    for (; tile < p.n_tiles; tile += gridDim.x) {
+        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        const int m1_0 = x << LOGW;
+        cp_async_wait_all();
+        pass_load_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
+        tile_passes<LOGN, false>(a, b, sm, sm_tw);
+        {
+            const int nxt = tile + gridDim.x;
+            if (nxt < p.n_tiles) {
+                const int t2 = nxt >> p.log_tiles, x2 = nxt & ((1 << p.log_tiles) - 1);
+                tile_prefetch<LOGN>(sm, p.T + (int64_t)t2 * p.n_fft + (x2 << LOGW), p.log_other);
             }
         }
-    }
-    pass_compute<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, nullptr);
-    pass_store_smem<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, sm);
-    __syncthreads();
-    pass_load_smem<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, sm);
-    pass_compute<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, p.tw + C::OFF1);
-    constexpr bool LAST1 = (RP::np == 2);
-    if (!LAST1) {
-        __syncthreads();
-        pass_store_smem<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, sm);
-        __syncthreads();
-        pass_load_smem<RP::r2, C::P2, LOGN, LOGW, NT, false>(a, b, sm);
-        pass_compute<RP::r2, C::P2, LOGN, LOGW, NT, false>(a, b, p.tw + C::OFF2);
-    }
-    {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
-        constexpr int RL = LAST1 ? RP::r1 : RP::r2;
-        constexpr int PL = LAST1 ? C::P1 : C::P2;
-        using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
-        const SkyABCD ab = p.abcd[td.sky_slot];
-        float *__restrict__ out = p.twoF + (int64_t)blockIdx.y * p.twoF_stride;
+        tile_last_pass<LOGN, false>(a, b, sm_tw);
+        {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
+            constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
+            constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
+            using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
+            const SkyABCD ab = p.abcd[p.tmpl[t].sky_slot];
+            float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride;
 #pragma unroll
-        for (int bb = 0; bb < PI::NB; ++bb) {
-            int i, w;
-            PI::item(bb, i, w);
+            for (int bb = 0; bb < PI::NB; ++bb) {
+                int i, w;
+                PI::item(bb, i, w);
 #pragma unroll
-            for (int r = 0; r < RL; ++r) {
-                const int64_t q = ((int64_t)PI::out_idx(i, r) << p.log_other) + m1_0 + w;
-                if (q < p.n_bins) {
-                    const float2 fa = a[bb * RL + r], fb = b[bb * RL + r];
-                    const float twoF = ab.b_over_d * (fa.x * fa.x + fa.y * fa.y) + ab.a_over_d * (fb.x * fb.x + fb.y * fb.y)
-                                     - ab.two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
-                    __stcs(out + q, twoF);
+                for (int r = 0; r < RL; ++r) {
+                    const int64_t q = ((int64_t)PI::out_idx(i, r) << p.log_other) + m1_0 + w;
+                    if (q < p.n_bins) {
+                        const float2 fa = a[bb * RL + r], fb = b[bb * RL + r];
+                        const float twoF = ab.b_over_d * (fa.x * fa.x + fa.y * fa.y) + ab.a_over_d * (fb.x * fb.x + fb.y * fb.y)
+                                         - ab.two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
+                        __stcs(out + q, twoF);
+                    }
                 }
             }
         }

@@ -37,6 +37,7 @@ struct fstat_plan {
     fstat_ephem_t eph{};
     double f_min = 0, band = 0, df = 0;
     int device = 0;
+    int n_sm = 148;
     // device memory
     float2 *d_series = nullptr;
     float *d_wslot = nullptr;
@@ -153,28 +154,29 @@ void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *s
     }
 }
 
-template <int LOGN> int launch_pass1(fstat_plan *p, const FftArgs &a, int n_cols_blocks, int n_t) {
+// Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
+template <int LOGN, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN>;
     static thread_local int configured_dev = -1;
+    static thread_local int resident = 0;
+    auto kern = P2 ? fft_pass2_kernel<LOGN> : fft_pass1_kernel<LOGN>;
     if (configured_dev != p->device) {
-        CUDA_TRY(p, cudaFuncSetAttribute(fft_pass1_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        int per_sm = 0;
+        CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, C::SMEM_BYTES));
+        resident = (per_sm > 0 ? per_sm : 1) * p->n_sm;
         configured_dev = p->device;
     }
-    fft_pass1_kernel<LOGN><<<dim3(n_cols_blocks, n_t), C::NT, C::SMEM_BYTES, p->stream>>>(a);
+    a.log_tiles = ilog2(tiles_per_tmpl);
+    a.n_tiles = tiles_per_tmpl * n_t;
+    const int grid = a.n_tiles < resident ? a.n_tiles : resident;
+    kern<<<grid, C::NT, C::SMEM_BYTES, p->stream>>>(a);
     ++p->launches;
     return FSTAT_OK;
 }
-template <int LOGN> int launch_pass2(fstat_plan *p, const FftArgs &a, int n_row_blocks, int n_t) {
-    using C = FftCfg<LOGN>;
-    static thread_local int configured_dev = -1;
-    if (configured_dev != p->device) {
-        CUDA_TRY(p, cudaFuncSetAttribute(fft_pass2_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured_dev = p->device;
-    }
-    fft_pass2_kernel<LOGN><<<dim3(n_row_blocks, n_t), C::NT, C::SMEM_BYTES, p->stream>>>(a);
-    ++p->launches;
-    return FSTAT_OK;
-}
+template <int LOGN> int launch_pass1(fstat_plan *p, FftArgs &a, int tiles, int n_t) { return launch_pass<LOGN, false>(p, a, tiles, n_t); }
+template <int LOGN> int launch_pass2(fstat_plan *p, FftArgs &a, int tiles, int n_t) { return launch_pass<LOGN, true>(p, a, tiles, n_t); }
 
 #define DISPATCH_LOGN(logn, fn, ...)                         \
     switch (logn) {                                          \
@@ -471,6 +473,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     auto bail = [&](int code) { g_setup_error = p->err; destroy_impl(p); return code; };
 #define SETUP_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { p->err = std::string(#expr) + ": " + cudaGetErrorString(e__); return bail(e__ == cudaErrorMemoryAllocation ? FSTAT_ENOMEM : FSTAT_ECUDA); } } while (0)
     SETUP_TRY(cudaGetDevice(&p->device));
+    SETUP_TRY(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device));
     p->stream = (cudaStream_t)cuda_stream;
     PlanGeom &g = p->g;
     g.n_det = n_det; g.dterms = dterms; g.n_samples = n_samples; g.k_margin = km; g.n_src = n_samples + 2 * km;
