@@ -77,7 +77,7 @@ template <int LOGN> struct FftCfg {
     static constexpr int OFF1 = 0;
     static constexpr int OFF2 = (RadixPlan<LOGN>::r1 - 1) * P1;
     static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN>::np > 2 ? (RadixPlan<LOGN>::r2 - 1) * P2 : 0);
-    static constexpr int SMEM_BYTES = N * W * 16 + TW_ENTRIES * 8;   // exchange buffer + twiddle table
+    static constexpr int SMEM_BYTES = N * W * 16 + TW_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
 };
 
 // Shared-memory exchange layout: element idx of lane w lives at 16-byte chunk
@@ -170,8 +170,8 @@ __device__ __forceinline__ void pass_load_smem(float2 (&a)[16], float2 (&b)[16],
 
 
 struct FftArgs {
-    const float4 *S;          // [n_sky_slots][n_fft] per-sky resampled series (zero beyond n_src)
-    float4 *T;                // [templates of this launch][n_fft] four-step intermediate
+    const float4 *S;          // [n_sky_slots][n_fft] resampled series, tile-blocked: [k2/W1][k1][k2%W1]
+    float4 *T;                // [templates of this launch][n_fft] intermediate, tile-blocked: [m1/W2][k2][m1%W2]
     const TmplDesc *tmpl;     // descriptors of the templates of this launch
     const SkyABCD *abcd;      // [n_sky_slots]
     float *twoF;              // output rows of this launch
@@ -180,8 +180,9 @@ struct FftArgs {
     int64_t n_fft, n_src, n_bins, k_margin;
     double dt;
     int log_other;            // log2 of the other factor (N2 for pass 1, N1 for pass 2)
+    int log_w_other;          // log2 W of the other pass (layout of T)
     int log_tiles;            // log2(tiles per template) = log_other - LOGW
-    int n_tiles;              // tiles_per_tmpl * templates in this launch
+    int n_tiles;              // tiles per template * templates in this launch
 };
 
 // exp(-2 pi i x) for a phase x in cycles held in fp64: reduce mod 1 in fp64, sincospif in fp32.
@@ -191,45 +192,64 @@ __device__ __forceinline__ float2 expm2pi(double cyc) {
     return make_float2(cp, sp);
 }
 
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+// ---- mbarrier + 1-D bulk copy (TMA, cp.async.bulk -> SASS UBLKCP) ------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned done = 0;
+    while (!done) {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::
+                 "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src), "r"(bytes),
+                 "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
-// Start the global -> shared copy of one tile: this thread copies exactly the 16 elements it
-// reads back itself in pass 0.  src points at element (row 0, lane 0) of the tile; rows are
-// 2^log_other elements apart.
+// One thread starts the copy of a whole tile (contiguous in global memory thanks to the
+// tile-blocked layouts) into the exchange buffer; completion is signalled on the mbarrier.
 template <int LOGN>
-__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, int log_other) {
+__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, uint64_t *bar) {
+    using C = FftCfg<LOGN>;
+    constexpr unsigned BYTES = C::N * C::W * 16, CHUNK = 16384;
+    if (threadIdx.x == 0) {
+        fence_proxy_async();                      // earlier generic-proxy reads of the buffer are ordered before the async writes
+        mbar_expect_tx(bar, BYTES);
+#pragma unroll
+        for (unsigned o = 0; o < BYTES; o += CHUNK)
+            bulk_g2s(reinterpret_cast<char *>(sm) + o, reinterpret_cast<const char *>(src) + o, CHUNK, bar);
+    }
+}
+
+// Pass-0 inputs out of the staging layout (linear: element idx of lane w at idx*W + w).
+template <int LOGN>
+__device__ __forceinline__ void tile_take_inputs(float2 (&a)[16], float2 (&b)[16], const float4 *sm) {
     using C = FftCfg<LOGN>;
     using RP = RadixPlan<LOGN>;
-    constexpr int LOGR0 = ilog2c(RP::r0);
     using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
 #pragma unroll
     for (int bb = 0; bb < PI::NB; ++bb) {
-        int i, w;
-        PI::item(bb, i, w);
-#pragma unroll
-        constexpr bool AFFINE = (C::LOGW >= 3) ? (PI::NI >= 8) : (PI::NI >= (1 << (LOGR0 + 3 - C::LOGW)));
-        const int base = sm_phys<C::LOGW, LOGR0>(i, w);
-        const float4 *g0 = src + ((int64_t)i << log_other) + w;
+        const int g = threadIdx.x + bb * C::NT;   // = i*W + w
 #pragma unroll
         for (int r = 0; r < RP::r0; ++r) {
-            const int idx = PI::in_idx(i, r);
-            cp_async16(sm + (AFFINE ? base + ((r * PI::NI) << C::LOGW) : sm_phys<C::LOGW, LOGR0>(idx, w)),
-                       g0 + ((int64_t)(r * PI::NI) << log_other));
+            const float4 v = sm[g + ((r * PI::NI) << C::LOGW)];
+            a[bb * RP::r0 + r] = make_float2(v.x, v.y);
+            b[bb * RP::r0 + r] = make_float2(v.z, v.w);
         }
     }
-    cp_async_commit();
 }
 
 // Radix passes of one tile between "inputs of pass 0 are in registers" and "inputs of the last
 // pass are in registers and the exchange buffer is free again" (barrier included).
-// LASTMAP_IFAST selects the lane mapping of the last pass (pass 1 of the four-step wants
-// consecutive lanes on consecutive outputs m1 of one column; pass 2 on consecutive rows).
-template <int LOGN, bool LASTMAP_IFAST>
+template <int LOGN>
 __device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], float4 *sm, const float2 *__restrict__ tw) {
     using C = FftCfg<LOGN>;
     using RP = RadixPlan<LOGN>;
@@ -239,24 +259,42 @@ __device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], fl
     pass_compute<RP::r0, 1, LOGN, LOGW, NT, false>(a, b, nullptr);
     pass_store_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
     __syncthreads();
-    pass_load_smem<RP::r1, C::P1, LOGN, LOGW, NT, LAST1 && LASTMAP_IFAST, LOGR0>(a, b, sm);
+    pass_load_smem<RP::r1, C::P1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
     if (!LAST1) {
         pass_compute<RP::r1, C::P1, LOGN, LOGW, NT, false>(a, b, tw + C::OFF1);
         __syncthreads();
         pass_store_smem<RP::r1, C::P1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
         __syncthreads();
-        pass_load_smem<RP::r2, C::P2, LOGN, LOGW, NT, LASTMAP_IFAST, LOGR0>(a, b, sm);
+        pass_load_smem<RP::r2, C::P2, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
     }
     __syncthreads();                                   // buffer free: the next tile may be prefetched
 }
 
-template <int LOGN, bool LASTMAP_IFAST>
+template <int LOGN>
 __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16], const float2 *__restrict__ tw) {
     using C = FftCfg<LOGN>;
     using RP = RadixPlan<LOGN>;
-    if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, LASTMAP_IFAST>(a, b, tw + C::OFF1);
-    else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, LASTMAP_IFAST>(a, b, tw + C::OFF2);
+    if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
+    else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
 }
+
+// Common kernel preamble: shared-memory carve-up, twiddles to shared memory, mbarrier init.
+#define FFT_KERNEL_PREAMBLE()                                                                     \
+    using C = FftCfg<LOGN>;                                                                       \
+    using RP = RadixPlan<LOGN>;                                                                   \
+    constexpr int LOGW = C::LOGW, NT = C::NT;                                                     \
+    extern __shared__ float4 sm[];                                                                \
+    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);                                 \
+    uint64_t *bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_ENTRIES);                          \
+    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];                     \
+    if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }                             \
+    __syncthreads();                                                                              \
+    float2 a[16], b[16];                                                                          \
+    unsigned parity = 0;                                                                          \
+    int tile = blockIdx.x;                                                                        \
+    if (tile >= p.n_tiles) return;                                                                \
+    const int tile_mask = (1 << p.log_tiles) - 1;                                                 \
+    constexpr int TILE_ELEMS = C::N * C::W
 
 // ---------------------------------------------------------------------------------------
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
@@ -265,27 +303,17 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16],
 template <int LOGN>
 __global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
-    using C = FftCfg<LOGN>;
-    using RP = RadixPlan<LOGN>;
-    constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
-    extern __shared__ float4 sm[];
-    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);
-    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];   // visible after the first barrier
-    float2 a[16], b[16];
-    int tile = blockIdx.x;
-    if (tile >= p.n_tiles) return;
-    {
-        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
-        tile_prefetch<LOGN>(sm, p.S + (int64_t)p.tmpl[t].sky_slot * p.n_fft + (x << LOGW), p.log_other);
-    }
+    FFT_KERNEL_PREAMBLE();
+    tile_prefetch<LOGN>(sm, p.S + (int64_t)p.tmpl[tile >> p.log_tiles].sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar);
     for (; tile < p.n_tiles; tile += gridDim.x) {
-        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const TmplDesc td = p.tmpl[t];
         const int k2_0 = x << LOGW;
         const int nxt = tile + gridDim.x;               // fetch the next tile's source slot early
         const int sky_next = (nxt < p.n_tiles) ? p.tmpl[nxt >> p.log_tiles].sky_slot : 0;
-        cp_async_wait_all();
-        pass_load_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
+        mbar_wait(bar, parity);
+        parity ^= 1;
+        tile_take_inputs<LOGN>(a, b, sm);
         {   // times exp(-i Phi_s) (S9).  The r0 inputs of one butterfly sit on an
             // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic
             // phi(tau) = tau^2 (c1 + c2 tau): its forward differences D1, D2 and the constant D3 are
@@ -319,20 +347,21 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 }
             }
         }
-        tile_passes<LOGN, true>(a, b, sm, sm_tw);
-        if (nxt < p.n_tiles) {
-            const int x2 = nxt & ((1 << p.log_tiles) - 1);
-            tile_prefetch<LOGN>(sm, p.S + (int64_t)sky_next * p.n_fft + (x2 << LOGW), p.log_other);
-        }
-        tile_last_pass<LOGN, true>(a, b, sm_tw);
-        {   // outputs m1 = i + r*NI (consecutive lanes -> consecutive m1), times the four-step twiddle
-            // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r: two exact sincospif per butterfly, powers by products.
+        tile_passes<LOGN>(a, b, sm, sm_tw);
+        if (nxt < p.n_tiles)
+            tile_prefetch<LOGN>(sm, p.S + (int64_t)sky_next * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar);
+        tile_last_pass<LOGN>(a, b, sm_tw);
+        {   // outputs m1 = i + r*NI of column k2 = k2_0 + w, times the four-step twiddle
+            // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r (two exact sincospif per butterfly, powers by
+            // products), stored tile-blocked for pass 2: T[m1 / W2][k2][m1 % W2] -- consecutive lanes
+            // (w, then i) fill whole 128-byte lines.
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
             constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
-            using PI = PassIdx<RL, PL, LOGN, LOGW, NT, true>;
+            using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
             float4 *__restrict__ T = p.T + (int64_t)t * p.n_fft;
             const float inv_n = 1.0f / (float)p.n_fft;
             const uint32_t nmask = (uint32_t)(p.n_fft - 1);
+            const int lw2 = p.log_w_other, ln2 = p.log_other;
 #pragma unroll
             for (int bb = 0; bb < PI::NB; ++bb) {
                 int i, w;
@@ -343,11 +372,17 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 float2 tw = make_float2(cp, sp);
                 sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
                 const float2 step = make_float2(cp, sp);
-                float4 *dst = T + ((int64_t)k2 << LOGN) + i;
+                float4 *colbase = T + ((int64_t)k2 << lw2);
+                float4 *dst = colbase + ((int64_t)(i >> lw2) << (ln2 + lw2)) + (i & ((1 << lw2) - 1));
+                const int64_t rstride = (int64_t)PI::NI << ln2;           // valid when NI is a multiple of W2
+                const bool affine = (PI::NI >> lw2) != 0;
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
                     const float2 xx = cmul(a[bb * RL + r], tw), yy = cmul(b[bb * RL + r], tw);
-                    __stcg(dst + r * PI::NI, make_float4(xx.x, xx.y, yy.x, yy.y));
+                    const int m1 = i + r * PI::NI;
+                    float4 *o = affine ? dst + r * rstride
+                                       : colbase + ((int64_t)(m1 >> lw2) << (ln2 + lw2)) + (m1 & ((1 << lw2) - 1));
+                    __stcg(o, make_float4(xx.x, xx.y, yy.x, yy.y));
                     if (r + 1 < RL) tw = cmul(tw, step);
                 }
             }
@@ -357,43 +392,29 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
 
 // ---------------------------------------------------------------------------------------
 // Pass 2: row FFTs of length N2 = 2^LOGN + the 2F combination of eq. 8 (Fig. 1).
-// Persistent; tile = (template, W adjacent rows m1).
+// Persistent; tile = (template, W adjacent rows m1) = one contiguous block of T.
 // ---------------------------------------------------------------------------------------
 template <int LOGN>
 __global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
 fft_pass2_kernel(const __grid_constant__ FftArgs p) {
-    using C = FftCfg<LOGN>;
-    using RP = RadixPlan<LOGN>;
-    constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
-    extern __shared__ float4 sm[];
-    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);
-    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];   // visible after the first barrier
-    float2 a[16], b[16];
-    int tile = blockIdx.x;
-    if (tile >= p.n_tiles) return;
-    {
-        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
-        tile_prefetch<LOGN>(sm, p.T + (int64_t)t * p.n_fft + (x << LOGW), p.log_other);
-    }
+    FFT_KERNEL_PREAMBLE();
+    tile_prefetch<LOGN>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar);
     for (; tile < p.n_tiles; tile += gridDim.x) {
-        const int t = tile >> p.log_tiles, x = tile & ((1 << p.log_tiles) - 1);
+        const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const int m1_0 = x << LOGW;
-        cp_async_wait_all();
-        pass_load_smem<RP::r0, 1, LOGN, LOGW, NT, false, LOGR0>(a, b, sm);
-        tile_passes<LOGN, false>(a, b, sm, sm_tw);
-        {
-            const int nxt = tile + gridDim.x;
-            if (nxt < p.n_tiles) {
-                const int t2 = nxt >> p.log_tiles, x2 = nxt & ((1 << p.log_tiles) - 1);
-                tile_prefetch<LOGN>(sm, p.T + (int64_t)t2 * p.n_fft + (x2 << LOGW), p.log_other);
-            }
-        }
-        tile_last_pass<LOGN, false>(a, b, sm_tw);
+        const int nxt = tile + gridDim.x;
+        const SkyABCD ab = p.abcd[p.tmpl[t].sky_slot];
+        mbar_wait(bar, parity);
+        parity ^= 1;
+        tile_take_inputs<LOGN>(a, b, sm);
+        tile_passes<LOGN>(a, b, sm, sm_tw);
+        if (nxt < p.n_tiles)
+            tile_prefetch<LOGN>(sm, p.T + (int64_t)(nxt >> p.log_tiles) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar);
+        tile_last_pass<LOGN>(a, b, sm_tw);
         {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
             constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
             using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
-            const SkyABCD ab = p.abcd[p.tmpl[t].sky_slot];
             float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride;
 #pragma unroll
             for (int bb = 0; bb < PI::NB; ++bb) {

@@ -200,10 +200,10 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
     a.dt = p->g.dt;
     int rc = FSTAT_OK;
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
-    a.tw = p->d_tw1; a.log_other = l2;
+    a.tw = p->d_tw1; a.log_other = l2; a.log_w_other = p->g.log_w2;
     { ProfScope ps(p, 1); DISPATCH_LOGN(l1, launch_pass1, p, a, (1 << l2) / tile_w(l1), nt); }
     if (rc) return rc;
-    a.tw = p->d_tw2; a.log_other = l1;
+    a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
     { ProfScope ps(p, 2); DISPATCH_LOGN(l2, launch_pass2, p, a, (1 << l1) / tile_w(l2), nt); }
     if (rc) return rc;
     CUDA_TRY(p, cudaGetLastError());
@@ -211,11 +211,11 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
 }
 
 // Sky-dependent kernels for sky groups [g0, g0+ng) -> S slots 0..ng-1, abcd slots 0..ng-1.
-int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst) {
+int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) {
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
     dim3 grid((unsigned)((g.n_src + 255) / 256), ng);
-    sky_resample_kernel<<<grid, 256, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst);
+    sky_resample_kernel<<<grid, 256, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
     dim3 grid2(p->abc_nblk, ng);
     sky_abc_partial_kernel<<<grid2, ABC_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_wslot, p->d_abc_partial);
     sky_abc_finalize_kernel<<<ng, 256, 0, p->stream>>>(p->d_abc_partial, p->abc_nblk, p->d_abcd, p->d_err);
@@ -343,7 +343,7 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
 
     for (size_t gb = 0; gb < groups.size(); gb += p->n_sky_slots) {
         const int ng = (int)std::min<size_t>(p->n_sky_slots, groups.size() - gb);
-        rc = launch_sky_batch(p, (int)gb, ng, p->d_S);
+        rc = launch_sky_batch(p, (int)gb, ng, p->d_S, 1);
         if (rc) return rc;
         const int t_begin = groups[gb].first;
         const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
@@ -398,11 +398,19 @@ void destroy_impl(fstat_plan *p) {
 }
 
 int default_inflight(int64_t n_fft) {
-    // keep the four-step intermediates of one launch within ~32 MB (L2-resident beside the source)
-    int64_t tb = (32ll << 20) / (n_fft * 16);
+    // templates per persistent launch: enough tiles (>= ~14 per resident CTA) that the last,
+    // partly filled round of tiles costs ~1 %, bounded by 256 MB of four-step intermediates
+    int64_t tb = (256ll << 20) / (n_fft * 16);
     if (tb < 1) tb = 1;
     if (tb > 64) tb = 64;
     return (int)tb;
+}
+
+int default_sky_slots(int64_t n_fft) {
+    int64_t s = (64ll << 20) / (n_fft * 16);
+    if (s < 1) s = 1;
+    if (s > 32) s = 32;
+    return (int)s;
 }
 
 }  // namespace
@@ -483,7 +491,8 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     const long long shift = llround((f_min - f_het) * (double)n_fft * dt);
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
     const int L = ilog2(n_fft);
-    g.log_n1 = L / 2; g.log_n2 = L - g.log_n1;
+    g.log_n2 = L / 2; g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
+    g.log_w1 = ilog2(tile_w(g.log_n1)); g.log_w2 = ilog2(tile_w(g.log_n2));
     p->eph = *eph; p->f_min = f_min; p->band = band; p->df = 1.0 / ((double)n_fft * dt);
     for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
     for (int m = -dterms; m <= dterms; ++m) {
@@ -507,7 +516,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     SETUP_TRY(cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     p->n_inflight = default_inflight(n_fft);
-    p->n_sky_slots = default_inflight(n_fft);
+    p->n_sky_slots = default_sky_slots(n_fft);
     SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
     SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
     SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
@@ -580,7 +589,7 @@ int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta, float *S_
     CUDA_TRY(plan, cudaMemcpyAsync(plan->d_sky, plan->h_sky, sizeof(SkyConst), cudaMemcpyHostToDevice, plan->stream));
     CUDA_TRY(plan, cudaEventRecord(plan->staging_ev, plan->stream));
     CUDA_TRY(plan, cudaMemsetAsync(S_dev, 0, (size_t)plan->g.n_fft * sizeof(float4), plan->stream));
-    rc = launch_sky_batch(plan, 0, 1, (float4 *)S_dev);
+    rc = launch_sky_batch(plan, 0, 1, (float4 *)S_dev, 0);
     if (rc) return rc;
     SkyABCD r;
     CUDA_TRY(plan, cudaMemcpyAsync(&r, plan->d_abcd, sizeof(SkyABCD), cudaMemcpyDeviceToHost, plan->stream));

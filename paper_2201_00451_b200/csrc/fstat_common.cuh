@@ -50,5 +50,6 @@ struct PlanGeom {
     double f_het;
     double omega_orb, phi_orb0, omega_rot, gmst0;
     uint32_t shift_mod;     // (round((f_min - f_het)/df)) mod n_fft
-    int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2
+    int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2 (log_n1 >= log_n2)
+    int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
 };

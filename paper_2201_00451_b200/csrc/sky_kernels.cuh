@@ -63,11 +63,13 @@ __device__ __forceinline__ void antenna_ab(const SkyConst &sc, int X, float cth,
 // H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
 //   series : [n_det][series_stride] float2, data starts at +SERIES_PAD (zeros around it)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
-//   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0)
+//   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
+//            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
+//            S[k2 / W1][k1][k2 % W1]
 __global__ void __launch_bounds__(256)
 sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ WinTable win,
                     const SkyConst *__restrict__ skies, const float2 *__restrict__ series,
-                    const float *__restrict__ wslot, float4 *__restrict__ S) {
+                    const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= g.n_src) return;
     const SkyConst &sc = skies[blockIdx.y];
@@ -121,7 +123,12 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
         yar = fmaf(w * a, er, yar); yai = fmaf(w * a, ei, yai);
         ybr = fmaf(w * b, er, ybr); ybi = fmaf(w * b, ei, ybi);
     }
-    S[(int64_t)blockIdx.y * g.n_fft + k] = make_float4(yar, yai, ybr, ybi);
+    int64_t off = k;
+    if (blocked) {
+        const int64_t k1 = k >> g.log_n2, k2 = k & (((int64_t)1 << g.log_n2) - 1);
+        off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
+    }
+    S[(int64_t)blockIdx.y * g.n_fft + off] = make_float4(yar, yai, ybr, ybi);
 }
 
 // A, B, C (eq. 8): sums of w a^2, w b^2, w a b over the valid detector-frame samples.
