@@ -5,7 +5,7 @@
 //   pass 1 (one CTA = W adjacent columns k2):   T[k2][m1] = W_N^{k2 m1} sum_k1 y[N2 k1 + k2] W_N1^{k1 m1}
 //   pass 2 (one CTA = W adjacent rows   m1):    X[m1 + N1 m2] = sum_k2 T[k2][m1] W_N2^{k2 m2}
 //
-// An element is a float4 = (Re Fa, Im Fa, Re Fb, Im Fb): both transforms run in lock step and
+// An element is a float4 = (Re Fa, Re Fb, Im Fa, Im Fb): both transforms run in lock step and
 // share every twiddle.  Each thread keeps 16 elements in registers; shared memory is the exchange
 // buffer between radix passes (one buffer, two barriers per exchange).  CTAs are persistent: each
 // loops over tiles, and as soon as the last radix pass of a tile has pulled its inputs out of
@@ -16,43 +16,56 @@
 #pragma once
 #include "fstat_common.cuh"
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
+// a register pair holds (Re Fa, Re Fb) or (Im Fa, Im Fb) and every add / multiply / FMA is one
+// Blackwell f32x2 instruction (SASS FADD2 / FMUL2 / FFMA2) with the twiddle as a broadcast scalar.
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 mul2s(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 fma2s(float2 a, float s, float2 c) { return __ffma2_rn(a, make_float2(s, s), c); }
+// scalar complex product (twiddle recurrences)
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
     return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
-
-// o * exp(-2 pi i j/16), j = 0..7, with the trivial cases spelled out (j is a compile-time
-// constant after unrolling).
-__device__ __forceinline__ float2 mul_w16(float2 o, int j) {
-    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
-    switch (j) {
-        case 0: return o;
-        case 1: return make_float2(fmaf(o.x, c1, o.y * s1), fmaf(o.y, c1, -o.x * s1));
-        case 2: return make_float2((o.x + o.y) * h, (o.y - o.x) * h);
-        case 3: return make_float2(fmaf(o.x, s1, o.y * c1), fmaf(o.y, s1, -o.x * c1));
-        case 4: return make_float2(o.y, -o.x);
-        case 5: return make_float2(fmaf(-o.x, s1, o.y * c1), fmaf(-o.y, s1, -o.x * c1));
-        case 6: return make_float2((o.y - o.x) * h, -(o.x + o.y) * h);
-        default: return make_float2(fmaf(-o.x, c1, o.y * s1), fmaf(-o.y, c1, -o.x * s1));
-    }
+// (x + i y) * (t.x + i t.y) on a packed pair
+__device__ __forceinline__ void pcmul(float2 &x, float2 &y, float2 t) {
+    const float2 nx = fma2s(x, t.x, mul2s(y, -t.y));
+    const float2 ny = fma2s(x, t.y, mul2s(y, t.x));
+    x = nx; y = ny;
 }
 
-// In-place forward DFT of length R (kernel exp(-2 pi i rq/R)), natural order in and out.
-template <int R> __device__ __forceinline__ void dft(float2 *v) {
-    float2 e[R / 2], o[R / 2];
+// (ox + i oy) * exp(-2 pi i j/16), j = 0..7 (j is a compile-time constant after unrolling).
+__device__ __forceinline__ void mul_w16(float2 &ox, float2 &oy, int j) {
+    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
+    float2 tx, ty;
+    switch (j) {
+        case 0: return;
+        case 1: tx = fma2s(ox, c1, mul2s(oy, s1)); ty = fma2s(oy, c1, mul2s(ox, -s1)); break;
+        case 2: tx = mul2s(add2(ox, oy), h); ty = mul2s(sub2(oy, ox), h); break;
+        case 3: tx = fma2s(ox, s1, mul2s(oy, c1)); ty = fma2s(oy, s1, mul2s(ox, -c1)); break;
+        case 4: tx = oy; ty = make_float2(-ox.x, -ox.y); break;
+        case 5: tx = fma2s(ox, -s1, mul2s(oy, c1)); ty = fma2s(oy, -s1, mul2s(ox, -c1)); break;
+        case 6: tx = mul2s(sub2(oy, ox), h); ty = mul2s(add2(ox, oy), -h); break;
+        default: tx = fma2s(ox, -c1, mul2s(oy, s1)); ty = fma2s(oy, -c1, mul2s(ox, -s1)); break;
+    }
+    ox = tx; oy = ty;
+}
+
+// In-place forward DFT of length R (kernel exp(-2 pi i rq/R)) on packed pairs, natural order.
+template <int R> __device__ __forceinline__ void dft(float2 *x, float2 *y) {
+    float2 ex[R / 2], ey[R / 2], ox[R / 2], oy[R / 2];
 #pragma unroll
-    for (int q = 0; q < R / 2; ++q) { e[q] = v[2 * q]; o[q] = v[2 * q + 1]; }
-    dft<R / 2>(e);
-    dft<R / 2>(o);
+    for (int q = 0; q < R / 2; ++q) { ex[q] = x[2 * q]; ey[q] = y[2 * q]; ox[q] = x[2 * q + 1]; oy[q] = y[2 * q + 1]; }
+    dft<R / 2>(ex, ey);
+    dft<R / 2>(ox, oy);
 #pragma unroll
     for (int k = 0; k < R / 2; ++k) {
-        const float2 t = mul_w16(o[k], k * (16 / R));
-        v[k] = cadd(e[k], t);
-        v[k + R / 2] = csub(e[k], t);
+        mul_w16(ox[k], oy[k], k * (16 / R));
+        x[k] = add2(ex[k], ox[k]); y[k] = add2(ey[k], oy[k]);
+        x[k + R / 2] = sub2(ex[k], ox[k]); y[k + R / 2] = sub2(ey[k], oy[k]);
     }
 }
-template <> __device__ __forceinline__ void dft<1>(float2 *) {}
+template <> __device__ __forceinline__ void dft<1>(float2 *, float2 *) {}
 
 // Radix plan per sub-FFT length 2^LOGN (16 register elements per thread).
 template <int LOGN> struct RadixPlan;
@@ -124,13 +137,10 @@ __device__ __forceinline__ void pass_compute(float2 (&a)[16], float2 (&b)[16], c
             const int k = i & (P - 1);
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                const float2 t = tw[(r - 1) * P + k];
-                a[bb * R + r] = cmul(a[bb * R + r], t);
-                b[bb * R + r] = cmul(b[bb * R + r], t);
+                pcmul(a[bb * R + r], b[bb * R + r], tw[(r - 1) * P + k]);
             }
         }
-        dft<R>(&a[bb * R]);
-        dft<R>(&b[bb * R]);
+        dft<R>(&a[bb * R], &b[bb * R]);
     }
 }
 
@@ -337,8 +347,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 float2 q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
 #pragma unroll
                 for (int r = 0; r < RP::r0; ++r) {
-                    a[bb * RP::r0 + r] = cmul(a[bb * RP::r0 + r], e);
-                    b[bb * RP::r0 + r] = cmul(b[bb * RP::r0 + r], e);
+                    pcmul(a[bb * RP::r0 + r], b[bb * RP::r0 + r], e);
                     if (r + 1 < RP::r0) {
                         e = cmul(e, d);
                         d = cmul(d, q);
@@ -378,7 +387,8 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 const bool affine = (PI::NI >> lw2) != 0;
 #pragma unroll
                 for (int r = 0; r < RL; ++r) {
-                    const float2 xx = cmul(a[bb * RL + r], tw), yy = cmul(b[bb * RL + r], tw);
+                    float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
+                    pcmul(xx, yy, tw);
                     const int m1 = i + r * PI::NI;
                     float4 *o = affine ? dst + r * rstride
                                        : colbase + ((int64_t)(m1 >> lw2) << (ln2 + lw2)) + (m1 & ((1 << lw2) - 1));
@@ -424,7 +434,8 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
                 for (int r = 0; r < RL; ++r) {
                     const int64_t q = ((int64_t)PI::out_idx(i, r) << p.log_other) + m1_0 + w;
                     if (q < p.n_bins) {
-                        const float2 fa = a[bb * RL + r], fb = b[bb * RL + r];
+                        const float2 fa = make_float2(a[bb * RL + r].x, b[bb * RL + r].x);    // unpack (re, im) of Fa, Fb
+                        const float2 fb = make_float2(a[bb * RL + r].y, b[bb * RL + r].y);
                         const float twoF = ab.b_over_d * (fa.x * fa.x + fa.y * fa.y) + ab.a_over_d * (fb.x * fb.x + fb.y * fb.y)
                                          - ab.two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
                         __stcs(out + q, twoF);

@@ -128,7 +128,8 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
         const int64_t k1 = k >> g.log_n2, k2 = k & (((int64_t)1 << g.log_n2) - 1);
         off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
     }
-    S[(int64_t)blockIdx.y * g.n_fft + off] = make_float4(yar, yai, ybr, ybi);
+    // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
+    S[(int64_t)blockIdx.y * g.n_fft + off] = blocked ? make_float4(yar, ybr, yai, ybi) : make_float4(yar, yai, ybr, ybi);
 }
 
 // A, B, C (eq. 8): sums of w a^2, w b^2, w a b over the valid detector-frame samples.
