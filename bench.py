@@ -194,12 +194,20 @@ def run_ours(args):
     if args.inflight:
         plan.set_inflight(args.inflight)
     n_t, nb = len(p.templates), plan.n_bins
-    out = torch.empty((n_t, nb), dtype=torch.float32, device="cuda")
+    topk = args.mode == "topk"
+    if topk:                      # config-4 style: only the k loudest bins of every template leave the GPU
+        out = (torch.empty((n_t, args.k), dtype=torch.float32, device="cuda"),
+               torch.empty((n_t, args.k), dtype=torch.int32, device="cuda"))
+    else:
+        out = torch.empty((n_t, nb), dtype=torch.float32, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     def step():
-        plan.compute(p.templates, out=out)
+        if topk:
+            plan.compute_topk(p.templates, args.k, out=out)
+        else:
+            plan.compute(p.templates, out=out)
 
     for _ in range(args.warmup):
         step()
@@ -247,6 +255,7 @@ def run_ours(args):
                             "algorithmic_bytes_per_template": bytes_per_t,
                             "achieved_gbs": tot_bytes / (ms * 1e-3) / 1e9 if ms > 0 else None}
         kernels["sky"] = {"ms_total": prof["sky"][0], "launches": prof["sky"][1]}
+        kernels["topk"] = {"ms_total": prof["topk"][0], "launches": prof["topk"][1]}
         dom = max(("fft_pass1", "fft_pass2"), key=lambda c: prof[c][0])
         ach = kernels[dom]["achieved_gbs"]
         both = (b1 + b2) * n_t * args.steps / ((prof["fft_pass1"][0] + prof["fft_pass2"][0]) * 1e-3) / 1e9
@@ -258,13 +267,24 @@ def run_ours(args):
     # ---- end to end through the host-buffer entry point (pinned host 2F, D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
-        host_out = torch.empty((n_t, nb), dtype=torch.float32, pin_memory=True)
-        plan.compute_host(p.templates, out=host_out)                  # warm-up (allocates the device ring)
+        if topk:
+            def e2e_step():
+                return plan.compute_topk_host(p.templates, args.k)    # blocks until (val, bin) are in host memory
+            d2h = n_t * args.k * 8
+            api = "fstat_compute_topk_host (host templates in, host top-k values + bins out)"
+        else:
+            host_out = torch.empty((n_t, nb), dtype=torch.float32, pin_memory=True)
+
+            def e2e_step():
+                return plan.compute_host(p.templates, out=host_out)   # blocks until the rows have landed
+            d2h = n_t * nb * 4
+            api = "fstat_compute_host (host templates in, pinned host 2F[n_tmpl][n_bins] out)"
+        e2e_step()                                                    # warm-up (allocates the device ring)
         n_e2e = max(1, min(args.steps, 3))
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            plan.compute_host(p.templates, out=host_out)              # blocks until the rows have landed
+            e2e_step()
         torch.cuda.synchronize()
         e_ms = 1e3 * (time.perf_counter() - t0) / n_e2e
         if world > 1:
@@ -272,10 +292,8 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e_ms = float(t.item())
         e2e = {"value": world * n_t * nb / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": n_e2e,
-               "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(n_t * nb * 4),
-               "api": "fstat_compute_host (host templates in, pinned host 2F[n_tmpl][n_bins] out); the series is uploaded once "
-                      "by fstat_setup (PAPER.md:93) and is not part of a step"}
-        del host_out
+               "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(d2h),
+               "api": api + "; the series is uploaded once by fstat_setup (PAPER.md:93) and is not part of a step"}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -288,7 +306,8 @@ def run_ours(args):
                 "templates_per_s": world * n_t / (ms_per_step * 1e-3),
                 "tau_eff_s_per_bin_per_detector": ms_per_step * 1e-3 / (n_t * nb * p.n_det),
                 "config": {"workload": args.workload, "n_det": p.n_det, "n_samples": p.n_samples, "dt": p.dt, "n_fft": p.n_fft,
-                           "n_bins": nb, "n_templates": n_t, "dterms": p.dterms, "multi_gpu": "independent replicas, no collective",
+                           "n_bins": nb, "n_templates": n_t, "dterms": p.dterms,
+                           "output": f"top-{args.k} per template" if topk else "full 2F[n_templates][n_bins]", "multi_gpu": "independent replicas, no collective",
                            "l2": "256 MiB flush buffer written between timed steps; each step also writes "
                                  f"{n_t * nb * 4 / 1e9:.2f} GB of 2F (> L2)"},
                 "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
@@ -307,6 +326,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--mode", default="full", choices=["full", "topk"])
+    ap.add_argument("--k", type=int, default=8)
     ap.add_argument("--cpu-templates", type=int, default=8)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

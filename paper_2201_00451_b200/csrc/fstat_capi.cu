@@ -214,8 +214,10 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
 int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) {
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
-    dim3 grid((unsigned)((g.n_src + 255) / 256), ng);
-    sky_resample_kernel<<<grid, 256, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
+    dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
+    if (g.dterms == 8) sky_resample_kernel<8><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
+    else if (g.dterms == 16) sky_resample_kernel<16><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
+    else sky_resample_kernel<0><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
     dim3 grid2(p->abc_nblk, ng);
     sky_abc_partial_kernel<<<grid2, ABC_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_wslot, p->d_abc_partial);
     sky_abc_finalize_kernel<<<ng, 256, 0, p->stream>>>(p->d_abc_partial, p->abc_nblk, p->d_abcd, p->d_err);
@@ -398,11 +400,15 @@ void destroy_impl(fstat_plan *p) {
 }
 
 int default_inflight(int64_t n_fft) {
-    // templates per persistent launch: enough tiles (>= ~14 per resident CTA) that the last,
-    // partly filled round of tiles costs ~1 %, bounded by 256 MB of four-step intermediates
+    // templates per persistent launch: enough 4096-element tiles (>= ~14 per resident CTA, 2 CTAs
+    // per SM) that the last, partly filled round of tiles costs ~1 %, bounded by 256 MB of
+    // four-step intermediates
+    const int64_t tiles_per_tmpl = n_fft / 4096 > 0 ? n_fft / 4096 : 1;
+    int64_t want = (14 * 2 * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
+    if (want < 8) want = 8;
     int64_t tb = (256ll << 20) / (n_fft * 16);
+    if (tb > want) tb = want;
     if (tb < 1) tb = 1;
-    if (tb > 64) tb = 64;
     return (int)tb;
 }
 
@@ -493,6 +499,15 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     const int L = ilog2(n_fft);
     g.log_n2 = L / 2; g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
     g.log_w1 = ilog2(tile_w(g.log_n1)); g.log_w2 = ilog2(tile_w(g.log_n2));
+    {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
+        const double wa = fabs(eph->omega_orb * eph->au_over_c_s) + fabs(eph->omega_rot * eph->re_over_c_s);
+        const double c2 = eph->omega_orb * eph->omega_orb * fabs(eph->au_over_c_s) + eph->omega_rot * eph->omega_rot * fabs(eph->re_over_c_s);
+        double e = wa * reach;
+        g.n_newton = 0;
+        while (e > 1e-11 && g.n_newton < 8) { e = 0.5 * c2 * e * e + wa * wa * wa * e; ++g.n_newton; }
+        const double half_block = 0.5 * SKY_THREADS * dt;
+        g.block_base = (fabs(eph->omega_rot) * half_block <= 0.1 && fabs(eph->omega_orb) * half_block <= 0.01) ? 1 : 0;
+    }
     p->eph = *eph; p->f_min = f_min; p->band = band; p->df = 1.0 / ((double)n_fft * dt);
     for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
     for (int m = -dterms; m <= dterms; ++m) {

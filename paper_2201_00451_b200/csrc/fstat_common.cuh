@@ -52,4 +52,6 @@ struct PlanGeom {
     uint32_t shift_mod;     // (round((f_min - f_het)/df)) mod n_fft
     int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2 (log_n1 >= log_n2)
     int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
+    int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
+    int block_base;         // 1: trigonometric base per block + small-angle rotation per thread
 };

@@ -34,23 +34,6 @@ __device__ __forceinline__ SsbBase ssb_base(const PlanGeom &g, double tau) {
     return b;
 }
 
-// Returns Delta = tau - T and cos/sin of the sidereal angle at T.
-__device__ __forceinline__ double ssb_invert(const PlanGeom &g, const SkyConst &sc, int X, const SsbBase &b,
-                                             double &cth, double &sth) {
-    double delta = sc.Pc * b.co + sc.Ps * b.so + sc.Qc[X] * b.cr + sc.Qs[X] * b.sr + sc.Q0[X];
-    cth = b.cr; sth = b.sr;
-#pragma unroll
-    for (int it = 0; it < 3; ++it) {      // contraction 1e-4 per step: 5e-2 s -> 5e-6 -> 5e-10 -> 5e-14
-        double se, ce, sr, cr;
-        small_sincos(g.omega_orb * delta, se, ce);
-        small_sincos(g.omega_rot * delta, sr, cr);
-        const double co = b.co * ce + b.so * se, so = b.so * ce - b.co * se;     // angle - eps
-        cth = b.cr * cr + b.sr * sr; sth = b.sr * cr - b.cr * sr;
-        delta = sc.Pc * co + sc.Ps * so + sc.Qc[X] * cth + sc.Qs[X] * sth + sc.Q0[X];
-    }
-    return delta;
-}
-
 // H2: a(t), b(t) from cos/sin of the sidereal angle (fp32).
 __device__ __forceinline__ void antenna_ab(const SkyConst &sc, int X, float cth, float sth, float &a, float &b) {
     const float ch = sc.cal[X] * cth + sc.sal[X] * sth;
@@ -60,76 +43,186 @@ __device__ __forceinline__ void antenna_ab(const SkyConst &sc, int X, float cth,
     b = sc.bc[X][0] * c2 + sc.bc[X][1] * s2 + sc.bc[X][2] * ch + sc.bc[X][3] * sh;
 }
 
+// Orbital-angle version of small_sincos: |e| = omega_orb * 500 s ~ 1e-4 rad for the Earth (error
+// < 1e-30); at the 0.05 rad fstat_setup admits the error is 1.5e-13 (7e-11 s of delay).
+__device__ __forceinline__ void tiny_sincos(double e, double &s, double &c) {
+    const double e2 = e * e;
+    s = e * (1.0 + e2 * (-1.0 / 6 + e2 * (1.0 / 120)));
+    c = 1.0 + e2 * (-0.5 + e2 * (1.0 / 24 + e2 * (-1.0 / 720)));
+}
+
+// H1 by Newton steps on F(T) = T + Delta_X(T) - tau, from T0 = tau - Delta_X(tau), where
+// |T0 - T*| <= |Delta'| |Delta| ~ 1e-4 * 500 s = 0.05 s.  One update leaves
+// |F''| (T0 - T*)^2 / 2 ~ 1.3e-10 s^-1 * 2.5e-3 s^2 / 2 = 2e-13 s for the Earth (needed: <~ 3e-8 s,
+// SURVEY 7); fstat_setup derives the step count g.n_newton from the ephemeris the same way.
+// Returns Delta = tau - T and cos/sin of the sidereal angle at the last evaluation point
+// (within 1e-5 s of T: the antenna patterns do not see the difference).
+__device__ __forceinline__ double ssb_invert_newton(const PlanGeom &g, const SkyConst &sc, int X, const SsbBase &b,
+                                                    double &cth, double &sth) {
+    double delta = sc.Pc * b.co + sc.Ps * b.so + sc.Qc[X] * b.cr + sc.Qs[X] * b.sr + sc.Q0[X];
+    cth = b.cr; sth = b.sr;
+    for (int it = 0; it < g.n_newton; ++it) {
+        double se, ce, sr, cr;
+        tiny_sincos(g.omega_orb * delta, se, ce);
+        small_sincos(g.omega_rot * delta, sr, cr);
+        const double co = b.co * ce + b.so * se, so = b.so * ce - b.co * se;      // angles at T_n = tau - delta
+        cth = b.cr * cr + b.sr * sr; sth = b.sr * cr - b.cr * sr;
+        const double f = (sc.Pc * co + sc.Ps * so + sc.Qc[X] * cth + sc.Qs[X] * sth + sc.Q0[X]) - delta;   // F(T_n)
+        const double dp = g.omega_orb * (sc.Ps * co - sc.Pc * so) + g.omega_rot * (sc.Qs[X] * cth - sc.Qc[X] * sth);   // Delta'(T_n)
+        delta += f * (1.0 - dp * (1.0 - dp));                                     // 1/(1+dp) to O(dp^3)
+    }
+    return delta;
+}
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+#define SKY_THREADS 256
+#define SKY_WIN (SKY_THREADS + 2 * FSTAT_MAX_DTERMS + 4)
+
 // H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
 //   series : [n_det][series_stride] float2, data starts at +SERIES_PAD (zeros around it)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
 //            S[k2 / W1][k1][k2 % W1]
-__global__ void __launch_bounds__(256)
+// The 256 outputs of a block read source samples j0 - D .. j0 + D with j0 - k constant to within
+// +-1 over the block (the delay drifts by <= 1e-4 samples per sample), so the block stages one
+// window of 256 + 2D + 2 samples per detector in shared memory and every thread takes its
+// 2D+1 taps from there; a thread whose taps fall outside the window (possible only for an
+// extreme user ephemeris) reads global memory instead.
+// DC = compile-time Dterms (8, 16) or 0 for the run-time value.
+// The trigonometric base of the timing model is evaluated once per block in fp64 at the block
+// centre and rotated to each thread's tau by the small angle omega * (tau - tau_c) (Taylor
+// series, exact to 1e-18 for angles < 0.1 rad); plans whose block span is too long for that
+// (g.block_base == 0) evaluate it per thread.
+template <int DC>
+__global__ void __launch_bounds__(SKY_THREADS)
 sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ WinTable win,
                     const SkyConst *__restrict__ skies, const float2 *__restrict__ series,
                     const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= g.n_src) return;
+    __shared__ float2 s_win[SKY_WIN];
+    __shared__ double s_base[4];
+    __shared__ long long s_r0;
+    const int D = DC ? DC : g.dterms;
+    const int64_t k0 = (int64_t)blockIdx.x * SKY_THREADS;
+    const int64_t k = k0 + threadIdx.x;
+    const bool live = k < g.n_src;
     const SkyConst &sc = skies[blockIdx.y];
     const int64_t krel = k - g.k_margin;
     const double tau = (double)krel * g.dt;
-    const SsbBase base = ssb_base(g, tau);
+    SsbBase base;
+    if (g.block_base) {
+        const double tau_c = (double)(k0 + SKY_THREADS / 2 - g.k_margin) * g.dt;
+        if (threadIdx.x == 0) sincos(g.phi_orb0 + g.omega_orb * tau_c, &s_base[1], &s_base[0]);
+        if (threadIdx.x == 32) sincos(g.gmst0 + g.omega_rot * tau_c, &s_base[3], &s_base[2]);
+        __syncthreads();
+        double se, ce, sr, cr;
+        tiny_sincos(g.omega_orb * (tau - tau_c), se, ce);
+        small_sincos(g.omega_rot * (tau - tau_c), sr, cr);
+        base.co = s_base[0] * ce - s_base[1] * se; base.so = s_base[1] * ce + s_base[0] * se;   // angle + eps
+        base.cr = s_base[2] * cr - s_base[3] * sr; base.sr = s_base[3] * cr + s_base[2] * sr;
+    } else {
+        base = ssb_base(g, tau);
+    }
 
-    float yar = 0.f, yai = 0.f, ybr = 0.f, ybi = 0.f;
-    const int D = g.dterms;
+    float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
     const float inv_dh = 1.0f / ((float)D + 0.5f);
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft)
     const uint64_t tshift = ((uint64_t)g.shift_mod * (uint64_t)k) & (uint64_t)(g.n_fft - 1);
     const double shift_cyc = (double)tshift / (double)g.n_fft;
+    const int wlen = SKY_THREADS + 2 * D + 2;
 
     for (int X = 0; X < g.n_det; ++X) {
         double cth, sth;
-        const double delta = ssb_invert(g, sc, X, base, cth, sth);
+        const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
         const double T = tau - delta;                       // detector epoch - t_start
-        if (!(T >= 0.0 && T < g.span)) continue;            // step 3: outside the data
-        const int slot = min((int)floor(T * g.inv_t_sft), g.n_slots - 1);
-        const float w = wslot[X * g.n_slots + slot];
-        if (w == 0.f) continue;                             // gap
+        float w = 0.f;
+        if (live && T >= 0.0 && T < g.span) {               // step 3: inside the data and not in a gap
+            const int slot = min((int)floor(T * g.inv_t_sft), g.n_slots - 1);
+            w = wslot[X * g.n_slots + slot];
+        }
         // fractional sample index u = krel - Delta/dt = j0 + d,  d in [-1/2, 1/2)
         const double v = -delta * g.inv_dt;
         const double vr = floor(v + 0.5);
         const float d = (float)(v - vr);
-        const int64_t j0 = krel + (int64_t)vr;
-        // kernel coefficients: sinc(d-m) W(d-m) = (-1)^m sin(pi d)/(pi (d-m)) * [0.54 + 0.46 cos(pi (d-m)/(D+1/2))]
-        const float spd = sinpif(d) * 0.318309886183790672f;
-        float sw, cw;
-        sincospif(d * inv_dh, &sw, &cw);
-        const float2 *x = series + (int64_t)X * g.series_stride + SERIES_PAD + j0;
-        float zr = 0.f, zi = 0.f;
-        for (int m = -D; m <= D; ++m) {
-            const float2 xv = __ldg(x + m);
-            const float wnd = 0.54f + 0.46f * (cw * win.c[m + D] + sw * win.s[m + D]);
-            float sinc;
-            if (m == 0) sinc = (fabsf(d) < 1e-4f) ? 1.0f - 1.6449340668f * d * d : spd / d;
-            else sinc = ((m & 1) ? -spd : spd) / (d - (float)m);
-            const float c = sinc * wnd;
-            zr = fmaf(xv.x, c, zr); zi = fmaf(xv.y, c, zi);
+        const int64_t r = (int64_t)vr;                      // j0 - krel
+        if (threadIdx.x == 0) s_r0 = r;
+        __syncthreads();
+        const int64_t r0 = s_r0;
+        // window = samples [jw, jw + wlen), jw = (k0 - K_m) + r0 - 1 - D
+        const int64_t jw = (k0 - g.k_margin) + r0 - 1 - D;
+        const float2 *xs = series + (int64_t)X * g.series_stride + SERIES_PAD;
+        for (int i = threadIdx.x; i < wlen; i += SKY_THREADS) {
+            const int64_t j = jw + i;
+            s_win[i] = (j >= -SERIES_PAD && j < g.n_samples + SERIES_PAD) ? __ldg(xs + j) : make_float2(0.f, 0.f);
         }
-        // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
-        double cyc = g.f_het * delta;
-        cyc = (cyc - floor(cyc)) + shift_cyc;
-        float sp, cp;
-        sincospif(-2.0f * (float)(cyc - floor(cyc)), &sp, &cp);
-        const float er = zr * cp - zi * sp, ei = zr * sp + zi * cp;
-        float a, b;
-        antenna_ab(sc, X, (float)cth, (float)sth, a, b);
-        yar = fmaf(w * a, er, yar); yai = fmaf(w * a, ei, yai);
-        ybr = fmaf(w * b, er, ybr); ybi = fmaf(w * b, ei, ybi);
+        __syncthreads();
+        if (w != 0.f) {
+            // kernel coefficients: sinc(d-m) W(d-m) = (-1)^m sin(pi d)/(pi (d-m)) * [0.54 + 0.46 cos(pi (d-m)/(D+1/2))];
+            // taps +m and -m share one reciprocal: 1/(d-m) = (d+m)/(d^2-m^2), 1/(d+m) = (d-m)/(d^2-m^2)
+            const float spd = sinpif(d) * 0.318309886183790672f;
+            float sw, cw;
+            sincospif(d * inv_dh, &sw, &cw);
+            const float cw46 = 0.46f * cw, sw46 = 0.46f * sw, d2 = d * d;
+            const int rel = (int)(r - r0);
+            const bool in_win = (rel >= -1 && rel <= 1);
+            float2 z;
+            {
+                const float c0 = ((fabsf(d) < 1e-4f) ? 1.0f - 1.6449340668f * d2 : spd / d) * (0.54f + cw46);
+                const float2 x0 = in_win ? s_win[threadIdx.x + rel + 1 + D] : __ldg(xs + krel + r);
+                z = make_float2(x0.x * c0, x0.y * c0);
+            }
+            if (in_win) {
+                const float2 *xc = s_win + (threadIdx.x + rel + 1 + D);
+                float sgn = -spd;
+#pragma unroll
+                for (int m = 1; m <= D; ++m) {
+                    const float fm = (float)m;
+                    const float s = sgn * rcp_approx(d2 - fm * fm);
+                    const float A = fmaf(cw46, win.c[m + D], 0.54f), B = sw46 * win.s[m + D];
+                    const float cp = s * (d + fm) * (A + B), cm = s * (d - fm) * (A - B);
+                    z = __ffma2_rn(xc[m], make_float2(cp, cp), z);
+                    z = __ffma2_rn(xc[-m], make_float2(cm, cm), z);
+                    sgn = -sgn;
+                }
+            } else {
+                const float2 *xc = xs + krel + r;
+                float sgn = -spd;
+                for (int m = 1; m <= D; ++m) {
+                    const float fm = (float)m;
+                    const float s = sgn * rcp_approx(d2 - fm * fm);
+                    const float A = fmaf(cw46, win.c[m + D], 0.54f), B = sw46 * win.s[m + D];
+                    const float cp = s * (d + fm) * (A + B), cm = s * (d - fm) * (A - B);
+                    z = __ffma2_rn(__ldg(xc + m), make_float2(cp, cp), z);
+                    z = __ffma2_rn(__ldg(xc - m), make_float2(cm, cm), z);
+                    sgn = -sgn;
+                }
+            }
+            // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
+            double cyc = g.f_het * delta;
+            cyc = (cyc - floor(cyc)) + shift_cyc;
+            float sp, cp;
+            sincospif(-2.0f * (float)(cyc - floor(cyc)), &sp, &cp);
+            const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
+            float a, b;
+            antenna_ab(sc, X, (float)cth, (float)sth, a, b);
+            ya.x = fmaf(w * a, er, ya.x); ya.y = fmaf(w * a, ei, ya.y);
+            yb.x = fmaf(w * b, er, yb.x); yb.y = fmaf(w * b, ei, yb.y);
+        }
+        __syncthreads();                                    // window buffer is reused by the next detector
     }
+    if (!live) return;
     int64_t off = k;
     if (blocked) {
         const int64_t k1 = k >> g.log_n2, k2 = k & (((int64_t)1 << g.log_n2) - 1);
         off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
     }
     // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
-    S[(int64_t)blockIdx.y * g.n_fft + off] = blocked ? make_float4(yar, ybr, yai, ybi) : make_float4(yar, yai, ybr, ybi);
+    S[(int64_t)blockIdx.y * g.n_fft + off] = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
 }
 
 // A, B, C (eq. 8): sums of w a^2, w b^2, w a b over the valid detector-frame samples.
