@@ -79,9 +79,14 @@ template <> struct RadixPlan<12> { static constexpr int np = 3, r0 = 16, r1 = 16
 
 __host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
-template <int LOGN> struct FftCfg {
-    static constexpr int LOGW = (LOGN == 12) ? 1 : 12 - LOGN;     // tile = 4096 elements (8192 for 2^12)
+// A tile is 2^LOGT elements = W = 2^(LOGT - LOGN) adjacent sub-FFTs, worked on by 2^LOGT / 16 threads:
+// LOGT = 11 (128 threads, 32 KB, 4 CTAs per SM) or 12 (256 threads, 64 KB, 2 CTAs per SM); sub-FFTs of
+// length 2^12 use LOGT = 13 (two per tile, so that the other pass still gets 32-byte store runs).
+template <int LOGN, int LOGT> struct FftCfg {
+    static_assert(LOGT >= LOGN && LOGT >= 11 && LOGT <= 13, "tile must hold at least one sub-FFT");
+    static constexpr int LOGW = LOGT - LOGN;
     static constexpr int W = 1 << LOGW;
+    static constexpr int MIN_CTAS = (LOGT == 11) ? 4 : (LOGT == 12) ? 2 : 1;
     static constexpr int N = 1 << LOGN;
     static constexpr int NT = (N * W) / 16;
     // twiddle table offsets (float2 entries): pass s >= 1 holds (R_s - 1) * P_s entries, [r-1][k]
@@ -185,6 +190,7 @@ struct FftArgs {
     const TmplDesc *tmpl;     // descriptors of the templates of this launch
     const SkyABCD *abcd;      // [n_sky_slots]
     float *twoF;              // output rows of this launch
+    uint32_t *gmax;           // top-k mode: [tile][warp] maximum (as topk_key) of the 512 bins each warp of pass 2 writes; else null
     int64_t twoF_stride;      // floats between rows
     const float2 *tw;         // twiddle table of this sub-FFT length
     int64_t n_fft, n_src, n_bins, k_margin;
@@ -217,32 +223,48 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
                      : "=r"(done) : "r"(a), "r"(parity) : "memory");
     }
 }
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *bar, uint64_t policy) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;\n" ::
                  "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src), "r"(bytes),
-                 "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+                 "r"((unsigned)__cvta_generic_to_shared(bar)), "l"(policy) : "memory");
+}
+// L2 eviction policies: the resampled series S is re-read by every template of the launch
+// (evict_last), the four-step intermediate T is written once and read once (evict_first).
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_global_hint(float4 *ptr, float4 v, uint64_t policy) {
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;\n" ::
+                 "l"(ptr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(policy) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
 // One thread starts the copy of a whole tile (contiguous in global memory thanks to the
 // tile-blocked layouts) into the exchange buffer; completion is signalled on the mbarrier.
-template <int LOGN>
-__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, uint64_t *bar) {
-    using C = FftCfg<LOGN>;
+template <int LOGN, int LOGT>
+__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, uint64_t *bar, uint64_t policy) {
+    using C = FftCfg<LOGN, LOGT>;
     constexpr unsigned BYTES = C::N * C::W * 16, CHUNK = 16384;
     if (threadIdx.x == 0) {
         fence_proxy_async();                      // earlier generic-proxy reads of the buffer are ordered before the async writes
         mbar_expect_tx(bar, BYTES);
 #pragma unroll
         for (unsigned o = 0; o < BYTES; o += CHUNK)
-            bulk_g2s(reinterpret_cast<char *>(sm) + o, reinterpret_cast<const char *>(src) + o, CHUNK, bar);
+            bulk_g2s(reinterpret_cast<char *>(sm) + o, reinterpret_cast<const char *>(src) + o, CHUNK, bar, policy);
     }
 }
 
 // Pass-0 inputs out of the staging layout (linear: element idx of lane w at idx*W + w).
-template <int LOGN>
+template <int LOGN, int LOGT>
 __device__ __forceinline__ void tile_take_inputs(float2 (&a)[16], float2 (&b)[16], const float4 *sm) {
-    using C = FftCfg<LOGN>;
+    using C = FftCfg<LOGN, LOGT>;
     using RP = RadixPlan<LOGN>;
     using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
 #pragma unroll
@@ -259,9 +281,9 @@ __device__ __forceinline__ void tile_take_inputs(float2 (&a)[16], float2 (&b)[16
 
 // Radix passes of one tile between "inputs of pass 0 are in registers" and "inputs of the last
 // pass are in registers and the exchange buffer is free again" (barrier included).
-template <int LOGN>
+template <int LOGN, int LOGT>
 __device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], float4 *sm, const float2 *__restrict__ tw) {
-    using C = FftCfg<LOGN>;
+    using C = FftCfg<LOGN, LOGT>;
     using RP = RadixPlan<LOGN>;
     constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
     constexpr bool LAST1 = (RP::np == 2);
@@ -280,9 +302,9 @@ __device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], fl
     __syncthreads();                                   // buffer free: the next tile may be prefetched
 }
 
-template <int LOGN>
+template <int LOGN, int LOGT>
 __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16], const float2 *__restrict__ tw) {
-    using C = FftCfg<LOGN>;
+    using C = FftCfg<LOGN, LOGT>;
     using RP = RadixPlan<LOGN>;
     if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
     else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
@@ -290,7 +312,7 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16],
 
 // Common kernel preamble: shared-memory carve-up, twiddles to shared memory, mbarrier init.
 #define FFT_KERNEL_PREAMBLE()                                                                     \
-    using C = FftCfg<LOGN>;                                                                       \
+    using C = FftCfg<LOGN, LOGT>;                                                                       \
     using RP = RadixPlan<LOGN>;                                                                   \
     constexpr int LOGW = C::LOGW, NT = C::NT;                                                     \
     extern __shared__ float4 sm[];                                                                \
@@ -310,20 +332,22 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16],
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
 // Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
 // ---------------------------------------------------------------------------------------
-template <int LOGN>
-__global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
+template <int LOGN, int LOGT>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT>::NT, FftCfg<LOGN, LOGT>::MIN_CTAS)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
     FFT_KERNEL_PREAMBLE();
-    tile_prefetch<LOGN>(sm, p.S + (int64_t)p.tmpl[tile >> p.log_tiles].sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar);
+    const uint64_t pol_S = l2_policy_evict_last(), pol_T = l2_policy_evict_first();
+    TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
+    tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S);
     for (; tile < p.n_tiles; tile += gridDim.x) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
-        const TmplDesc td = p.tmpl[t];
+        const TmplDesc td = td_next;
         const int k2_0 = x << LOGW;
-        const int nxt = tile + gridDim.x;               // fetch the next tile's source slot early
-        const int sky_next = (nxt < p.n_tiles) ? p.tmpl[nxt >> p.log_tiles].sky_slot : 0;
+        const int nxt = tile + gridDim.x;               // fetch the next tile's descriptor early
+        if (nxt < p.n_tiles) td_next = p.tmpl[nxt >> p.log_tiles];
         mbar_wait(bar, parity);
         parity ^= 1;
-        tile_take_inputs<LOGN>(a, b, sm);
+        tile_take_inputs<LOGN, LOGT>(a, b, sm);
         {   // times exp(-i Phi_s) (S9).  The r0 inputs of one butterfly sit on an
             // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic
             // phi(tau) = tau^2 (c1 + c2 tau): its forward differences D1, D2 and the constant D3 are
@@ -356,10 +380,10 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 }
             }
         }
-        tile_passes<LOGN>(a, b, sm, sm_tw);
+        tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < p.n_tiles)
-            tile_prefetch<LOGN>(sm, p.S + (int64_t)sky_next * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar);
-        tile_last_pass<LOGN>(a, b, sm_tw);
+            tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S);
+        tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
         {   // outputs m1 = i + r*NI of column k2 = k2_0 + w, times the four-step twiddle
             // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r (two exact sincospif per butterfly, powers by
             // products), stored tile-blocked for pass 2: T[m1 / W2][k2][m1 % W2] -- consecutive lanes
@@ -392,7 +416,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                     const int m1 = i + r * PI::NI;
                     float4 *o = affine ? dst + r * rstride
                                        : colbase + ((int64_t)(m1 >> lw2) << (ln2 + lw2)) + (m1 & ((1 << lw2) - 1));
-                    __stcg(o, make_float4(xx.x, xx.y, yy.x, yy.y));
+                    st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
                     if (r + 1 < RL) tw = cmul(tw, step);
                 }
             }
@@ -404,28 +428,33 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
 // Pass 2: row FFTs of length N2 = 2^LOGN + the 2F combination of eq. 8 (Fig. 1).
 // Persistent; tile = (template, W adjacent rows m1) = one contiguous block of T.
 // ---------------------------------------------------------------------------------------
-template <int LOGN>
-__global__ void __launch_bounds__(FftCfg<LOGN>::NT, (LOGN == 12) ? 1 : 2)
+template <int LOGN, int LOGT>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT>::NT, FftCfg<LOGN, LOGT>::MIN_CTAS)
 fft_pass2_kernel(const __grid_constant__ FftArgs p) {
     FFT_KERNEL_PREAMBLE();
-    tile_prefetch<LOGN>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar);
+    const uint64_t pol_T = l2_policy_evict_first();
+    int sky_next = p.tmpl[tile >> p.log_tiles].sky_slot;
+    tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_T);
     for (; tile < p.n_tiles; tile += gridDim.x) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const int m1_0 = x << LOGW;
         const int nxt = tile + gridDim.x;
-        const SkyABCD ab = p.abcd[p.tmpl[t].sky_slot];
+        const SkyABCD *abp = p.abcd + sky_next;
+        const float b_over_d = abp->b_over_d, a_over_d = abp->a_over_d, two_c_over_d = abp->two_c_over_d;
+        if (nxt < p.n_tiles) sky_next = p.tmpl[nxt >> p.log_tiles].sky_slot;
         mbar_wait(bar, parity);
         parity ^= 1;
-        tile_take_inputs<LOGN>(a, b, sm);
-        tile_passes<LOGN>(a, b, sm, sm_tw);
+        tile_take_inputs<LOGN, LOGT>(a, b, sm);
+        tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < p.n_tiles)
-            tile_prefetch<LOGN>(sm, p.T + (int64_t)(nxt >> p.log_tiles) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar);
-        tile_last_pass<LOGN>(a, b, sm_tw);
+            tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(nxt >> p.log_tiles) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_T);
+        tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
         {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
             constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
             using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
             float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride;
+            float tmax = __int_as_float(0xff800000);
 #pragma unroll
             for (int bb = 0; bb < PI::NB; ++bb) {
                 int i, w;
@@ -436,11 +465,16 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
                     if (q < p.n_bins) {
                         const float2 fa = make_float2(a[bb * RL + r].x, b[bb * RL + r].x);    // unpack (re, im) of Fa, Fb
                         const float2 fb = make_float2(a[bb * RL + r].y, b[bb * RL + r].y);
-                        const float twoF = ab.b_over_d * (fa.x * fa.x + fa.y * fa.y) + ab.a_over_d * (fb.x * fb.x + fb.y * fb.y)
-                                         - ab.two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
+                        const float twoF = b_over_d * (fa.x * fa.x + fa.y * fa.y) + a_over_d * (fb.x * fb.x + fb.y * fb.y)
+                                         - two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
                         __stcs(out + q, twoF);
+                        tmax = fmaxf(tmax, twoF);
                     }
                 }
+            }
+            if (p.gmax) {   // H8: per-warp maximum for the top-k selection (topk_kernels.cuh)
+                const uint32_t key = __reduce_max_sync(0xffffffffu, topk_key(tmax));
+                if ((threadIdx.x & 31) == 0) p.gmax[(int64_t)tile * (NT / 32) + (threadIdx.x >> 5)] = key;
             }
         }
     }

@@ -50,7 +50,7 @@ struct fstat_plan {
     TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
     int *d_err = nullptr;
     float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
-    float *d_cand_v = nullptr; int *d_cand_i = nullptr; size_t cand_cap = 0;
+    uint32_t *d_gmax = nullptr;       // top-k: per-group maxima of the rows in flight [n_inflight][n_groups]
     HostRing ring;
     float *d_topk_v = nullptr; int *d_topk_i = nullptr; size_t topk_cap = 0;
     // pinned staging
@@ -155,11 +155,11 @@ void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *s
 }
 
 // Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
-template <int LOGN, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
-    using C = FftCfg<LOGN>;
+template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
+    using C = FftCfg<LOGN, LOGT>;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
-    auto kern = P2 ? fft_pass2_kernel<LOGN> : fft_pass1_kernel<LOGN>;
+    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT> : fft_pass1_kernel<LOGN, LOGT>;
     if (configured_dev != p->device) {
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
@@ -175,36 +175,42 @@ template <int LOGN, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tile
     ++p->launches;
     return FSTAT_OK;
 }
-template <int LOGN> int launch_pass1(fstat_plan *p, FftArgs &a, int tiles, int n_t) { return launch_pass<LOGN, false>(p, a, tiles, n_t); }
-template <int LOGN> int launch_pass2(fstat_plan *p, FftArgs &a, int tiles, int n_t) { return launch_pass<LOGN, true>(p, a, tiles, n_t); }
-
-#define DISPATCH_LOGN(logn, fn, ...)                         \
-    switch (logn) {                                          \
-        case 6: rc = fn<6>(__VA_ARGS__); break;              \
-        case 7: rc = fn<7>(__VA_ARGS__); break;              \
-        case 8: rc = fn<8>(__VA_ARGS__); break;              \
-        case 9: rc = fn<9>(__VA_ARGS__); break;              \
-        case 10: rc = fn<10>(__VA_ARGS__); break;            \
-        case 11: rc = fn<11>(__VA_ARGS__); break;            \
-        default: rc = fn<12>(__VA_ARGS__); break;            \
+#define DISPATCH_TILE(logn, logt, P2, ...)                                                        \
+    switch ((logn) * 16 + (logt)) {                                                              \
+        case 6 * 16 + 11: rc = launch_pass<6, 11, P2>(__VA_ARGS__); break;                       \
+        case 7 * 16 + 11: rc = launch_pass<7, 11, P2>(__VA_ARGS__); break;                       \
+        case 8 * 16 + 11: rc = launch_pass<8, 11, P2>(__VA_ARGS__); break;                       \
+        case 9 * 16 + 11: rc = launch_pass<9, 11, P2>(__VA_ARGS__); break;                       \
+        case 10 * 16 + 11: rc = launch_pass<10, 11, P2>(__VA_ARGS__); break;                     \
+        case 11 * 16 + 11: rc = launch_pass<11, 11, P2>(__VA_ARGS__); break;                     \
+        case 6 * 16 + 12: rc = launch_pass<6, 12, P2>(__VA_ARGS__); break;                       \
+        case 7 * 16 + 12: rc = launch_pass<7, 12, P2>(__VA_ARGS__); break;                       \
+        case 8 * 16 + 12: rc = launch_pass<8, 12, P2>(__VA_ARGS__); break;                       \
+        case 9 * 16 + 12: rc = launch_pass<9, 12, P2>(__VA_ARGS__); break;                       \
+        case 10 * 16 + 12: rc = launch_pass<10, 12, P2>(__VA_ARGS__); break;                     \
+        case 11 * 16 + 12: rc = launch_pass<11, 12, P2>(__VA_ARGS__); break;                     \
+        case 12 * 16 + 13: rc = launch_pass<12, 13, P2>(__VA_ARGS__); break;                     \
+        default: rc = fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination"); break;    \
     }
 
-int tile_w(int logn) { return logn == 12 ? 2 : (1 << (12 - logn)); }
+// log2 of the tile size used for a sub-FFT of length 2^logn under the plan's tile setting
+int tile_log1(const fstat_plan *p) { return p->g.log_n1 == 12 ? 13 : p->g.log_tile1; }
+int tile_log2(const fstat_plan *p) { return p->g.log_n2 == 12 ? 13 : p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
-int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_stride) {
+int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
     FftArgs a{};
     a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd;
-    a.twoF = rows; a.twoF_stride = row_stride;
+    a.twoF = rows; a.twoF_stride = row_stride; a.gmax = gmax;
     a.n_fft = p->g.n_fft; a.n_src = p->g.n_src; a.n_bins = p->g.n_bins; a.k_margin = p->g.k_margin;
     a.dt = p->g.dt;
     int rc = FSTAT_OK;
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
     a.tw = p->d_tw1; a.log_other = l2; a.log_w_other = p->g.log_w2;
-    { ProfScope ps(p, 1); DISPATCH_LOGN(l1, launch_pass1, p, a, (1 << l2) / tile_w(l1), nt); }
+    { ProfScope ps(p, 1); DISPATCH_TILE(l1, tile_log1(p), false, p, a, 1 << (l2 - p->g.log_w1), nt); }
     if (rc) return rc;
     a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
-    { ProfScope ps(p, 2); DISPATCH_LOGN(l2, launch_pass2, p, a, (1 << l1) / tile_w(l2), nt); }
+    { ProfScope ps(p, 2); DISPATCH_TILE(l2, tile_log2(p), true, p, a, 1 << (l1 - p->g.log_w2), nt); }
     if (rc) return rc;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -258,18 +264,28 @@ struct OutSpec {
     int32_t *bin = nullptr;
 };
 
-int ensure_topk_scratch(fstat_plan *p, int k) {
+// groups of 512 bins (one warp of a pass-2 tile each) per row, and how pass 2 maps them to bins
+TopkGeom topk_geom(const fstat_plan *p) {
+    const int l2 = p->g.log_n2, lt = tile_log2(p);
+    const std::vector<int> rl = radix_list(l2);
+    TopkGeom tg{};
+    tg.nt = (1 << lt) / 16;
+    tg.log_w = lt - l2;
+    tg.log_rl = ilog2(rl.back());
+    tg.pl = 1;
+    for (size_t i = 0; i + 1 < rl.size(); ++i) tg.pl *= rl[i];
+    tg.log_other = p->g.log_n1;
+    tg.n_groups = (int)(p->g.n_fft >> lt) * (tg.nt / 32);
+    return tg;
+}
+
+int ensure_topk_scratch(fstat_plan *p) {
     const int64_t nb = p->g.n_bins;
-    const int nblk = (int)((nb + TOPK_SLICE - 1) / TOPK_SLICE);
     if (!p->d_rows) CUDA_TRY(p, cudaMalloc(&p->d_rows, (size_t)p->n_inflight * nb * sizeof(float)));
-    const size_t need = (size_t)p->n_inflight * nblk * k;
-    if (need > p->cand_cap) {
-        if (p->d_cand_v) cudaFree(p->d_cand_v);
-        if (p->d_cand_i) cudaFree(p->d_cand_i);
-        p->d_cand_v = nullptr; p->d_cand_i = nullptr; p->cand_cap = 0;
-        CUDA_TRY(p, cudaMalloc(&p->d_cand_v, need * sizeof(float)));
-        CUDA_TRY(p, cudaMalloc(&p->d_cand_i, need * sizeof(int)));
-        p->cand_cap = need;
+    if (!p->d_gmax) {
+        const TopkGeom tg = topk_geom(p);
+        CUDA_TRY(p, cudaMalloc(&p->d_gmax, (size_t)p->n_inflight * tg.n_groups * sizeof(uint32_t)));
+        CUDA_TRY(p, cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tg.n_groups * (int)sizeof(uint32_t)));
     }
     return FSTAT_OK;
 }
@@ -324,7 +340,7 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaEventRecord(p->staging_ev, p->stream));
 
-    if (out.mode == OUT_TOPK) { rc = ensure_topk_scratch(p, out.k); if (rc) return rc; }
+    if (out.mode == OUT_TOPK) { rc = ensure_topk_scratch(p); if (rc) return rc; }
     if (out.mode == OUT_HOST_ROWS) { rc = ensure_host_ring(p); if (rc) return rc; }
 
     const int64_t nb = p->g.n_bins;
@@ -360,14 +376,13 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
                 if (rc) return rc;
                 ring_fill += nt;
             } else {
-                rc = launch_fft_chunk(p, t0, nt, p->d_rows, nb);
+                rc = launch_fft_chunk(p, t0, nt, p->d_rows, nb, p->d_gmax);
                 if (rc) return rc;
-                const int nblk = (int)((nb + TOPK_SLICE - 1) / TOPK_SLICE);
                 ProfScope ps(p, 3);
-                topk_stage1_kernel<<<dim3(nblk, nt), TOPK_THREADS, 0, p->stream>>>(p->d_rows, nb, nb, out.k, p->d_cand_v, p->d_cand_i);
-                topk_stage2_kernel<<<nt, TOPK_THREADS, 0, p->stream>>>(p->d_cand_v, p->d_cand_i, nblk * out.k, out.k,
-                                                                       out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k);
-                p->launches += 2;
+                const TopkGeom tg = topk_geom(p);
+                topk_select_kernel<<<nt, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), p->stream>>>(
+                    p->d_rows, nb, nb, out.k, p->d_gmax, tg, out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k);
+                p->launches += 1;
                 CUDA_TRY(p, cudaGetLastError());
             }
         }
@@ -386,7 +401,7 @@ void destroy_impl(fstat_plan *p) {
     if (p->stream) cudaStreamSynchronize(p->stream);
     cudaFree(p->d_series); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd); cudaFree(p->d_abc_partial);
-    cudaFree(p->d_tmpl); cudaFree(p->d_err); cudaFree(p->d_rows); cudaFree(p->d_cand_v); cudaFree(p->d_cand_i);
+    cudaFree(p->d_tmpl); cudaFree(p->d_err); cudaFree(p->d_rows); cudaFree(p->d_gmax);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
     for (int i = 0; i < 2; ++i) { cudaFree(p->ring.buf[i]); if (p->ring.done[i]) cudaEventDestroy(p->ring.done[i]); }
     if (p->h_sky) cudaFreeHost(p->h_sky);
@@ -399,14 +414,15 @@ void destroy_impl(fstat_plan *p) {
     delete p;
 }
 
-int default_inflight(int64_t n_fft) {
-    // templates per persistent launch: enough 4096-element tiles (>= ~14 per resident CTA, 2 CTAs
-    // per SM) that the last, partly filled round of tiles costs ~1 %, bounded by 256 MB of
-    // four-step intermediates
-    const int64_t tiles_per_tmpl = n_fft / 4096 > 0 ? n_fft / 4096 : 1;
-    int64_t want = (14 * 2 * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
-    if (want < 8) want = 8;
-    int64_t tb = (256ll << 20) / (n_fft * 16);
+int default_inflight(int64_t n_fft, int log_tile) {
+    // templates per persistent launch.  Measured on B200 (profiles/r01_v3_inflight.md): every launch pair
+    // costs ~35 us of ramp-up, tail and launch gap whatever its size, and keeping the four-step
+    // intermediate L2-resident buys nothing (the passes are FMA-pipe bound, not DRAM bound), so
+    // launches are made large: ~64 rounds of 4096-element tiles over the 296 resident CTAs, bounded by
+    // 2 GB of intermediates.
+    const int64_t tiles_per_tmpl = (n_fft >> log_tile) > 0 ? (n_fft >> log_tile) : 1;
+    int64_t want = (64 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
+    int64_t tb = (2048ll << 20) / (n_fft * 16);
     if (tb > want) tb = want;
     if (tb < 1) tb = 1;
     return (int)tb;
@@ -498,7 +514,17 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
     const int L = ilog2(n_fft);
     g.log_n2 = L / 2; g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
-    g.log_w1 = ilog2(tile_w(g.log_n1)); g.log_w2 = ilog2(tile_w(g.log_n2));
+    {   // tile sizes of the two FFT passes (profiles/r01_v3_tiles.md): 2^11-element tiles (128 threads, 4 CTAs per
+        // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
+        // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
+        // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
+        g.log_tile1 = g.log_n1 <= 10 ? 11 : 12;
+        g.log_tile2 = 12;
+        const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
+        if (e1 && (atoi(e1) == 11 || atoi(e1) == 12) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
+        if (e2 && (atoi(e2) == 11 || atoi(e2) == 12) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
+    }
+    g.log_w1 = tile_log1(p) - g.log_n1; g.log_w2 = tile_log2(p) - g.log_n2;
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
         const double wa = fabs(eph->omega_orb * eph->au_over_c_s) + fabs(eph->omega_rot * eph->re_over_c_s);
         const double c2 = eph->omega_orb * eph->omega_orb * fabs(eph->au_over_c_s) + eph->omega_rot * eph->omega_rot * fabs(eph->re_over_c_s);
@@ -530,7 +556,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
     SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     SETUP_TRY(cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
-    p->n_inflight = default_inflight(n_fft);
+    p->n_inflight = default_inflight(n_fft, g.log_tile2);
     p->n_sky_slots = default_sky_slots(n_fft);
     SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
     SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
@@ -632,11 +658,11 @@ int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight) {
     if (!plan || n_inflight < 0 || n_inflight > 4096) return FSTAT_EINVAL;
     CUDA_TRY(plan, cudaSetDevice(plan->device));
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
-    const int tb = n_inflight == 0 ? default_inflight(plan->g.n_fft) : n_inflight;
+    const int tb = n_inflight == 0 ? default_inflight(plan->g.n_fft, plan->g.log_tile2) : n_inflight;
     if (tb == plan->n_inflight) return FSTAT_OK;
     cudaFree(plan->d_T); plan->d_T = nullptr;
     cudaFree(plan->d_rows); plan->d_rows = nullptr;
-    cudaFree(plan->d_cand_v); cudaFree(plan->d_cand_i); plan->d_cand_v = nullptr; plan->d_cand_i = nullptr; plan->cand_cap = 0;
+    cudaFree(plan->d_gmax); plan->d_gmax = nullptr;
     for (int i = 0; i < 2; ++i) { cudaFree(plan->ring.buf[i]); plan->ring.buf[i] = nullptr; if (plan->ring.done[i]) cudaEventDestroy(plan->ring.done[i]); plan->ring.done[i] = nullptr; }
     plan->ring.rows = 0;
     plan->n_inflight = tb;

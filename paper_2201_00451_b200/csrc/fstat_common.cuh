@@ -8,6 +8,16 @@
 #define FSTAT_MAX_TOPK 64
 #define SERIES_PAD 64            // zero samples kept on both sides of every series
 
+#ifdef __CUDACC__
+// Order-preserving map float -> uint32 (NaN lowest, then -inf ... +inf).
+__device__ __forceinline__ uint32_t topk_key(float v) {
+    const uint32_t b = __float_as_uint(v);
+    if (v != v) return 0u;
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+#endif
+
 // Per-sky constants, computed on the host in double (cheap, O(n_det)) -- DESIGN.md "H1/H2".
 struct SkyConst {
     // Roemer delay: Delta = Pc cos(phi_o) + Ps sin(phi_o) + Qc[X] cos(theta) + Qs[X] sin(theta) + Q0[X]
@@ -52,6 +62,7 @@ struct PlanGeom {
     uint32_t shift_mod;     // (round((f_min - f_het)/df)) mod n_fft
     int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2 (log_n1 >= log_n2)
     int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
+    int log_tile1, log_tile2;   // log2 of the tile size of FFT pass 1 / 2 (11 or 12; sub-FFTs of length 2^12 use 13)
     int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
     int block_base;         // 1: trigonometric base per block + small-angle rotation per thread
 };

@@ -74,6 +74,28 @@ __device__ __forceinline__ double ssb_invert_newton(const PlanGeom &g, const Sky
     return delta;
 }
 
+// sin(pi x)/(pi x) and cos(pi x) for |x| <= 1/2 as Taylor polynomials in x^2 (truncation < 4e-8 / 7e-9):
+// no division, no range reduction, relative accuracy at x -> 0 (the main tap needs sinc(d) to 1e-7).
+__device__ __forceinline__ float sinc_pi_poly(float x2) {
+    float p = 1.4842879e-4f;                  // pi^12/13!
+    p = fmaf(p, x2, -2.3460810e-3f);          // -pi^10/11!
+    p = fmaf(p, x2, 2.6147848e-2f);           // pi^8/9!
+    p = fmaf(p, x2, -1.9075182e-1f);          // -pi^6/7!
+    p = fmaf(p, x2, 8.1174243e-1f);           // pi^4/5!
+    p = fmaf(p, x2, -1.6449341f);             // -pi^2/3!
+    return fmaf(p, x2, 1.0f);
+}
+__device__ __forceinline__ float cos_pi_poly(float x2) {
+    float p = -1.0463811e-4f;                 // -pi^14/14!
+    p = fmaf(p, x2, 1.9295743e-3f);           // pi^12/12!
+    p = fmaf(p, x2, -2.5806891e-2f);          // -pi^10/10!
+    p = fmaf(p, x2, 2.3533063e-1f);           // pi^8/8!
+    p = fmaf(p, x2, -1.3352628f);             // -pi^6/6!
+    p = fmaf(p, x2, 4.0587121f);              // pi^4/4!
+    p = fmaf(p, x2, -4.9348022f);             // -pi^2/2!
+    return fmaf(p, x2, 1.0f);
+}
+
 __device__ __forceinline__ float rcp_approx(float x) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -132,8 +154,9 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
     float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
     const float inv_dh = 1.0f / ((float)D + 0.5f);
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft)
-    const uint64_t tshift = ((uint64_t)g.shift_mod * (uint64_t)k) & (uint64_t)(g.n_fft - 1);
-    const double shift_cyc = (double)tshift / (double)g.n_fft;
+    // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two)
+    const uint32_t tshift = (uint32_t)(((uint64_t)g.shift_mod * (uint64_t)k) & (uint64_t)(g.n_fft - 1));
+    const float shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
     const int wlen = SKY_THREADS + 2 * D + 2;
 
     for (int X = 0; X < g.n_det; ++X) {
@@ -164,15 +187,14 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
         if (w != 0.f) {
             // kernel coefficients: sinc(d-m) W(d-m) = (-1)^m sin(pi d)/(pi (d-m)) * [0.54 + 0.46 cos(pi (d-m)/(D+1/2))];
             // taps +m and -m share one reciprocal: 1/(d-m) = (d+m)/(d^2-m^2), 1/(d+m) = (d-m)/(d^2-m^2)
-            const float spd = sinpif(d) * 0.318309886183790672f;
-            float sw, cw;
-            sincospif(d * inv_dh, &sw, &cw);
-            const float cw46 = 0.46f * cw, sw46 = 0.46f * sw, d2 = d * d;
+            const float d2 = d * d, sincd = sinc_pi_poly(d2), spd = d * sincd;        // spd = sin(pi d)/pi
+            const float xw = d * inv_dh, xw2 = xw * xw;
+            const float cw46 = 0.46f * cos_pi_poly(xw2), sw46 = (0.46f * 3.14159265358979f) * xw * sinc_pi_poly(xw2);
             const int rel = (int)(r - r0);
             const bool in_win = (rel >= -1 && rel <= 1);
             float2 z;
             {
-                const float c0 = ((fabsf(d) < 1e-4f) ? 1.0f - 1.6449340668f * d2 : spd / d) * (0.54f + cw46);
+                const float c0 = sincd * (0.54f + cw46);
                 const float2 x0 = in_win ? s_win[threadIdx.x + rel + 1 + D] : __ldg(xs + krel + r);
                 z = make_float2(x0.x * c0, x0.y * c0);
             }
@@ -203,10 +225,12 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
                 }
             }
             // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
-            double cyc = g.f_het * delta;
-            cyc = (cyc - floor(cyc)) + shift_cyc;
+            // (phase reduced mod 1 in fp64, then fp32: |arg| <= pi, where sin/cos.approx are good to 5e-7 abs)
+            const double cyc = g.f_het * delta;
+            float fc = (float)(cyc - floor(cyc)) + shift_cyc;
+            fc -= rintf(fc);
             float sp, cp;
-            sincospif(-2.0f * (float)(cyc - floor(cyc)), &sp, &cp);
+            __sincosf(-6.283185307179586f * fc, &sp, &cp);
             const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
             float a, b;
             antenna_ab(sc, X, (float)cth, (float)sth, a, b);

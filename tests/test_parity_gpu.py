@@ -170,3 +170,41 @@ def test_empty_detector_gives_edom():
             plan.sync()
         assert ei.value.code == FSTAT_EDOM
         assert np.isnan(out.cpu().numpy()).all()
+
+
+@pytest.mark.parametrize("log_nfft,k", [(12, 3), (17, 1), (18, 64), (20, 16)])
+def test_topk_select_matches_own_rows(log_nfft, k):
+    # the fused selection (per-warp maxima from FFT pass 2 -> threshold -> hot groups) must reproduce,
+    # bit for bit, the (2F desc, bin asc) selection applied to the full rows the same plan computes
+    n = int(0.7 * (1 << log_nfft))
+    p = synth.small_problem(seed=40 + log_nfft, n_samples=n, dt=0.5 if log_nfft > 17 else 1.0, n_fft=1 << log_nfft,
+                            n_templates=3, gap_frac=0.3, rho=9.0)
+    with _plan(p) as plan:
+        val, idx = plan.compute_topk(p.templates, k)
+        full = plan.compute(p.templates)
+        plan.sync()
+        val, idx, full = val.cpu().numpy(), idx.cpu().numpy(), full.cpu().numpy()
+    for t in range(len(p.templates)):
+        ev, ei = O.topk(full[t], k)
+        np.testing.assert_array_equal(idx[t], ei)
+        np.testing.assert_array_equal(val[t], ev)
+
+
+def test_topk_degenerate_rows_take_the_exact_slow_path():
+    # all-zero data: every bin ties at 2F = 0 -> bins 0..k-1 in order (S15)
+    p = synth.small_problem(seed=41, n_samples=20000, n_fft=1 << 15, n_templates=2, rho=None, noise=False)
+    with _plan(p) as plan:
+        val, idx = plan.compute_topk(p.templates, 5)
+        plan.sync()
+        np.testing.assert_array_equal(idx.cpu().numpy(), np.tile(np.arange(5, dtype=np.int32), (2, 1)))
+        np.testing.assert_array_equal(val.cpu().numpy(), np.zeros((2, 5), dtype=np.float32))
+    # D <= 0 (no valid data): rows are NaN -> (-inf, -1)
+    from paper_2201_00451_b200.binding import FstatError
+    q = synth.small_problem(seed=16, n_det=1, n_samples=8000, n_fft=1 << 14, n_templates=1)
+    q.timestamps = [q.timestamps[0][:0]]
+    q.weights = [q.weights[0][:0]]
+    with _plan(q) as plan:
+        val, idx = plan.compute_topk(q.templates, 4)
+        with pytest.raises(FstatError):
+            plan.sync()
+        assert np.all(idx.cpu().numpy() == -1) and np.all(np.isneginf(val.cpu().numpy()))
