@@ -415,7 +415,7 @@ void destroy_impl(fstat_plan *p) {
 }
 
 int default_inflight(int64_t n_fft, int log_tile) {
-    // templates per persistent launch.  Measured on B200 (profiles/r01_v3_inflight.md): every launch pair
+    // templates per persistent launch.  Measured on B200 (profiles/r01_v3_experiments.md): every launch pair
     // costs ~35 us of ramp-up, tail and launch gap whatever its size, and keeping the four-step
     // intermediate L2-resident buys nothing (the passes are FMA-pipe bound, not DRAM bound), so
     // launches are made large: ~64 rounds of 4096-element tiles over the 296 resident CTAs, bounded by
@@ -514,7 +514,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
     const int L = ilog2(n_fft);
     g.log_n2 = L / 2; g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
-    {   // tile sizes of the two FFT passes (profiles/r01_v3_tiles.md): 2^11-element tiles (128 threads, 4 CTAs per
+    {   // tile sizes of the two FFT passes (profiles/r01_v3_experiments.md): 2^11-element tiles (128 threads, 4 CTAs per
         // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
