@@ -49,10 +49,32 @@ def make_workload(name: str, rank: int = 0):
         p = synth.small_problem(n_samples=20000, n_fft=1 << 15, n_templates=64)
     else:
         raise SystemExit(f"unknown workload {name}")
-    if rank > 0:                              # replicas: every rank searches its own fdot sub-bank
-        span = float(np.ptp(p.templates[:, 3])) or 1e-9
-        p.templates[:, 3] -= rank * span
+    p.templates = replica_templates(p.templates, rank)
     return p
+
+
+def replica_templates(templates, rank: int):
+    """Multi-GPU = independent replicas: rank r searches the fdot sub-bank shifted by r spans,
+    so the ranks' banks tile the fdot axis without overlap; no data-path collective."""
+    t = np.array(templates, dtype=np.float64, copy=True)
+    if rank > 0:
+        span = float(np.ptp(t[:, 3])) or 1e-9
+        step = span / max(len(np.unique(t[:, 3])) - 1, 1)
+        t[:, 3] -= rank * (span + step)
+    return t
+
+
+def aggregate_ranks(total_ms: float, units: int, steps: int, dist=None, device=None):
+    """Whole-job value: units all ranks processed / the slowest rank's device time (max over ranks)."""
+    world = 1
+    if dist is not None and dist.is_initialized():
+        import torch
+        world = dist.get_world_size()
+        t = torch.tensor([total_ms], dtype=torch.float64, device=device or "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / steps
+    return world * units / (ms_per_step * 1e-3), ms_per_step
 
 
 def algorithmic_bytes(p):
@@ -233,12 +255,8 @@ def run_ours(args):
     launches = plan.launch_count() - l0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
-    value = world * n_t * nb / (ms_per_step * 1e-3)
+    value, ms_per_step = aggregate_ranks(total_ms, n_t * nb, args.steps, dist if world > 1 else None, "cuda")
+    total_ms = ms_per_step * args.steps
 
     # ---- roofline of the dominant kernel class (CUDA events inside the library, same timed steps)
     roofline = None
