@@ -513,7 +513,13 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     const long long shift = llround((f_min - f_het) * (double)n_fft * dt);
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
     const int L = ilog2(n_fft);
-    g.log_n2 = L / 2; g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
+    // n_fft = 2^log_n1 x 2^log_n2.  Pass 2 gets the shorter transform: its tile then spans more rows, which is what
+    // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
+    // 2^11-element tiles.  Split per size as measured on B200 (profiles/r01_v3_experiments.md, section 4).
+    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10
+             : L == 22 ? (2 * n_bins > n_fft ? 10 : 11) : L - 12;
+    { const char *e = getenv("FSTAT_LOGN2"); if (e && atoi(e) >= 6 && atoi(e) <= 12 && L - atoi(e) >= 6 && L - atoi(e) <= 12) g.log_n2 = atoi(e); }
+    g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
     {   // tile sizes of the two FFT passes (profiles/r01_v3_experiments.md): 2^11-element tiles (128 threads, 4 CTAs per
         // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
