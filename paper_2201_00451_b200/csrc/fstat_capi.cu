@@ -45,10 +45,10 @@ struct fstat_plan {
     float4 *d_S = nullptr;   int n_sky_slots = 0;
     float4 *d_T = nullptr;   int n_inflight = 0;
     SkyConst *d_sky = nullptr; size_t sky_cap = 0;
-    SkyABCD *d_abcd = nullptr;
-    double *d_abc_partial = nullptr; int abc_nblk = 0;
+    SkyABCD *d_abcd = nullptr; SkyABCD *h_abcd = nullptr;   // per sky group of the current call (capacity sky_cap)
+    double mom[FSTAT_MAX_DET][MOM_TERMS];                   // antenna moment matrices M_X (sky_kernels.cuh)
+    bool pending_edom = false;                              // a template since the last sync had D <= 0
     TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
-    int *d_err = nullptr;
     float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
     uint32_t *d_gmax = nullptr;       // top-k: per-group maxima of the rows in flight [n_inflight][n_groups]
     HostRing ring;
@@ -56,7 +56,6 @@ struct fstat_plan {
     // pinned staging
     SkyConst *h_sky = nullptr; TmplDesc *h_tmpl = nullptr;
     cudaEvent_t staging_ev = nullptr; cudaEvent_t chunk_ev = nullptr;
-    int *h_err = nullptr;
     int64_t launches = 0;
     std::string err;
     // optional per-kernel-class timing (fstat_set_profile)
@@ -154,6 +153,47 @@ void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *s
     }
 }
 
+// A, B, C, D of one sky position from the moment matrices: A = sum_X alpha_X^T M_X alpha_X etc., with
+// alpha_X, beta_X the coefficients of a_X(t), b_X(t) in the basis (1, cos 2th, sin 2th, cos th, sin th).
+void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
+    double A = 0, B = 0, C = 0;
+    const double C1 = cos(alpha), S1 = sin(alpha), C2 = cos(2 * alpha), S2 = sin(2 * alpha);
+    for (int X = 0; X < p->g.n_det; ++X) {
+        const fstat_detector_t &d = p->det[X];
+        const double lam = d.lat_rad, gam = d.xarm_azimuth_rad + 0.75 * M_PI;
+        const double s2g = sin(2 * gam), c2g = cos(2 * gam);
+        const double ac0 = 0.75 * s2g * cos(lam) * cos(lam) * cos(delta) * cos(delta);
+        const double ac1 = s2g * (3.0 - cos(2 * lam)) * (3.0 - cos(2 * delta)) / 16.0;
+        const double ac2 = -0.25 * c2g * sin(lam) * (3.0 - cos(2 * delta));
+        const double ac3 = 0.25 * s2g * sin(2 * lam) * sin(2 * delta);
+        const double ac4 = -0.5 * c2g * cos(lam) * sin(2 * delta);
+        const double bc0 = c2g * sin(lam) * sin(delta);
+        const double bc1 = 0.25 * s2g * (3.0 - cos(2 * lam)) * sin(delta);
+        const double bc2 = c2g * cos(lam) * cos(delta);
+        const double bc3 = 0.5 * s2g * sin(2 * lam) * cos(delta);
+        // h = alpha - th:  cos 2h = C2 cos 2th + S2 sin 2th,  sin 2h = S2 cos 2th - C2 sin 2th, same for h
+        const double av[5] = {ac0, ac1 * C2 + ac2 * S2, ac1 * S2 - ac2 * C2, ac3 * C1 + ac4 * S1, ac3 * S1 - ac4 * C1};
+        const double bv[5] = {0.0, bc0 * C2 + bc1 * S2, bc0 * S2 - bc1 * C2, bc2 * C1 + bc3 * S1, bc2 * S1 - bc3 * C1};
+        double M[5][5];
+        int q = 0;
+        for (int r = 0; r < 5; ++r)
+            for (int cc = r; cc < 5; ++cc) { M[r][cc] = M[cc][r] = p->mom[X][q++]; }
+        for (int r = 0; r < 5; ++r)
+            for (int cc = 0; cc < 5; ++cc) {
+                A += av[r] * M[r][cc] * av[cc];
+                B += bv[r] * M[r][cc] * bv[cc];
+                C += av[r] * M[r][cc] * bv[cc];
+            }
+    }
+    out->A = A; out->B = B; out->C = C; out->D = A * B - C * C;
+    out->bad = !(out->D > 0.0);
+    if (out->bad) {
+        out->b_over_d = out->a_over_d = out->two_c_over_d = std::nanf("");
+    } else {
+        out->b_over_d = (float)(B / out->D); out->a_over_d = (float)(A / out->D); out->two_c_over_d = (float)(2.0 * C / out->D);
+    }
+}
+
 // Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
 template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN, LOGT>;
@@ -198,9 +238,9 @@ int tile_log1(const fstat_plan *p) { return p->g.log_n1 == 12 ? 13 : p->g.log_ti
 int tile_log2(const fstat_plan *p) { return p->g.log_n2 == 12 ? 13 : p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
-int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
+int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
     FftArgs a{};
-    a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd;
+    a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd + g0;
     a.twoF = rows; a.twoF_stride = row_stride; a.gmax = gmax;
     a.n_fft = p->g.n_fft; a.n_src = p->g.n_src; a.n_bins = p->g.n_bins; a.k_margin = p->g.k_margin;
     a.dt = p->g.dt;
@@ -216,7 +256,7 @@ int launch_fft_chunk(fstat_plan *p, int t0, int nt, float *rows, int64_t row_str
     return FSTAT_OK;
 }
 
-// Sky-dependent kernels for sky groups [g0, g0+ng) -> S slots 0..ng-1, abcd slots 0..ng-1.
+// Sky-dependent kernel for sky groups [g0, g0+ng) -> S slots 0..ng-1.
 int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) {
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
@@ -224,10 +264,7 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) 
     if (g.dterms == 8) sky_resample_kernel<8><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
     else if (g.dterms == 16) sky_resample_kernel<16><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
     else sky_resample_kernel<0><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
-    dim3 grid2(p->abc_nblk, ng);
-    sky_abc_partial_kernel<<<grid2, ABC_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_wslot, p->d_abc_partial);
-    sky_abc_finalize_kernel<<<ng, 256, 0, p->stream>>>(p->d_abc_partial, p->abc_nblk, p->d_abcd, p->d_err);
-    p->launches += 3;
+    p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
 }
@@ -245,10 +282,14 @@ int ensure_tmpl_capacity(fstat_plan *p, size_t n_tmpl, size_t n_groups) {
     if (n_groups > p->sky_cap) {
         if (p->d_sky) cudaFree(p->d_sky);
         if (p->h_sky) cudaFreeHost(p->h_sky);
-        p->d_sky = nullptr; p->h_sky = nullptr; p->sky_cap = 0;
+        if (p->d_abcd) cudaFree(p->d_abcd);
+        if (p->h_abcd) cudaFreeHost(p->h_abcd);
+        p->d_sky = nullptr; p->h_sky = nullptr; p->d_abcd = nullptr; p->h_abcd = nullptr; p->sky_cap = 0;
         const size_t cap = n_groups + n_groups / 2 + 16;
         CUDA_TRY(p, cudaMalloc(&p->d_sky, cap * sizeof(SkyConst)));
         CUDA_TRY(p, cudaMallocHost(&p->h_sky, cap * sizeof(SkyConst)));
+        CUDA_TRY(p, cudaMalloc(&p->d_abcd, cap * sizeof(SkyABCD)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_abcd, cap * sizeof(SkyABCD)));
         p->sky_cap = cap;
     }
     return FSTAT_OK;
@@ -329,6 +370,8 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     CUDA_TRY(p, cudaEventSynchronize(p->staging_ev));
     for (size_t gi = 0; gi < groups.size(); ++gi) {
         fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &p->h_sky[gi]);
+        sky_abcd(p, groups[gi].alpha, groups[gi].delta, &p->h_abcd[gi]);
+        if (p->h_abcd[gi].bad) p->pending_edom = true;
         for (int t = groups[gi].first; t < groups[gi].first + groups[gi].count; ++t) {
             p->h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
             p->h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
@@ -337,6 +380,7 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         }
     }
     CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, p->h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_abcd, p->h_abcd, groups.size() * sizeof(SkyABCD), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaEventRecord(p->staging_ev, p->stream));
 
@@ -368,15 +412,15 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         for (int t0 = t_begin; t0 < t_end; t0 += TB) {
             const int nt = std::min(TB, t_end - t0);
             if (out.mode == OUT_DEV_ROWS) {
-                rc = launch_fft_chunk(p, t0, nt, out.rows + (int64_t)t0 * nb, nb);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb);
                 if (rc) return rc;
             } else if (out.mode == OUT_HOST_ROWS) {
                 if (ring_fill + nt > p->ring.rows) { rc = flush_ring(); if (rc) return rc; }
-                rc = launch_fft_chunk(p, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb);
                 if (rc) return rc;
                 ring_fill += nt;
             } else {
-                rc = launch_fft_chunk(p, t0, nt, p->d_rows, nb, p->d_gmax);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->d_rows, nb, p->d_gmax);
                 if (rc) return rc;
                 ProfScope ps(p, 3);
                 const TopkGeom tg = topk_geom(p);
@@ -400,13 +444,13 @@ void destroy_impl(fstat_plan *p) {
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
     cudaFree(p->d_series); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
-    cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd); cudaFree(p->d_abc_partial);
-    cudaFree(p->d_tmpl); cudaFree(p->d_err); cudaFree(p->d_rows); cudaFree(p->d_gmax);
+    cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
+    cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
     for (int i = 0; i < 2; ++i) { cudaFree(p->ring.buf[i]); if (p->ring.done[i]) cudaEventDestroy(p->ring.done[i]); }
     if (p->h_sky) cudaFreeHost(p->h_sky);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
-    if (p->h_err) cudaFreeHost(p->h_err);
+    if (p->h_abcd) cudaFreeHost(p->h_abcd);
     if (p->staging_ev) cudaEventDestroy(p->staging_ev);
     if (p->chunk_ev) cudaEventDestroy(p->chunk_ev);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
@@ -567,12 +611,27 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
     SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
     SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
-    SETUP_TRY(cudaMalloc(&p->d_abcd, (size_t)p->n_sky_slots * sizeof(SkyABCD)));
-    p->abc_nblk = (int)((n_samples * n_det + ABC_THREADS * ABC_PER_THREAD - 1) / (ABC_THREADS * ABC_PER_THREAD));
-    SETUP_TRY(cudaMalloc(&p->d_abc_partial, (size_t)p->n_sky_slots * p->abc_nblk * 3 * sizeof(double)));
-    SETUP_TRY(cudaMalloc(&p->d_err, sizeof(int)));
-    SETUP_TRY(cudaMemsetAsync(p->d_err, 0, sizeof(int), p->stream));
-    SETUP_TRY(cudaMallocHost(&p->h_err, sizeof(int)));
+    {   // antenna moment matrices M_X (sky_kernels.cuh), once per plan
+        const int nblk = (int)((n_samples + MOM_THREADS * MOM_PER_THREAD - 1) / (MOM_THREADS * MOM_PER_THREAD));
+        double *d_part = nullptr, *d_lon = nullptr;
+        std::vector<double> lon(n_det), part((size_t)n_det * nblk * MOM_TERMS);
+        for (int X = 0; X < n_det; ++X) lon[X] = det[X].lon_east_rad;
+        SETUP_TRY(cudaMalloc(&d_part, part.size() * sizeof(double)));
+        SETUP_TRY(cudaMalloc(&d_lon, n_det * sizeof(double)));
+        SETUP_TRY(cudaMemcpyAsync(d_lon, lon.data(), n_det * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+        antenna_moments_kernel<<<dim3(nblk, n_det), MOM_THREADS, 0, p->stream>>>(g, p->d_wslot, d_lon, d_part);
+        ++p->launches;
+        SETUP_TRY(cudaGetLastError());
+        SETUP_TRY(cudaMemcpyAsync(part.data(), d_part, part.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+        SETUP_TRY(cudaStreamSynchronize(p->stream));
+        cudaFree(d_part); cudaFree(d_lon);
+        for (int X = 0; X < n_det; ++X)
+            for (int q = 0; q < MOM_TERMS; ++q) {
+                double t = 0.0;
+                for (int b = 0; b < nblk; ++b) t += part[((size_t)X * nblk + b) * MOM_TERMS + q];
+                p->mom[X][q] = t;
+            }
+    }
     SETUP_TRY(cudaEventRecord(p->staging_ev, p->stream));
     // the caller may free its buffers when we return
     SETUP_TRY(cudaStreamSynchronize(p->stream));
@@ -639,7 +698,7 @@ int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta, float *S_
     rc = launch_sky_batch(plan, 0, 1, (float4 *)S_dev, 0);
     if (rc) return rc;
     SkyABCD r;
-    CUDA_TRY(plan, cudaMemcpyAsync(&r, plan->d_abcd, sizeof(SkyABCD), cudaMemcpyDeviceToHost, plan->stream));
+    sky_abcd(plan, alpha, delta, &r);
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
     abcd_host[0] = r.A; abcd_host[1] = r.B; abcd_host[2] = r.C; abcd_host[3] = r.D;
     return FSTAT_OK;
@@ -647,10 +706,10 @@ int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta, float *S_
 
 int fstat_sync(fstat_plan_t *plan) {
     if (!plan) return FSTAT_EINVAL;
-    CUDA_TRY(plan, cudaMemcpyAsync(plan->h_err, plan->d_err, sizeof(int), cudaMemcpyDeviceToHost, plan->stream));
-    CUDA_TRY(plan, cudaMemsetAsync(plan->d_err, 0, sizeof(int), plan->stream));
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
-    if (*plan->h_err) return fail(plan, FSTAT_EDOM, "antenna determinant D <= 0 for at least one template (outputs are NaN)");
+    const bool bad = plan->pending_edom;
+    plan->pending_edom = false;
+    if (bad) return fail(plan, FSTAT_EDOM, "antenna determinant D <= 0 for at least one template (outputs are NaN)");
     return FSTAT_OK;
 }
 

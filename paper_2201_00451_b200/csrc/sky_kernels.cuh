@@ -249,83 +249,53 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
     S[(int64_t)blockIdx.y * g.n_fft + off] = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
 }
 
-// A, B, C (eq. 8): sums of w a^2, w b^2, w a b over the valid detector-frame samples.
-// grid = (nblk, n_sky); each block writes one double3 partial; finalize reduces them in
-// a fixed order (deterministic).
-#define ABC_THREADS 256
-#define ABC_PER_THREAD 8
-__global__ void __launch_bounds__(ABC_THREADS)
-sky_abc_partial_kernel(PlanGeom g, const SkyConst *__restrict__ skies, const float *__restrict__ wslot,
-                       double *__restrict__ partial /* [n_sky][gridDim.x][3] */) {
-    const SkyConst &sc = skies[blockIdx.y];
-    const int64_t total = g.n_samples * g.n_det;
-    const double inv2pi = 0.15915494309189533577;
-    float sA = 0.f, sB = 0.f, sC = 0.f;
-    const int64_t base = (int64_t)blockIdx.x * (ABC_THREADS * ABC_PER_THREAD);
+// A, B, C (eq. 8, S11): sums of w a^2, w b^2, w a b over the valid detector-frame
+// samples.  a(t) and b(t) are linear in the basis u(t) = (1, cos 2th, sin 2th, cos th, sin th) of the
+// site's sidereal angle th(t) = gmst0 + omega_rot t' + lon_X, with coefficients that depend on the sky
+// position only, so  sum_j w_j a_j^2 = alpha^T M_X alpha  with the sky-independent moment matrix
+// M_X = sum_j w_j u_j u_j^T.  This kernel accumulates the 15 distinct entries of M_X once per plan (fp64);
+// per sky position A, B, C, D then cost O(25 n_det) flops on the host (fstat_capi.cu).
+// grid = (nblk, n_det); each block writes its 15 partial sums; the host adds them in a fixed order.
+#define MOM_THREADS 256
+#define MOM_PER_THREAD 8
+#define MOM_TERMS 15
+__global__ void __launch_bounds__(MOM_THREADS)
+antenna_moments_kernel(PlanGeom g, const float *__restrict__ wslot, const double *__restrict__ lon,
+                       double *__restrict__ partial /* [n_det][gridDim.x][15] */) {
+    const int X = blockIdx.y;
+    double acc[MOM_TERMS];
+#pragma unroll
+    for (int q = 0; q < MOM_TERMS; ++q) acc[q] = 0.0;
+    const int64_t base = (int64_t)blockIdx.x * (MOM_THREADS * MOM_PER_THREAD);
 #pragma unroll 1
-    for (int i = 0; i < ABC_PER_THREAD; ++i) {
-        const int64_t idx = base + i * ABC_THREADS + threadIdx.x;
-        if (idx >= total) break;
-        const int X = (int)(idx / g.n_samples);
-        const int64_t j = idx - (int64_t)X * g.n_samples;
+    for (int i = 0; i < MOM_PER_THREAD; ++i) {
+        const int64_t j = base + i * MOM_THREADS + threadIdx.x;
+        if (j >= g.n_samples) break;
         const double tp = (double)j * g.dt;
         const int slot = min((int)floor(tp * g.inv_t_sft), g.n_slots - 1);
-        const float w = wslot[X * g.n_slots + slot];
-        if (w == 0.f) continue;
-        double rev = (g.gmst0 + g.omega_rot * tp) * inv2pi;
-        rev -= floor(rev);
-        float sth, cth;
-        sincospif(2.0f * (float)rev, &sth, &cth);
-        float a, b;
-        antenna_ab(sc, X, cth, sth, a, b);
-        sA = fmaf(w * a, a, sA); sB = fmaf(w * b, b, sB); sC = fmaf(w * a, b, sC);
-    }
-    __shared__ double red[3][ABC_THREADS / 32];
-    double dA = sA, dB = sB, dC = sC;
+        const double w = (double)wslot[X * g.n_slots + slot];
+        if (w == 0.0) continue;
+        double s1, c1;
+        sincos(g.gmst0 + g.omega_rot * tp + lon[X], &s1, &c1);
+        const double u[5] = {1.0, c1 * c1 - s1 * s1, 2.0 * s1 * c1, c1, s1};
+        int q = 0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        dA += __shfl_down_sync(0xffffffffu, dA, o);
-        dB += __shfl_down_sync(0xffffffffu, dB, o);
-        dC += __shfl_down_sync(0xffffffffu, dC, o);
+        for (int r = 0; r < 5; ++r)
+#pragma unroll
+            for (int c = r; c < 5; ++c) acc[q++] += w * u[r] * u[c];
     }
-    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = dA; red[1][threadIdx.x >> 5] = dB; red[2][threadIdx.x >> 5] = dC; }
+    __shared__ double red[MOM_TERMS][MOM_THREADS / 32];
+#pragma unroll
+    for (int q = 0; q < MOM_TERMS; ++q) {
+        double v = acc[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) red[q][threadIdx.x >> 5] = v;
+    }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        double tA = 0, tB = 0, tC = 0;
-        for (int wv = 0; wv < ABC_THREADS / 32; ++wv) { tA += red[0][wv]; tB += red[1][wv]; tC += red[2][wv]; }
-        double *p = partial + ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * 3;
-        p[0] = tA; p[1] = tB; p[2] = tC;
-    }
-}
-
-// One block per sky: fixed-order tree reduction of the partials, then the eq. 8 coefficients.
-__global__ void __launch_bounds__(256)
-sky_abc_finalize_kernel(const double *__restrict__ partial, int nblk, SkyABCD *__restrict__ out, int *__restrict__ err_flag) {
-    __shared__ double red[3][256];
-    const double *p = partial + (int64_t)blockIdx.x * nblk * 3;
-    double tA = 0, tB = 0, tC = 0;
-    for (int i = threadIdx.x; i < nblk; i += 256) { tA += p[i * 3]; tB += p[i * 3 + 1]; tC += p[i * 3 + 2]; }
-    red[0][threadIdx.x] = tA; red[1][threadIdx.x] = tB; red[2][threadIdx.x] = tC;
-    __syncthreads();
-    for (int s = 128; s > 0; s >>= 1) {
-        if (threadIdx.x < s) {
-            red[0][threadIdx.x] += red[0][threadIdx.x + s];
-            red[1][threadIdx.x] += red[1][threadIdx.x + s];
-            red[2][threadIdx.x] += red[2][threadIdx.x + s];
-        }
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) {
-        SkyABCD r;
-        r.A = red[0][0]; r.B = red[1][0]; r.C = red[2][0];
-        r.D = r.A * r.B - r.C * r.C;
-        r.bad = !(r.D > 0.0);
-        if (r.bad) {
-            r.b_over_d = r.a_over_d = r.two_c_over_d = __int_as_float(0x7fc00000);
-            atomicExch(err_flag, 1);
-        } else {
-            r.b_over_d = (float)(r.B / r.D); r.a_over_d = (float)(r.A / r.D); r.two_c_over_d = (float)(2.0 * r.C / r.D);
-        }
-        out[blockIdx.x] = r;
+    if (threadIdx.x < MOM_TERMS) {
+        double t = 0.0;
+        for (int wv = 0; wv < MOM_THREADS / 32; ++wv) t += red[threadIdx.x][wv];
+        partial[((int64_t)X * gridDim.x + blockIdx.x) * MOM_TERMS + threadIdx.x] = t;
     }
 }
