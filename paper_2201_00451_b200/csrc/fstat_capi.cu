@@ -197,21 +197,22 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
 // Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
 template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN, LOGT>;
+    constexpr int SMEM = C::SMEM_BYTES;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
     auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT> : fft_pass1_kernel<LOGN, LOGT>;
     if (configured_dev != p->device) {
-        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         int per_sm = 0;
-        CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, C::SMEM_BYTES));
+        CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, SMEM));
         resident = (per_sm > 0 ? per_sm : 1) * p->n_sm;
         configured_dev = p->device;
     }
     a.log_tiles = ilog2(tiles_per_tmpl);
     a.n_tiles = tiles_per_tmpl * n_t;
     const int grid = a.n_tiles < resident ? a.n_tiles : resident;
-    kern<<<grid, C::NT, C::SMEM_BYTES, p->stream>>>(a);
+    kern<<<grid, C::NT, SMEM, p->stream>>>(a);
     ++p->launches;
     return FSTAT_OK;
 }
@@ -230,6 +231,8 @@ template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a
         case 10 * 16 + 12: rc = launch_pass<10, 12, P2>(__VA_ARGS__); break;                     \
         case 11 * 16 + 12: rc = launch_pass<11, 12, P2>(__VA_ARGS__); break;                     \
         case 12 * 16 + 13: rc = launch_pass<12, 13, P2>(__VA_ARGS__); break;                     \
+        case 11 * 16 + 13: rc = launch_pass<11, 13, P2>(__VA_ARGS__); break;                     \
+        case 10 * 16 + 13: rc = launch_pass<10, 13, P2>(__VA_ARGS__); break;                     \
         default: rc = fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination"); break;    \
     }
 
@@ -561,7 +564,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
     // 2^11-element tiles.  Split per size as measured on B200 (profiles/r01_v3_experiments.md, section 4).
     g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10
-             : L == 22 ? (2 * n_bins > n_fft ? 10 : 11) : L - 12;
+             : L - 11 <= 12 ? 11 : 12;
     { const char *e = getenv("FSTAT_LOGN2"); if (e && atoi(e) >= 6 && atoi(e) <= 12 && L - atoi(e) >= 6 && L - atoi(e) <= 12) g.log_n2 = atoi(e); }
     g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
     {   // tile sizes of the two FFT passes (profiles/r01_v3_experiments.md): 2^11-element tiles (128 threads, 4 CTAs per
@@ -569,10 +572,10 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
         g.log_tile1 = g.log_n1 <= 10 ? 11 : 12;
-        g.log_tile2 = 12;
+        g.log_tile2 = (L == 22 && 2 * n_bins > n_fft) ? 13 : 12;    // full-band 2^22 (config 4): 4 rows per tile, 16-byte 2F runs
         const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
         if (e1 && (atoi(e1) == 11 || atoi(e1) == 12) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
-        if (e2 && (atoi(e2) == 11 || atoi(e2) == 12) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
+        if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
     }
     g.log_w1 = tile_log1(p) - g.log_n1; g.log_w2 = tile_log2(p) - g.log_n2;
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
