@@ -571,8 +571,11 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
-        g.log_tile1 = g.log_n1 <= 10 ? 11 : 12;
         g.log_tile2 = (L == 22 && 2 * n_bins > n_fft) ? 13 : 12;    // full-band 2^22 (config 4): 4 rows per tile, 16-byte 2F runs
+        // pass 1: 2^11 tiles when its transposed store still writes >= 32-byte runs (W2 >= 2 rows per pass-2 tile
+        // when the pass-1 tile holds a single column)
+        const int w2_rows = 1 << ((g.log_n2 == 12 ? 13 : g.log_tile2) - g.log_n2);
+        g.log_tile1 = (g.log_n1 <= 10 || (g.log_n1 == 11 && w2_rows >= 4)) ? 11 : 12;
         const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
         if (e1 && (atoi(e1) == 11 || atoi(e1) == 12) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
         if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
