@@ -88,6 +88,22 @@ def algorithmic_bytes(p):
     return b1, b2
 
 
+def ncu_traffic(cls: str, n_fft: int, launches: int, templates: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of this kernel class from the committed
+    `ncu --set full` capture (profiles/r01_traffic.csv holds bytes per template; a launch of the timed run
+    processes templates/launches of them).  None when no capture exists for this FFT length."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    try:
+        for line in open(path):
+            f = [c.strip() for c in line.split(",")]
+            if len(f) >= 4 and f[0] == cls and f[1].isdigit() and int(f[1]) == n_fft:
+                per_t = float(f[2]) + float(f[3])
+                return per_t * templates / max(launches, 1), "profiles/r01_traffic.csv (ncu --set full, per template x templates per launch)"
+    except OSError:
+        pass
+    return None, None
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -277,9 +293,16 @@ def run_ours(args):
         dom = max(("fft_pass1", "fft_pass2"), key=lambda c: prof[c][0])
         ach = kernels[dom]["achieved_gbs"]
         both = (b1 + b2) * n_t * args.steps / ((prof["fft_pass1"][0] + prof["fft_pass2"][0]) * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": None, "peak_source": peak_src,
+        # fp32 work of the two FFTs of a template (2 x 5 N log2 N flop) against the plain-FMA peak
+        fft_ms = prof["fft_pass1"][0] + prof["fft_pass2"][0]
+        flops = 2 * 5.0 * p.n_fft * float(np.log2(p.n_fft)) * n_t * args.steps
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        traffic, traffic_src = ncu_traffic(dom, p.n_fft, kernels[dom]["launches"], n_t * args.steps)
+        roofline = {"bound": "hbm", "kernel": dom + "_kernel", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                     "fft_pair_achieved": both, "fft_pair_frac": both / peak,
+                    "alu_tflops": flops / (fft_ms * 1e-3) / 1e12, "alu_peak_tflops": alu_peak,
+                    "alu_frac": flops / (fft_ms * 1e-3) / 1e12 / alu_peak,
                     "share_of_step": prof[dom][0] / total_ms if world == 1 else None}
 
     # ---- end to end through the host-buffer entry point (pinned host 2F, D2H inside the timed region)
@@ -313,6 +336,27 @@ def run_ours(args):
                "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(d2h),
                "api": api + "; the series is uploaded once by fstat_setup (PAPER.md:93) and is not part of a step"}
 
+    # ---- context only: the library FFT alone (cuFFT through torch.fft) on the same shape: two batched complex64
+    # transforms of n_fft points per template, nothing else of the path (no resampling, phases or 2F)
+    cufft = None
+    if args.cufft_compare and rank == 0:
+        nb_t = max(1, min(32, (1 << 28) // p.n_fft))
+        x = torch.randn((2 * nb_t, p.n_fft), dtype=torch.complex64, device="cuda")
+        for _ in range(3):
+            y = torch.fft.fft(x)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(10):
+            y = torch.fft.fft(x)
+        e1.record()
+        torch.cuda.synchronize()
+        us = 1e3 * e0.elapsed_time(e1) / 10 / nb_t
+        cufft = {"us_per_template_two_ffts": us, "ours_us_per_template_whole_path": 1e3 * ms_per_step / n_t,
+                 "note": "torch.fft.fft (cuFFT) on [2 x %d, %d] complex64, out of place; comparison baseline only, "
+                         "not on the product path" % (nb_t, p.n_fft)}
+        del x, y
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(p, args.cpu_templates)
@@ -329,7 +373,7 @@ def run_ours(args):
                            "l2": "256 MiB flush buffer written between timed steps; each step also writes "
                                  f"{n_t * nb * 4 / 1e9:.2f} GB of 2F (> L2)"},
                 "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
-                "cpu_baseline": cpu}
+                "cpu_baseline": cpu, "cufft_compare": cufft}
         print(json.dumps(line))
     plan.close()
     if world > 1:
@@ -350,6 +394,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-events", action="store_true")
+    ap.add_argument("--cufft-compare", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
