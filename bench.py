@@ -390,7 +390,7 @@ def main():
     ap.add_argument("--inflight", type=int, default=0)
     ap.add_argument("--mode", default="full", choices=["full", "topk"])
     ap.add_argument("--k", type=int, default=8)
-    ap.add_argument("--cpu-templates", type=int, default=8)
+    ap.add_argument("--cpu-templates", type=int, default=32)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-events", action="store_true")
