@@ -231,14 +231,15 @@ template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a
         case 10 * 16 + 12: rc = launch_pass<10, 12, P2>(__VA_ARGS__); break;                     \
         case 11 * 16 + 12: rc = launch_pass<11, 12, P2>(__VA_ARGS__); break;                     \
         case 12 * 16 + 13: rc = launch_pass<12, 13, P2>(__VA_ARGS__); break;                     \
+        case 12 * 16 + 12: rc = launch_pass<12, 12, P2>(__VA_ARGS__); break;                     \
         case 11 * 16 + 13: rc = launch_pass<11, 13, P2>(__VA_ARGS__); break;                     \
         case 10 * 16 + 13: rc = launch_pass<10, 13, P2>(__VA_ARGS__); break;                     \
         default: rc = fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination"); break;    \
     }
 
 // log2 of the tile size used for a sub-FFT of length 2^logn under the plan's tile setting
-int tile_log1(const fstat_plan *p) { return p->g.log_n1 == 12 ? 13 : p->g.log_tile1; }
-int tile_log2(const fstat_plan *p) { return p->g.log_n2 == 12 ? 13 : p->g.log_tile2; }
+int tile_log1(const fstat_plan *p) { return p->g.log_tile1; }
+int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
 int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
@@ -563,7 +564,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     // n_fft = 2^log_n1 x 2^log_n2.  Pass 2 gets the shorter transform: its tile then spans more rows, which is what
     // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
     // 2^11-element tiles.  Split per size as measured on B200 (profiles/r01_v3_experiments.md, section 4).
-    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10
+    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 20 ? 8 : L == 21 ? 10
              : L - 11 <= 12 ? 11 : 12;
     { const char *e = getenv("FSTAT_LOGN2"); if (e && atoi(e) >= 6 && atoi(e) <= 12 && L - atoi(e) >= 6 && L - atoi(e) <= 12) g.log_n2 = atoi(e); }
     g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
@@ -571,13 +572,13 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
-        g.log_tile2 = (L == 22 && 2 * n_bins > n_fft) ? 13 : 12;    // full-band 2^22 (config 4): 4 rows per tile, 16-byte 2F runs
-        // pass 1: 2^11 tiles when its transposed store still writes >= 32-byte runs (W2 >= 2 rows per pass-2 tile
-        // when the pass-1 tile holds a single column)
-        const int w2_rows = 1 << ((g.log_n2 == 12 ? 13 : g.log_tile2) - g.log_n2);
-        g.log_tile1 = (g.log_n1 <= 10 || (g.log_n1 == 11 && w2_rows >= 4)) ? 11 : 12;
+        g.log_tile2 = (g.log_n2 == 12 || (L == 22 && 2 * n_bins > n_fft)) ? 13 : 12;   // full-band 2^22 (config 4): 4 rows per tile, 16-byte 2F runs
+        // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
+        // of a single column needs >= 4 rows per pass-2 tile
+        const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
+        g.log_tile1 = g.log_n1 <= 10 ? 11 : (w2_rows >= 4 ? g.log_n1 : g.log_n1 + 1);
         const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
-        if (e1 && (atoi(e1) == 11 || atoi(e1) == 12) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
+        if (e1 && (atoi(e1) >= 11 && atoi(e1) <= 13) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
         if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
     }
     g.log_w1 = tile_log1(p) - g.log_n1; g.log_w2 = tile_log2(p) - g.log_n2;

@@ -59,6 +59,13 @@ def test_parity_large_fft_one_template(log_nfft):
     _check_bank(p, [p.injection_template])
 
 
+def test_parity_maximum_fft_length():
+    # n_fft = 2^24 = 2^12 x 2^12: the largest size fstat_setup accepts (both passes run their 2^12-point kernels)
+    p = synth.small_problem(seed=124, n_det=1, n_samples=int(0.75 * (1 << 24)), dt=0.5, n_fft=1 << 24, n_templates=1,
+                            gap_frac=0.4, rho=15.0)
+    _check_bank(p, [0])
+
+
 def test_parity_fs_equals_band_full_output():
     # config-4 shape: band = sample rate, every FFT output is a bin, f_het at band centre
     p = synth.small_problem(seed=3, n_samples=30000, dt=0.5, n_fft=1 << 16, n_templates=2, band=2.0, rho=10.0)
