@@ -409,12 +409,13 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 float4 *dst = colbase + ((int64_t)(i >> lw2) << (ln2 + lw2)) + (i & ((1 << lw2) - 1));
                 const int64_t rstride = (int64_t)PI::NI << ln2;           // valid when NI is a multiple of W2
                 const bool affine = (PI::NI >> lw2) != 0;
+                float4 *orun = dst;
 #pragma unroll
-                for (int r = 0; r < RL; ++r) {
+                for (int r = 0; r < RL; ++r, orun += rstride) {
                     float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
                     pcmul(xx, yy, tw);
                     const int m1 = i + r * PI::NI;
-                    float4 *o = affine ? dst + r * rstride
+                    float4 *o = affine ? orun
                                        : colbase + ((int64_t)(m1 >> lw2) << (ln2 + lw2)) + (m1 & ((1 << lw2) - 1));
                     st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
                     if (r + 1 < RL) tw = cmul(tw, step);
@@ -455,14 +456,16 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
             using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
             float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride;
             float tmax = __int_as_float(0xff800000);
+            const int nb = (int)p.n_bins;                       // bins fit 32 bits (n_fft <= 2^24)
+            const int q_step = PL << p.log_other;               // out_idx(i, r) is linear in r with slope P
 #pragma unroll
             for (int bb = 0; bb < PI::NB; ++bb) {
                 int i, w;
                 PI::item(bb, i, w);
+                int q = (PI::out_idx(i, 0) << p.log_other) + m1_0 + w;
 #pragma unroll
-                for (int r = 0; r < RL; ++r) {
-                    const int64_t q = ((int64_t)PI::out_idx(i, r) << p.log_other) + m1_0 + w;
-                    if (q < p.n_bins) {
+                for (int r = 0; r < RL; ++r, q += q_step) {
+                    if (q < nb) {
                         const float2 fa = make_float2(a[bb * RL + r].x, b[bb * RL + r].x);    // unpack (re, im) of Fa, Fb
                         const float2 fb = make_float2(a[bb * RL + r].y, b[bb * RL + r].y);
                         const float twoF = b_over_d * (fa.x * fa.x + fa.y * fa.y) + a_over_d * (fb.x * fb.x + fb.y * fb.y)
