@@ -30,7 +30,6 @@ struct HostRing {            // device row buffers for the *_host variants
 
 struct fstat_plan {
     PlanGeom g{};
-    WinTable win{};
     cudaStream_t stream = nullptr;
     cudaStream_t copy_stream = nullptr;
     fstat_detector_t det[FSTAT_MAX_DET];
@@ -40,6 +39,7 @@ struct fstat_plan {
     int n_sm = 148;
     // device memory
     float2 *d_series = nullptr;
+    float2 *d_farrow = nullptr;       // [n_det][N+1][FARROW_NC] Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
     float4 *d_S = nullptr;   int n_sky_slots = 0;
@@ -125,6 +125,39 @@ std::vector<float2> make_twiddles(int logn) {
         P *= R;
     }
     return tw;
+}
+
+// Farrow coefficients (sky_kernels.cuh): c_m(d) = sinc(d-m) [0.54 + 0.46 cos(pi (d-m)/(D+1/2))] on d in [-1/2, 1/2]
+// as sum_p a[m][p] d^p: Chebyshev interpolation at FARROW_NC nodes in t = 2d, converted to powers of d.  fp64.
+std::vector<float> farrow_coefficients(int dterms) {
+    const int Q = FARROW_NC;
+    std::vector<float> out((size_t)(2 * dterms + 1) * Q);
+    // T_k(t) as polynomials in t
+    std::vector<std::vector<double>> Tk(Q, std::vector<double>(Q, 0.0));
+    Tk[0][0] = 1.0;
+    if (Q > 1) Tk[1][1] = 1.0;
+    for (int k = 2; k < Q; ++k)
+        for (int e = 0; e < Q; ++e) Tk[k][e] = (e > 0 ? 2.0 * Tk[k - 1][e - 1] : 0.0) - Tk[k - 2][e];
+    for (int m = -dterms; m <= dterms; ++m) {
+        double fv[FARROW_NC], ck[FARROW_NC];
+        for (int i = 0; i < Q; ++i) {
+            const double d = 0.5 * cos(M_PI * (i + 0.5) / Q), v = d - m;
+            const double sinc = (fabs(v) < 1e-12) ? 1.0 : sin(M_PI * v) / (M_PI * v);
+            fv[i] = sinc * (0.54 + 0.46 * cos(M_PI * v / (dterms + 0.5)));
+        }
+        for (int k = 0; k < Q; ++k) {
+            double acc = 0.0;
+            for (int i = 0; i < Q; ++i) acc += fv[i] * cos(M_PI * k * (i + 0.5) / Q);
+            ck[k] = (k == 0 ? 1.0 : 2.0) * acc / Q;
+        }
+        double pw = 1.0;                                     // t^e = (2d)^e
+        for (int e = 0; e < Q; ++e, pw *= 2.0) {
+            double a = 0.0;
+            for (int k = e; k < Q; ++k) a += ck[k] * Tk[k][e];
+            out[(size_t)(m + dterms) * Q + e] = (float)(a * pw);
+        }
+    }
+    return out;
 }
 
 void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *sc) {
@@ -265,9 +298,7 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) 
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
     dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
-    if (g.dterms == 8) sky_resample_kernel<8><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
-    else if (g.dterms == 16) sky_resample_kernel<16><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
-    else sky_resample_kernel<0><<<grid, SKY_THREADS, 0, p->stream>>>(g, p->win, p->d_sky + g0, p->d_series, p->d_wslot, S_dst, blocked);
+    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_farrow, p->d_wslot, S_dst, blocked);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -447,7 +478,7 @@ void destroy_impl(fstat_plan *p) {
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_series); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
+    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
     cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
@@ -593,10 +624,6 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     }
     p->eph = *eph; p->f_min = f_min; p->band = band; p->df = 1.0 / ((double)n_fft * dt);
     for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
-    for (int m = -dterms; m <= dterms; ++m) {
-        p->win.c[m + dterms] = (float)cos(M_PI * m / (dterms + 0.5));
-        p->win.s[m + dterms] = (float)sin(M_PI * m / (dterms + 0.5));
-    }
 
     SETUP_TRY(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
     SETUP_TRY(cudaEventCreateWithFlags(&p->staging_ev, cudaEventDisableTiming));
@@ -618,6 +645,19 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
     SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
     SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
+    {   // Farrow-filtered copies of the series (sky_kernels.cuh), once per plan
+        const std::vector<float> fc = farrow_coefficients(dterms);
+        float *d_fc = nullptr;
+        SETUP_TRY(cudaMalloc(&d_fc, fc.size() * sizeof(float)));
+        SETUP_TRY(cudaMemcpyAsync(d_fc, fc.data(), fc.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
+        SETUP_TRY(cudaMalloc(&p->d_farrow, (size_t)n_det * (n_samples + 1) * FARROW_NC * sizeof(float2)));
+        dim3 grid((unsigned)((n_samples + 1 + SKY_THREADS - 1) / SKY_THREADS), n_det);
+        farrow_filter_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_series, d_fc, p->d_farrow);
+        ++p->launches;
+        SETUP_TRY(cudaGetLastError());
+        SETUP_TRY(cudaStreamSynchronize(p->stream));
+        cudaFree(d_fc);
+    }
     {   // antenna moment matrices M_X (sky_kernels.cuh), once per plan
         const int nblk = (int)((n_samples + MOM_THREADS * MOM_PER_THREAD - 1) / (MOM_THREADS * MOM_PER_THREAD));
         double *d_part = nullptr, *d_lon = nullptr;

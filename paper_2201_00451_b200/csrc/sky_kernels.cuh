@@ -4,13 +4,6 @@
 #pragma once
 #include "fstat_common.cuh"
 
-// Window table, passed by value as a kernel parameter (lands in the constant bank; no
-// module-level state shared between plans).
-struct WinTable {
-    float c[2 * FSTAT_MAX_DTERMS + 1];   // cos(pi m /(D+1/2)), m = -D..D
-    float s[2 * FSTAT_MAX_DTERMS + 1];   // sin(pi m /(D+1/2))
-};
-
 // sin, cos of a small angle |e| <~ 0.1 rad in double by Taylor series (error < 1e-18 for
 // |e| < 0.05: omega_rot * Delta_max = 0.036, omega_orb * Delta_max = 1e-4).
 __device__ __forceinline__ void small_sincos(double e, double &s, double &c) {
@@ -74,65 +67,58 @@ __device__ __forceinline__ double ssb_invert_newton(const PlanGeom &g, const Sky
     return delta;
 }
 
-// sin(pi x)/(pi x) and cos(pi x) for |x| <= 1/2 as Taylor polynomials in x^2 (truncation < 4e-8 / 7e-9):
-// no division, no range reduction, relative accuracy at x -> 0 (the main tap needs sinc(d) to 1e-7).
-__device__ __forceinline__ float sinc_pi_poly(float x2) {
-    float p = 1.4842879e-4f;                  // pi^12/13!
-    p = fmaf(p, x2, -2.3460810e-3f);          // -pi^10/11!
-    p = fmaf(p, x2, 2.6147848e-2f);           // pi^8/9!
-    p = fmaf(p, x2, -1.9075182e-1f);          // -pi^6/7!
-    p = fmaf(p, x2, 8.1174243e-1f);           // pi^4/5!
-    p = fmaf(p, x2, -1.6449341f);             // -pi^2/3!
-    return fmaf(p, x2, 1.0f);
-}
-__device__ __forceinline__ float cos_pi_poly(float x2) {
-    float p = -1.0463811e-4f;                 // -pi^14/14!
-    p = fmaf(p, x2, 1.9295743e-3f);           // pi^12/12!
-    p = fmaf(p, x2, -2.5806891e-2f);          // -pi^10/10!
-    p = fmaf(p, x2, 2.3533063e-1f);           // pi^8/8!
-    p = fmaf(p, x2, -1.3352628f);             // -pi^6/6!
-    p = fmaf(p, x2, 4.0587121f);              // pi^4/4!
-    p = fmaf(p, x2, -4.9348022f);             // -pi^2/2!
-    return fmaf(p, x2, 1.0f);
-}
-
-__device__ __forceinline__ float rcp_approx(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
 #define SKY_THREADS 256
-#define SKY_WIN (SKY_THREADS + 2 * FSTAT_MAX_DTERMS + 4)
+#define FARROW_NC 10          // polynomial coefficients per tap (degree 9: 8e-8 max error for Dterms >= 8, 3e-7 for Dterms 1)
+
+// H3 in Farrow form.  The interpolation weight of tap m, c_m(d) = sinc(d-m) W(d-m) for d in [-1/2, 1/2)
+// (S6), is an entire function of d; fstat_setup expands it as c_m(d) = sum_p a[m][p] d^p
+// (Chebyshev interpolation of degree 9, converted to powers of d, fp64 -> fp32).  Then
+//     z(j0 + d) = sum_m x[j0+m] c_m(d) = sum_p d^p Y_p[j0],   Y_p[j] = sum_m a[m][p] x[j+m]:
+// the 2D+1 taps are folded, once per plan and independent of the sky position, into FARROW_NC filtered
+// copies of the series (this kernel); per SSB grid point the resampler then reads FARROW_NC complex
+// numbers (80 contiguous bytes) and runs one Horner recurrence instead of evaluating 2D+1 weights.
+//   series : [n_det][series_stride] float2 (data at +SERIES_PAD, zeros around it)
+//   coef   : [2D+1][FARROW_NC] float, row m+D
+//   Y      : [n_det][N+1][FARROW_NC] float2
+__global__ void __launch_bounds__(SKY_THREADS)
+farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float *__restrict__ coef, float2 *__restrict__ Y) {
+    __shared__ float s_coef[(2 * FSTAT_MAX_DTERMS + 1) * FARROW_NC];
+    const int D = g.dterms, X = blockIdx.y;
+    for (int e = threadIdx.x; e < (2 * D + 1) * FARROW_NC; e += SKY_THREADS) s_coef[e] = coef[e];
+    __syncthreads();
+    const int64_t j = (int64_t)blockIdx.x * SKY_THREADS + threadIdx.x;
+    if (j > g.n_samples) return;
+    const float2 *x = series + (int64_t)X * g.series_stride + SERIES_PAD + j;
+    float2 acc[FARROW_NC];
+#pragma unroll
+    for (int p = 0; p < FARROW_NC; ++p) acc[p] = make_float2(0.f, 0.f);
+    for (int m = -D; m <= D; ++m) {
+        const float2 xv = __ldg(x + m);
+        const float *c = s_coef + (m + D) * FARROW_NC;
+#pragma unroll
+        for (int p = 0; p < FARROW_NC; ++p) acc[p] = __ffma2_rn(xv, make_float2(c[p], c[p]), acc[p]);
+    }
+    float4 *out = reinterpret_cast<float4 *>(Y + ((int64_t)X * (g.n_samples + 1) + j) * FARROW_NC);
+#pragma unroll
+    for (int p = 0; p < FARROW_NC / 2; ++p) out[p] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
+}
 
 // H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
-//   series : [n_det][series_stride] float2, data starts at +SERIES_PAD (zeros around it)
+//   Y      : [n_det][N+1][FARROW_NC] float2, the Farrow-filtered series (above)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
 //            S[k2 / W1][k1][k2 % W1]
-// The 256 outputs of a block read source samples j0 - D .. j0 + D with j0 - k constant to within
-// +-1 over the block (the delay drifts by <= 1e-4 samples per sample), so the block stages one
-// window of 256 + 2D + 2 samples per detector in shared memory and every thread takes its
-// 2D+1 taps from there; a thread whose taps fall outside the window (possible only for an
-// extreme user ephemeris) reads global memory instead.
-// DC = compile-time Dterms (8, 16) or 0 for the run-time value.
 // The trigonometric base of the timing model is evaluated once per block in fp64 at the block
 // centre and rotated to each thread's tau by the small angle omega * (tau - tau_c) (Taylor
 // series, exact to 1e-18 for angles < 0.1 rad); plans whose block span is too long for that
 // (g.block_base == 0) evaluate it per thread.
-template <int DC>
 __global__ void __launch_bounds__(SKY_THREADS)
-sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ WinTable win,
-                    const SkyConst *__restrict__ skies, const float2 *__restrict__ series,
+sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const float2 *__restrict__ Y,
                     const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
-    __shared__ float2 s_win[SKY_WIN];
     __shared__ double s_base[4];
-    __shared__ long long s_r0;
-    const int D = DC ? DC : g.dterms;
     const int64_t k0 = (int64_t)blockIdx.x * SKY_THREADS;
     const int64_t k = k0 + threadIdx.x;
-    const bool live = k < g.n_src;
     const SkyConst &sc = skies[blockIdx.y];
     const int64_t krel = k - g.k_margin;
     const double tau = (double)krel * g.dt;
@@ -150,96 +136,52 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const __grid_constant__ 
     } else {
         base = ssb_base(g, tau);
     }
+    if (k >= g.n_src) return;
 
     float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
-    const float inv_dh = 1.0f / ((float)D + 0.5f);
-    // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft)
+    // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft);
     // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two)
     const uint32_t tshift = (uint32_t)(((uint64_t)g.shift_mod * (uint64_t)k) & (uint64_t)(g.n_fft - 1));
     const float shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
-    const int wlen = SKY_THREADS + 2 * D + 2;
 
     for (int X = 0; X < g.n_det; ++X) {
         double cth, sth;
         const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
         const double T = tau - delta;                       // detector epoch - t_start
-        float w = 0.f;
-        if (live && T >= 0.0 && T < g.span) {               // step 3: inside the data and not in a gap
-            const int slot = min((int)floor(T * g.inv_t_sft), g.n_slots - 1);
-            w = wslot[X * g.n_slots + slot];
-        }
+        if (!(T >= 0.0 && T < g.span)) continue;            // step 3: outside the data
+        const int slot = min((int)floor(T * g.inv_t_sft), g.n_slots - 1);
+        const float w = wslot[X * g.n_slots + slot];
+        if (w == 0.f) continue;                             // gap
         // fractional sample index u = krel - Delta/dt = j0 + d,  d in [-1/2, 1/2)
         const double v = -delta * g.inv_dt;
         const double vr = floor(v + 0.5);
         const float d = (float)(v - vr);
-        const int64_t r = (int64_t)vr;                      // j0 - krel
-        if (threadIdx.x == 0) s_r0 = r;
-        __syncthreads();
-        const int64_t r0 = s_r0;
-        // window = samples [jw, jw + wlen), jw = (k0 - K_m) + r0 - 1 - D
-        const int64_t jw = (k0 - g.k_margin) + r0 - 1 - D;
-        const float2 *xs = series + (int64_t)X * g.series_stride + SERIES_PAD;
-        for (int i = threadIdx.x; i < wlen; i += SKY_THREADS) {
-            const int64_t j = jw + i;
-            s_win[i] = (j >= -SERIES_PAD && j < g.n_samples + SERIES_PAD) ? __ldg(xs + j) : make_float2(0.f, 0.f);
-        }
-        __syncthreads();
-        if (w != 0.f) {
-            // kernel coefficients: sinc(d-m) W(d-m) = (-1)^m sin(pi d)/(pi (d-m)) * [0.54 + 0.46 cos(pi (d-m)/(D+1/2))];
-            // taps +m and -m share one reciprocal: 1/(d-m) = (d+m)/(d^2-m^2), 1/(d+m) = (d-m)/(d^2-m^2)
-            const float d2 = d * d, sincd = sinc_pi_poly(d2), spd = d * sincd;        // spd = sin(pi d)/pi
-            const float xw = d * inv_dh, xw2 = xw * xw;
-            const float cw46 = 0.46f * cos_pi_poly(xw2), sw46 = (0.46f * 3.14159265358979f) * xw * sinc_pi_poly(xw2);
-            const int rel = (int)(r - r0);
-            const bool in_win = (rel >= -1 && rel <= 1);
-            float2 z;
-            {
-                const float c0 = sincd * (0.54f + cw46);
-                const float2 x0 = in_win ? s_win[threadIdx.x + rel + 1 + D] : __ldg(xs + krel + r);
-                z = make_float2(x0.x * c0, x0.y * c0);
-            }
-            if (in_win) {
-                const float2 *xc = s_win + (threadIdx.x + rel + 1 + D);
-                float sgn = -spd;
+        const int64_t j0 = krel + (int64_t)vr;              // in [0, N] because 0 <= T < span
+        // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
+        const float4 *y = reinterpret_cast<const float4 *>(Y + ((int64_t)X * (g.n_samples + 1) + j0) * FARROW_NC);
+        float4 c[FARROW_NC / 2];
 #pragma unroll
-                for (int m = 1; m <= D; ++m) {
-                    const float fm = (float)m;
-                    const float s = sgn * rcp_approx(d2 - fm * fm);
-                    const float A = fmaf(cw46, win.c[m + D], 0.54f), B = sw46 * win.s[m + D];
-                    const float cp = s * (d + fm) * (A + B), cm = s * (d - fm) * (A - B);
-                    z = __ffma2_rn(xc[m], make_float2(cp, cp), z);
-                    z = __ffma2_rn(xc[-m], make_float2(cm, cm), z);
-                    sgn = -sgn;
-                }
-            } else {
-                const float2 *xc = xs + krel + r;
-                float sgn = -spd;
-                for (int m = 1; m <= D; ++m) {
-                    const float fm = (float)m;
-                    const float s = sgn * rcp_approx(d2 - fm * fm);
-                    const float A = fmaf(cw46, win.c[m + D], 0.54f), B = sw46 * win.s[m + D];
-                    const float cp = s * (d + fm) * (A + B), cm = s * (d - fm) * (A - B);
-                    z = __ffma2_rn(__ldg(xc + m), make_float2(cp, cp), z);
-                    z = __ffma2_rn(__ldg(xc - m), make_float2(cm, cm), z);
-                    sgn = -sgn;
-                }
-            }
-            // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
-            // (phase reduced mod 1 in fp64, then fp32: |arg| <= pi, where sin/cos.approx are good to 5e-7 abs)
-            const double cyc = g.f_het * delta;
-            float fc = (float)(cyc - floor(cyc)) + shift_cyc;
-            fc -= rintf(fc);
-            float sp, cp;
-            __sincosf(-6.283185307179586f * fc, &sp, &cp);
-            const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
-            float a, b;
-            antenna_ab(sc, X, (float)cth, (float)sth, a, b);
-            ya.x = fmaf(w * a, er, ya.x); ya.y = fmaf(w * a, ei, ya.y);
-            yb.x = fmaf(w * b, er, yb.x); yb.y = fmaf(w * b, ei, yb.y);
+        for (int p = 0; p < FARROW_NC / 2; ++p) c[p] = __ldg(y + p);
+        const float2 dd = make_float2(d, d);
+        float2 z = make_float2(c[FARROW_NC / 2 - 1].z, c[FARROW_NC / 2 - 1].w);
+#pragma unroll
+        for (int p = FARROW_NC / 2 - 1; p >= 0; --p) {
+            if (p < FARROW_NC / 2 - 1) z = __ffma2_rn(z, dd, make_float2(c[p].z, c[p].w));
+            z = __ffma2_rn(z, dd, make_float2(c[p].x, c[p].y));
         }
-        __syncthreads();                                    // window buffer is reused by the next detector
+        // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
+        // (phase reduced mod 1 in fp64, then fp32: |arg| <= pi, where sin/cos.approx are good to 5e-7 abs)
+        const double cyc = g.f_het * delta;
+        float fc = (float)(cyc - floor(cyc)) + shift_cyc;
+        fc -= rintf(fc);
+        float sp, cp;
+        __sincosf(-6.283185307179586f * fc, &sp, &cp);
+        const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
+        float a, b;
+        antenna_ab(sc, X, (float)cth, (float)sth, a, b);
+        ya.x = fmaf(w * a, er, ya.x); ya.y = fmaf(w * a, ei, ya.y);
+        yb.x = fmaf(w * b, er, yb.x); yb.y = fmaf(w * b, ei, yb.y);
     }
-    if (!live) return;
     int64_t off = k;
     if (blocked) {
         const int64_t k1 = k >> g.log_n2, k2 = k & (((int64_t)1 << g.log_n2) - 1);
