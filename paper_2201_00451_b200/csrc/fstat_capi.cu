@@ -39,6 +39,7 @@ struct fstat_plan {
     int n_sm = 148;
     // device memory
     float2 *d_series = nullptr;
+    double4 *d_base = nullptr;        // [n_src] trigonometric base of the timing model per SSB grid point
     float2 *d_farrow = nullptr;       // [n_det][N+1][FARROW_NC] Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
@@ -298,7 +299,7 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) 
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
     dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
-    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_farrow, p->d_wslot, S_dst, blocked);
+    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_base, p->d_farrow, p->d_wslot, S_dst, blocked);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -478,7 +479,7 @@ void destroy_impl(fstat_plan *p) {
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
+    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_base); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
     cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
@@ -619,8 +620,6 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         double e = wa * reach;
         g.n_newton = 0;
         while (e > 1e-11 && g.n_newton < 8) { e = 0.5 * c2 * e * e + wa * wa * wa * e; ++g.n_newton; }
-        const double half_block = 0.5 * SKY_THREADS * dt;
-        g.block_base = (fabs(eph->omega_rot) * half_block <= 0.1 && fabs(eph->omega_orb) * half_block <= 0.01) ? 1 : 0;
     }
     p->eph = *eph; p->f_min = f_min; p->band = band; p->df = 1.0 / ((double)n_fft * dt);
     for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
@@ -653,6 +652,10 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         SETUP_TRY(cudaMalloc(&p->d_farrow, (size_t)n_det * (n_samples + 1) * FARROW_NC * sizeof(float2)));
         dim3 grid((unsigned)((n_samples + 1 + SKY_THREADS - 1) / SKY_THREADS), n_det);
         farrow_filter_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_series, d_fc, p->d_farrow);
+        ++p->launches;
+        SETUP_TRY(cudaGetLastError());
+        SETUP_TRY(cudaMalloc(&p->d_base, (size_t)g.n_src * sizeof(double4)));
+        ssb_base_kernel<<<(unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), SKY_THREADS, 0, p->stream>>>(g, p->d_base);
         ++p->launches;
         SETUP_TRY(cudaGetLastError());
         SETUP_TRY(cudaStreamSynchronize(p->stream));

@@ -64,5 +64,4 @@ struct PlanGeom {
     int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
     int log_tile1, log_tile2;   // log2 of the tile size of FFT pass 1 / 2 (11 or 12; sub-FFTs of length 2^12 use 13)
     int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
-    int block_base;         // 1: trigonometric base per block + small-angle rotation per thread
 };

@@ -103,88 +103,99 @@ farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float 
     for (int p = 0; p < FARROW_NC / 2; ++p) out[p] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
 }
 
+// Trigonometric base of the timing model at every SSB grid point: (cos, sin) of the orbital phase and of the
+// Greenwich sidereal angle at tau_k.  Sky-independent: computed once per plan in fp64 (32 bytes per grid point).
+__global__ void __launch_bounds__(SKY_THREADS)
+ssb_base_kernel(PlanGeom g, double4 *__restrict__ base) {
+    const int64_t k = (int64_t)blockIdx.x * SKY_THREADS + threadIdx.x;
+    if (k >= g.n_src) return;
+    const SsbBase b = ssb_base(g, (double)(k - g.k_margin) * g.dt);
+    base[k] = make_double4(b.co, b.so, b.cr, b.sr);
+}
+
 // H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
+//   base   : [n_src] double4 from ssb_base_kernel
 //   Y      : [n_det][N+1][FARROW_NC] float2, the Farrow-filtered series (above)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
 //            S[k2 / W1][k1][k2 % W1]
-// The trigonometric base of the timing model is evaluated once per block in fp64 at the block
-// centre and rotated to each thread's tau by the small angle omega * (tau - tau_c) (Taylor
-// series, exact to 1e-18 for angles < 0.1 rad); plans whose block span is too long for that
-// (g.block_base == 0) evaluate it per thread.
+// Detectors are taken two at a time: both timing inversions first, then the 2 x 80 bytes of Farrow
+// coefficients are requested together (the kernel is bound by the latency of these L2 reads), then
+// the two Horner recurrences, phase factors and antenna weights.
 __global__ void __launch_bounds__(SKY_THREADS)
-sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const float2 *__restrict__ Y,
-                    const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
-    __shared__ double s_base[4];
-    const int64_t k0 = (int64_t)blockIdx.x * SKY_THREADS;
-    const int64_t k = k0 + threadIdx.x;
+sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ base_tab,
+                    const float2 *__restrict__ Y, const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
+    const int k = blockIdx.x * SKY_THREADS + threadIdx.x;          // n_src <= n_fft <= 2^24
+    if (k >= g.n_src) return;
     const SkyConst &sc = skies[blockIdx.y];
-    const int64_t krel = k - g.k_margin;
+    const int krel = k - (int)g.k_margin;
     const double tau = (double)krel * g.dt;
     SsbBase base;
-    if (g.block_base) {
-        const double tau_c = (double)(k0 + SKY_THREADS / 2 - g.k_margin) * g.dt;
-        if (threadIdx.x == 0) sincos(g.phi_orb0 + g.omega_orb * tau_c, &s_base[1], &s_base[0]);
-        if (threadIdx.x == 32) sincos(g.gmst0 + g.omega_rot * tau_c, &s_base[3], &s_base[2]);
-        __syncthreads();
-        double se, ce, sr, cr;
-        tiny_sincos(g.omega_orb * (tau - tau_c), se, ce);
-        small_sincos(g.omega_rot * (tau - tau_c), sr, cr);
-        base.co = s_base[0] * ce - s_base[1] * se; base.so = s_base[1] * ce + s_base[0] * se;   // angle + eps
-        base.cr = s_base[2] * cr - s_base[3] * sr; base.sr = s_base[3] * cr + s_base[2] * sr;
-    } else {
-        base = ssb_base(g, tau);
+    {
+        const double2 *bp = reinterpret_cast<const double2 *>(base_tab + k);
+        const double2 b0 = __ldg(bp), b1 = __ldg(bp + 1);
+        base.co = b0.x; base.so = b0.y; base.cr = b1.x; base.sr = b1.y;
     }
-    if (k >= g.n_src) return;
-
     float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft);
-    // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two)
-    const uint32_t tshift = (uint32_t)(((uint64_t)g.shift_mod * (uint64_t)k) & (uint64_t)(g.n_fft - 1));
+    // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32)
+    const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
     const float shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
+    const int n_rows = (int)g.n_samples + 1;
 
-    for (int X = 0; X < g.n_det; ++X) {
-        double cth, sth;
-        const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
-        const double T = tau - delta;                       // detector epoch - t_start
-        if (!(T >= 0.0 && T < g.span)) continue;            // step 3: outside the data
-        const int slot = min((int)floor(T * g.inv_t_sft), g.n_slots - 1);
-        const float w = wslot[X * g.n_slots + slot];
-        if (w == 0.f) continue;                             // gap
-        // fractional sample index u = krel - Delta/dt = j0 + d,  d in [-1/2, 1/2)
-        const double v = -delta * g.inv_dt;
-        const double vr = floor(v + 0.5);
-        const float d = (float)(v - vr);
-        const int64_t j0 = krel + (int64_t)vr;              // in [0, N] because 0 <= T < span
-        // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
-        const float4 *y = reinterpret_cast<const float4 *>(Y + ((int64_t)X * (g.n_samples + 1) + j0) * FARROW_NC);
-        float4 c[FARROW_NC / 2];
+    for (int X0 = 0; X0 < g.n_det; X0 += 2) {
+        float w[2], d[2], fc[2], ca[2], cb[2];
+        const float4 *y[2];
 #pragma unroll
-        for (int p = 0; p < FARROW_NC / 2; ++p) c[p] = __ldg(y + p);
-        const float2 dd = make_float2(d, d);
-        float2 z = make_float2(c[FARROW_NC / 2 - 1].z, c[FARROW_NC / 2 - 1].w);
-#pragma unroll
-        for (int p = FARROW_NC / 2 - 1; p >= 0; --p) {
-            if (p < FARROW_NC / 2 - 1) z = __ffma2_rn(z, dd, make_float2(c[p].z, c[p].w));
-            z = __ffma2_rn(z, dd, make_float2(c[p].x, c[p].y));
+        for (int u = 0; u < 2; ++u) {
+            const int X = min(X0 + u, g.n_det - 1);
+            double cth, sth;
+            const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
+            const double T = tau - delta;                       // detector epoch - t_start
+            w[u] = 0.f;
+            if (X0 + u < g.n_det && T >= 0.0 && T < g.span) {  // step 3: inside the data and not in a gap
+                const int slot = min((int)(T * g.inv_t_sft), g.n_slots - 1);
+                w[u] = wslot[X * g.n_slots + slot];
+            }
+            // fractional sample index u = krel - Delta/dt = j0 + d,  d in [-1/2, 1/2)
+            const double v = -delta * g.inv_dt;
+            const double vr = floor(v + 0.5);
+            d[u] = (float)(v - vr);
+            const int j0 = min(max(krel + (int)vr, 0), n_rows - 1);   // in [0, N] whenever w != 0
+            y[u] = reinterpret_cast<const float4 *>(Y + ((int64_t)X * n_rows + j0) * FARROW_NC);
+            // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
+            // (phase reduced mod 1 in fp64, then fp32)
+            const double cyc = g.f_het * delta;
+            fc[u] = (float)(cyc - floor(cyc)) + shift_cyc;
+            antenna_ab(sc, X, (float)cth, (float)sth, ca[u], cb[u]);
         }
-        // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
-        // (phase reduced mod 1 in fp64, then fp32: |arg| <= pi, where sin/cos.approx are good to 5e-7 abs)
-        const double cyc = g.f_het * delta;
-        float fc = (float)(cyc - floor(cyc)) + shift_cyc;
-        fc -= rintf(fc);
-        float sp, cp;
-        __sincosf(-6.283185307179586f * fc, &sp, &cp);
-        const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
-        float a, b;
-        antenna_ab(sc, X, (float)cth, (float)sth, a, b);
-        ya.x = fmaf(w * a, er, ya.x); ya.y = fmaf(w * a, ei, ya.y);
-        yb.x = fmaf(w * b, er, yb.x); yb.y = fmaf(w * b, ei, yb.y);
+        float4 c[2][FARROW_NC / 2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+#pragma unroll
+            for (int p = 0; p < FARROW_NC / 2; ++p) c[u][p] = __ldg(y[u] + p);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
+            const float2 dd = make_float2(d[u], d[u]);
+            float2 z = make_float2(c[u][FARROW_NC / 2 - 1].z, c[u][FARROW_NC / 2 - 1].w);
+#pragma unroll
+            for (int p = FARROW_NC / 2 - 1; p >= 0; --p) {
+                if (p < FARROW_NC / 2 - 1) z = __ffma2_rn(z, dd, make_float2(c[u][p].z, c[u][p].w));
+                z = __ffma2_rn(z, dd, make_float2(c[u][p].x, c[u][p].y));
+            }
+            float f = fc[u] - rintf(fc[u]), sp, cp;             // |arg| <= pi, where sin/cos.approx are good to 5e-7 abs
+            __sincosf(-6.283185307179586f * f, &sp, &cp);
+            const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
+            const float wa = w[u] * ca[u], wb = w[u] * cb[u];
+            ya.x = fmaf(wa, er, ya.x); ya.y = fmaf(wa, ei, ya.y);
+            yb.x = fmaf(wb, er, yb.x); yb.y = fmaf(wb, ei, yb.y);
+        }
     }
-    int64_t off = k;
+    int off = k;
     if (blocked) {
-        const int64_t k1 = k >> g.log_n2, k2 = k & (((int64_t)1 << g.log_n2) - 1);
+        const int k1 = k >> g.log_n2, k2 = k & ((1 << g.log_n2) - 1);
         off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
     }
     // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
