@@ -40,7 +40,7 @@ struct fstat_plan {
     // device memory
     float2 *d_series = nullptr;
     double4 *d_base = nullptr;        // [n_src] trigonometric base of the timing model per SSB grid point
-    float2 *d_farrow = nullptr;       // [n_det][N+1][FARROW_NC] Farrow-filtered series (sky_kernels.cuh)
+    float2 *d_farrow = nullptr;       // [n_det][FARROW_NC/2][N+1] float4: Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
     float4 *d_S = nullptr;   int n_sky_slots = 0;

@@ -76,10 +76,10 @@ __device__ __forceinline__ double ssb_invert_newton(const PlanGeom &g, const Sky
 //     z(j0 + d) = sum_m x[j0+m] c_m(d) = sum_p d^p Y_p[j0],   Y_p[j] = sum_m a[m][p] x[j+m]:
 // the 2D+1 taps are folded, once per plan and independent of the sky position, into FARROW_NC filtered
 // copies of the series (this kernel); per SSB grid point the resampler then reads FARROW_NC complex
-// numbers (80 contiguous bytes) and runs one Horner recurrence instead of evaluating 2D+1 weights.
+// numbers (five coalesced float4 loads) and runs one Horner recurrence instead of evaluating 2D+1 weights.
 //   series : [n_det][series_stride] float2 (data at +SERIES_PAD, zeros around it)
 //   coef   : [2D+1][FARROW_NC] float, row m+D
-//   Y      : [n_det][N+1][FARROW_NC] float2
+//   Y      : [n_det][FARROW_NC/2][N+1] float4 = (Re Y_2c, Im Y_2c, Re Y_2c+1, Im Y_2c+1)
 __global__ void __launch_bounds__(SKY_THREADS)
 farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float *__restrict__ coef, float2 *__restrict__ Y) {
     __shared__ float s_coef[(2 * FSTAT_MAX_DTERMS + 1) * FARROW_NC];
@@ -98,9 +98,11 @@ farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float 
 #pragma unroll
         for (int p = 0; p < FARROW_NC; ++p) acc[p] = __ffma2_rn(xv, make_float2(c[p], c[p]), acc[p]);
     }
-    float4 *out = reinterpret_cast<float4 *>(Y + ((int64_t)X * (g.n_samples + 1) + j) * FARROW_NC);
+    // chunk-major: chunk c = (Y_2c, Y_2c+1) of all j contiguous, so that consecutive grid points read consecutive float4
+    float4 *out = reinterpret_cast<float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * (g.n_samples + 1) + j;
 #pragma unroll
-    for (int p = 0; p < FARROW_NC / 2; ++p) out[p] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
+    for (int p = 0; p < FARROW_NC / 2; ++p)
+        out[(int64_t)p * (g.n_samples + 1)] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
 }
 
 // Trigonometric base of the timing model at every SSB grid point: (cos, sin) of the orbital phase and of the
@@ -115,7 +117,7 @@ ssb_base_kernel(PlanGeom g, double4 *__restrict__ base) {
 
 // H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
 //   base   : [n_src] double4 from ssb_base_kernel
-//   Y      : [n_det][N+1][FARROW_NC] float2, the Farrow-filtered series (above)
+//   Y      : [n_det][FARROW_NC/2][N+1] float4, the Farrow-filtered series (above)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
@@ -163,7 +165,7 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
             const double vr = floor(v + 0.5);
             d[u] = (float)(v - vr);
             const int j0 = min(max(krel + (int)vr, 0), n_rows - 1);   // in [0, N] whenever w != 0
-            y[u] = reinterpret_cast<const float4 *>(Y + ((int64_t)X * n_rows + j0) * FARROW_NC);
+            y[u] = reinterpret_cast<const float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * n_rows + j0;
             // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
             // (phase reduced mod 1 in fp64, then fp32)
             const double cyc = g.f_het * delta;
@@ -174,7 +176,7 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
 #pragma unroll
         for (int u = 0; u < 2; ++u)
 #pragma unroll
-            for (int p = 0; p < FARROW_NC / 2; ++p) c[u][p] = __ldg(y[u] + p);
+            for (int p = 0; p < FARROW_NC / 2; ++p) c[u][p] = __ldg(y[u] + (int64_t)p * n_rows);
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
