@@ -131,6 +131,14 @@ FSTAT_API int fstat_compute(fstat_plan_t *plan, const fstat_template_t *tmpl_hos
 FSTAT_API int fstat_compute_topk(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, int32_t k,
                        float *val_dev, int32_t *bin_dev);
 
+/* fstat_compute_threshold -- GPU-side candidate retention ("2F > threshold"): for every template
+ * the (at most k, 1..64) loudest bins with 2F > threshold, sorted like fstat_compute_topk (unused entries are
+ * (-inf, -1)), and the exact number of bins above the threshold (which may exceed k).
+ *  val_dev float32[n_tmpl][k], bin_dev int32[n_tmpl][k], count_dev int32[n_tmpl]: caller-owned DEVICE memory.
+ *  threshold must be finite (FSTAT_EINVAL otherwise). */
+FSTAT_API int fstat_compute_threshold(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float threshold,
+                            int32_t k, float *val_dev, int32_t *bin_dev, int32_t *count_dev);
+
 /* Host-buffer variants (the end-to-end entry points): outputs are HOST memory (pinned
  * memory makes the copies asynchronous and overlapped); they return after the data
  * has landed and report FSTAT_EDOM if a template had D <= 0. */

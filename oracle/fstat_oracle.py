@@ -282,6 +282,14 @@ def topk(twoF_row: np.ndarray, k: int):
     return twoF_row[order], order.astype(np.int32)
 
 
+def threshold_candidates(twoF_row: np.ndarray, threshold: float, k: int):
+    """Candidate retention of PAPER.md:307: the (at most k) loudest bins with 2F > threshold, ordered like topk(),
+    and the number of bins above the threshold."""
+    above = np.nonzero(twoF_row > threshold)[0]
+    order = above[np.lexsort((above, -twoF_row[above]))][:k]
+    return twoF_row[order], order.astype(np.int32), int(len(above))
+
+
 def comparison_metrics(x: np.ndarray, y: np.ndarray):
     """r_1, r_2 of eq. 9 and the angle of eq. 10."""
     r1 = 2.0 * np.sum(np.abs(x - y)) / (np.sum(np.abs(x)) + np.sum(np.abs(y)))

@@ -18,7 +18,7 @@ from . import build as _build
 FSTAT_OK, FSTAT_EINVAL, FSTAT_ESIZE, FSTAT_EDOM, FSTAT_ECUDA, FSTAT_ENOMEM = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
-    "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_host",
+    "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_threshold", "fstat_compute_host",
     "fstat_compute_topk_host", "fstat_resample_sky", "fstat_sync", "fstat_launch_count",
     "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile", "fstat_destroy", "fstat_strerror", "fstat_last_error",
 ]
@@ -69,6 +69,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_compute.argtypes = [vp, vp, i32, vp]
     lib.fstat_compute_topk.restype = C.c_int
     lib.fstat_compute_topk.argtypes = [vp, vp, i32, i32, vp, vp]
+    lib.fstat_compute_threshold.restype = C.c_int
+    lib.fstat_compute_threshold.argtypes = [vp, vp, i32, C.c_float, i32, vp, vp, vp]
     lib.fstat_compute_host.restype = C.c_int
     lib.fstat_compute_host.argtypes = [vp, vp, i32, vp]
     lib.fstat_compute_topk_host.restype = C.c_int
@@ -185,6 +187,17 @@ class FstatPlan:
         val, idx = out
         self._check(self.lib.fstat_compute_topk(self.handle, t.ctypes.data, t.shape[0], k, val.data_ptr(), idx.data_ptr()))
         return val, idx
+
+    def compute_threshold(self, templates, threshold: float, k: int):
+        """fstat_compute_threshold: (val[n,k], bin[n,k], count[n]) device tensors."""
+        t = _templates_array(templates)
+        torch = self._torch
+        val = torch.empty((t.shape[0], k), dtype=torch.float32, device="cuda")
+        idx = torch.empty((t.shape[0], k), dtype=torch.int32, device="cuda")
+        cnt = torch.empty((t.shape[0],), dtype=torch.int32, device="cuda")
+        self._check(self.lib.fstat_compute_threshold(self.handle, t.ctypes.data, t.shape[0], float(threshold), k,
+                                                     val.data_ptr(), idx.data_ptr(), cnt.data_ptr()))
+        return val, idx, cnt
 
     def compute_host(self, templates, out=None):
         """fstat_compute_host: 2F rows land in HOST memory (pinned torch tensor by default)."""

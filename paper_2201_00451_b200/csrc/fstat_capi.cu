@@ -339,6 +339,8 @@ struct OutSpec {
     int k = 0;
     float *val = nullptr;        // device [n_tmpl][k]
     int32_t *bin = nullptr;
+    float thr = 0.f;             // threshold mode (count != null): only bins with 2F > thr
+    int32_t *count = nullptr;    // device [n_tmpl]
 };
 
 // groups of 512 bins (one warp of a pass-2 tile each) per row, and how pass 2 maps them to bins
@@ -461,7 +463,8 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
                 ProfScope ps(p, 3);
                 const TopkGeom tg = topk_geom(p);
                 topk_select_kernel<<<nt, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), p->stream>>>(
-                    p->d_rows, nb, nb, out.k, p->d_gmax, tg, out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k);
+                    p->d_rows, nb, nb, out.k, p->d_gmax, tg, out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k,
+                    out.thr, out.count ? out.count + t0 : nullptr);
                 p->launches += 1;
                 CUDA_TRY(p, cudaGetLastError());
             }
@@ -704,6 +707,15 @@ int fstat_compute(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t
 
 int fstat_compute_topk(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, int32_t k, float *val_dev, int32_t *bin_dev) {
     OutSpec o; o.mode = OUT_TOPK; o.k = k; o.val = val_dev; o.bin = bin_dev;
+    return compute_impl(plan, tmpl_host, n_tmpl, o);
+}
+
+int fstat_compute_threshold(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float threshold, int32_t k,
+                            float *val_dev, int32_t *bin_dev, int32_t *count_dev) {
+    if (!plan) return FSTAT_EINVAL;
+    if (!std::isfinite(threshold)) return fail(plan, FSTAT_EINVAL, "non-finite threshold");
+    if (n_tmpl > 0 && !count_dev) return fail(plan, FSTAT_EINVAL, "null count output");
+    OutSpec o; o.mode = OUT_TOPK; o.k = k; o.val = val_dev; o.bin = bin_dev; o.thr = threshold; o.count = count_dev;
     return compute_impl(plan, tmpl_host, n_tmpl, o);
 }
 

@@ -62,7 +62,8 @@ __device__ __forceinline__ int64_t topk_group_bin(const TopkGeom &tg, int group,
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n_bins, int k,
                    const uint32_t *__restrict__ gmax, const __grid_constant__ TopkGeom tg,
-                   float *__restrict__ out_v, int *__restrict__ out_i) {
+                   float *__restrict__ out_v, int *__restrict__ out_i,
+                   float thr, int *__restrict__ out_count) {
     extern __shared__ uint32_t s_g[];                 // [n_groups] keys
     __shared__ int s_hist[256];
     __shared__ uint32_t s_prefix;
@@ -79,8 +80,29 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
     const float NEG = __int_as_float(0xff800000);
     const int G = tg.n_groups;
     for (int g = threadIdx.x; g < G; g += TOPK_THREADS) s_g[g] = gm[g];
-    if (threadIdx.x == 0) { s_prefix = 0u; s_remaining = k; s_nhot = 0; s_ncand = 0; }
+    __shared__ int s_count;
+    if (threadIdx.x == 0) { s_prefix = 0u; s_remaining = k; s_nhot = 0; s_ncand = 0; s_count = 0; }
     __syncthreads();
+    // threshold mode (out_count != null): only bins with 2F > thr are reported, and their exact number
+    // is counted by re-reading the groups whose maximum exceeds thr
+    const bool thr_mode = (out_count != nullptr);
+    if (thr_mode) {
+        const uint32_t kt = topk_key(thr);
+        const int lane = threadIdx.x & 31;
+        for (int g0 = (threadIdx.x >> 5); g0 < G; g0 += TOPK_THREADS / 32) {
+            if (s_g[g0] <= kt) continue;                      // uniform per warp
+            int c = 0;
+#pragma unroll 4
+            for (int e = 0; e < 16; ++e) {
+                const int64_t q = topk_group_bin(tg, g0, lane, e);
+                if (q < n_bins && row[q] > thr) ++c;
+            }
+            c = __reduce_add_sync(0xffffffffu, c);
+            if (lane == 0 && c) atomicAdd(&s_count, c);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) out_count[blockIdx.x] = s_count;
+    }
     bool slow = (G < k);
     uint32_t L = 0u;
     if (!slow) {
@@ -149,7 +171,7 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
             block_argbest(v, i, s_v, s_i);
             if (pos >= 0 && myi == i && myv == v) s_ci[pos] = -1;    // winner removes itself (bins are unique)
             if (threadIdx.x == 0) {
-                const bool ok = (i != 0x7fffffff);
+                const bool ok = (i != 0x7fffffff) && (!thr_mode || v > thr);
                 ov[round] = ok ? v : NEG;
                 oi[round] = ok ? i : -1;
             }
@@ -167,7 +189,7 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
             if (after_prev && x > NEG && topk_better(x, (int)q, v, i)) { v = x; i = (int)q; }
         }
         block_argbest(v, i, s_v, s_i);
-        const bool ok = (i != 0x7fffffff);
+        const bool ok = (i != 0x7fffffff) && (!thr_mode || v > thr);
         if (threadIdx.x == 0) { ov[round] = ok ? v : NEG; oi[round] = ok ? i : -1; }
         if (!ok) {
             for (int r2 = round + 1 + threadIdx.x; r2 < k; r2 += TOPK_THREADS) { ov[r2] = NEG; oi[r2] = -1; }

@@ -282,3 +282,16 @@ def test_topk_ties_and_order():
     v = np.array([1.0, 5.0, 3.0, 5.0, 2.0, 5.0])
     vals, idx = O.topk(v, 4)
     assert list(idx) == [1, 3, 5, 2] and list(vals) == [5.0, 5.0, 5.0, 3.0]
+
+
+def test_threshold_candidates_brute_force():
+    rng = np.random.default_rng(5)
+    row = rng.chisquare(4, 500).astype(np.float64)
+    row[[7, 300]] = row.max() + 1.0                      # a tie at the top: lower bin first
+    v, i, c = O.threshold_candidates(row, 9.0, 6)
+    brute = sorted([(-(row[q]), q) for q in range(len(row)) if row[q] > 9.0])
+    assert c == len(brute)
+    assert [q for _, q in brute[:6]] == list(i) and i[0] == 7 and i[1] == 300
+    assert np.all(v == row[i]) and np.all(v > 9.0)
+    v, i, c = O.threshold_candidates(row, 1e9, 6)
+    assert c == 0 and len(i) == 0

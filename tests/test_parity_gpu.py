@@ -215,3 +215,26 @@ def test_topk_degenerate_rows_take_the_exact_slow_path():
         with pytest.raises(FstatError):
             plan.sync()
         assert np.all(idx.cpu().numpy() == -1) and np.all(np.isneginf(val.cpu().numpy()))
+
+
+@pytest.mark.parametrize("thr,k", [(18.0, 16), (30.0, 4), (1e6, 3), (12.0, 64)])
+def test_threshold_retention_matches_oracle_rule(thr, k):
+    # keep 2F > threshold on the GPU.  Bit-exact against the same rule applied to the GPU's own rows;
+    # the loudest candidate and the count agree with the oracle's rows up to bins within tolerance of the threshold.
+    p = synth.small_problem(seed=50, n_samples=60000, n_fft=1 << 17, n_templates=3, gap_frac=0.3, rho=11.0)
+    cpu = O.fstat_2F_bank(p)
+    with _plan(p) as plan:
+        val, idx, cnt = plan.compute_threshold(p.templates, thr, k)
+        full = plan.compute(p.templates)
+        plan.sync()
+        val, idx, cnt, full = val.cpu().numpy(), idx.cpu().numpy(), cnt.cpu().numpy(), full.cpu().numpy()
+    for t in range(len(p.templates)):
+        ev, ei, ec = O.threshold_candidates(full[t], np.float32(thr), k)
+        assert cnt[t] == ec
+        n = len(ei)
+        np.testing.assert_array_equal(idx[t, :n], ei)
+        np.testing.assert_array_equal(val[t, :n], ev)
+        assert np.all(idx[t, n:] == -1) and np.all(np.isneginf(val[t, n:]))
+        # against the oracle: bins clearly above / below the threshold are counted alike
+        lo = int(np.sum(cpu[t] > thr * (1 + 2 * TOL) + 8 * TOL)); hi = int(np.sum(cpu[t] > thr * (1 - 2 * TOL) - 8 * TOL))
+        assert lo <= cnt[t] <= hi
