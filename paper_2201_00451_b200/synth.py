@@ -41,6 +41,8 @@ EPHEM_DEFAULT = dict(
 H1 = dict(lat_rad=46.455 * DEG, lon_east_rad=-119.408 * DEG, xarm_azimuth_rad=36.0 * DEG)
 L1 = dict(lat_rad=30.563 * DEG, lon_east_rad=-90.774 * DEG, xarm_azimuth_rad=108.0 * DEG)
 
+V1 = dict(lat_rad=43.631 * DEG, lon_east_rad=10.504 * DEG, xarm_azimuth_rad=341.0 * DEG)   # a third, Virgo-like site (tests)
+
 T_SFT = 1800.0
 T_START = 1.0e9  # arbitrary epoch; every formula uses t' = t - t_start
 
@@ -351,7 +353,7 @@ def small_problem(seed: int = 7, n_det: int = 2, n_samples: int = 20000, dt: flo
         inj = Injection(rho=rho, cosi=-0.4, psi=1.1, phi0=2.0, f=f_min + 0.31 * band, fdot=float(fdots[it]),
                         fddot=fddot, alpha=SKY0[0], delta=SKY0[1])
     tm = _fdot_bank(SKY0[0], SKY0[1], f_min, fdots, (fddot,))
-    dets = [H1, L1][:n_det]
+    dets = [H1, L1, V1][:n_det]
     return make_problem(f"small_s{seed}", dets, n_samples, dt, f_min, band, f_min + band / 2, n_fft, dterms, tm,
                         seed=seed, gap_frac=gap_frac, weight_range=(0.5, 2.0) if weights else None,
                         injection=inj, injection_template=it if inj else None, noise=noise, ephem=ephem,

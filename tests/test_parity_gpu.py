@@ -79,6 +79,13 @@ def test_parity_dterms16_single_detector_no_gaps():
     _check_bank(p)
 
 
+def test_parity_three_detectors():
+    # odd detector count: the sky kernel takes detectors two at a time, the last one alone
+    p = synth.small_problem(seed=5, n_det=3, n_samples=30000, n_fft=1 << 16, n_templates=2, gap_frac=0.35, rho=14.0)
+    gpu, cpu = _check_bank(p)
+    assert int(np.argmax(gpu.max(axis=1))) == int(np.argmax(cpu.max(axis=1))) == p.injection_template
+
+
 def test_resampled_series_and_antenna_sums_match_oracle():
     p = synth.small_problem(seed=9, n_samples=30000, n_fft=1 << 15, n_templates=1)
     al, de = synth.SKY0
