@@ -43,7 +43,7 @@ struct fstat_plan {
     float2 *d_farrow = nullptr;       // [n_det][FARROW_NC/2][N+1] float4: Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
-    float4 *d_S = nullptr;   int n_sky_slots = 0;
+    float4 *d_S = nullptr;   int n_sky_slots = 0, max_sky_slots = 1;   // S buffers: allocated / allowed (grown on demand)
     float4 *d_T = nullptr;   int n_inflight = 0;
     SkyConst *d_sky = nullptr; size_t sky_cap = 0;
     SkyABCD *d_abcd = nullptr; SkyABCD *h_abcd = nullptr;   // per sky group of the current call (capacity sky_cap)
@@ -383,6 +383,8 @@ int ensure_host_ring(fstat_plan *p) {
     return FSTAT_OK;
 }
 
+int ensure_sky_slots(fstat_plan *p, size_t want);
+
 int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, const OutSpec &out) {
     if (!p) return FSTAT_EINVAL;
     if (n_tmpl < 0 || (n_tmpl > 0 && !tm)) return fail(p, FSTAT_EINVAL, "null template array");
@@ -403,6 +405,8 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         ++groups.back().count;
     }
     int rc = ensure_tmpl_capacity(p, n_tmpl, groups.size());
+    if (rc) return rc;
+    rc = ensure_sky_slots(p, groups.size());
     if (rc) return rc;
     // staging buffers are reused between calls: wait until the previous upload has been consumed
     CUDA_TRY(p, cudaEventSynchronize(p->staging_ev));
@@ -511,11 +515,27 @@ int default_inflight(int64_t n_fft, int log_tile) {
     return (int)tb;
 }
 
-int default_sky_slots(int64_t n_fft) {
-    int64_t s = (64ll << 20) / (n_fft * 16);
+int max_sky_slots_for(int64_t n_fft) {
+    // sky positions resampled per batch: a search over the sky wants large batches (every FFT launch pair costs
+    // ~35 us whatever its size, profiles/r01_v3_experiments.md), bounded by 1 GB of resampled series
+    int64_t s = (1024ll << 20) / (n_fft * 16);
     if (s < 1) s = 1;
-    if (s > 32) s = 32;
+    if (s > 1024) s = 1024;
     return (int)s;
+}
+
+// make room for `want` sky positions per batch (up to the plan's maximum)
+int ensure_sky_slots(fstat_plan *p, size_t want) {
+    int need = (int)std::min<size_t>(want, (size_t)p->max_sky_slots);
+    if (need <= p->n_sky_slots) return FSTAT_OK;
+    if (need < 2 * p->n_sky_slots) need = std::min(2 * p->n_sky_slots, p->max_sky_slots);
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    cudaFree(p->d_S); p->d_S = nullptr; p->n_sky_slots = 0;
+    const size_t bytes = (size_t)need * p->g.n_fft * sizeof(float4);
+    if (cudaMalloc(&p->d_S, bytes) != cudaSuccess) { cudaGetLastError(); return fail(p, FSTAT_ENOMEM, "device allocation of the resampled-series buffers failed"); }
+    CUDA_TRY(p, cudaMemsetAsync(p->d_S, 0, bytes, p->stream));     // the kernels only ever write k < n_src: the zero padding stays
+    p->n_sky_slots = need;
+    return FSTAT_OK;
 }
 
 }  // namespace
@@ -643,9 +663,8 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     SETUP_TRY(cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
     p->n_inflight = default_inflight(n_fft, g.log_tile2);
-    p->n_sky_slots = default_sky_slots(n_fft);
-    SETUP_TRY(cudaMalloc(&p->d_S, (size_t)p->n_sky_slots * n_fft * sizeof(float4)));
-    SETUP_TRY(cudaMemsetAsync(p->d_S, 0, (size_t)p->n_sky_slots * n_fft * sizeof(float4), p->stream));
+    p->max_sky_slots = max_sky_slots_for(n_fft);
+    if (ensure_sky_slots(p, 1) != FSTAT_OK) return bail(FSTAT_ENOMEM);
     SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
     {   // Farrow-filtered copies of the series (sky_kernels.cuh), once per plan
         const std::vector<float> fc = farrow_coefficients(dterms);
