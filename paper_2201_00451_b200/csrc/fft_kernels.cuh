@@ -51,6 +51,20 @@ __device__ __forceinline__ void mul_w16(float2 &ox, float2 &oy, int j) {
     ox = tx; oy = ty;
 }
 
+// (ox + i oy) * exp(-2 pi i j/32), j = 0..15 (compile-time constant after unrolling).
+__device__ __forceinline__ void mul_w32(float2 &ox, float2 &oy, int j) {
+    if ((j & 1) == 0) { mul_w16(ox, oy, j >> 1); return; }
+    // cos, sin of 2 pi j / 32 for odd j
+    const float c = (j == 1 || j == 15) ? 0.98078528040323043f : (j == 3 || j == 13) ? 0.83146961230254524f
+                  : (j == 5 || j == 11) ? 0.55557023301960218f : 0.19509032201612825f;
+    const float sn = (j == 1 || j == 15) ? 0.19509032201612825f : (j == 3 || j == 13) ? 0.55557023301960218f
+                   : (j == 5 || j == 11) ? 0.83146961230254524f : 0.98078528040323043f;
+    const float cc = (j > 8) ? -c : c;                      // cos(2 pi j/32) is negative for j in (8, 16)
+    // (x + i y)(cc - i sn) = (x cc + y sn) + i (y cc - x sn)
+    const float2 tx = fma2s(ox, cc, mul2s(oy, sn)), ty = fma2s(oy, cc, mul2s(ox, -sn));
+    ox = tx; oy = ty;
+}
+
 // In-place forward DFT of length R (kernel exp(-2 pi i rq/R)) on packed pairs, natural order.
 template <int R> __device__ __forceinline__ void dft(float2 *x, float2 *y) {
     float2 ex[R / 2], ey[R / 2], ox[R / 2], oy[R / 2];
@@ -60,15 +74,15 @@ template <int R> __device__ __forceinline__ void dft(float2 *x, float2 *y) {
     dft<R / 2>(ox, oy);
 #pragma unroll
     for (int k = 0; k < R / 2; ++k) {
-        mul_w16(ox[k], oy[k], k * (16 / R));
+        mul_w32(ox[k], oy[k], k * (32 / R));
         x[k] = add2(ex[k], ox[k]); y[k] = add2(ey[k], oy[k]);
         x[k + R / 2] = sub2(ex[k], ox[k]); y[k + R / 2] = sub2(ey[k], oy[k]);
     }
 }
 template <> __device__ __forceinline__ void dft<1>(float2 *, float2 *) {}
 
-// Radix plan per sub-FFT length 2^LOGN (16 register elements per thread).
-template <int LOGN> struct RadixPlan;
+// Radix plan per sub-FFT length 2^LOGN and register elements per thread E (16, or 32 for the two-pass plans of pass 2).
+template <int LOGN, int E = 16> struct RadixPlan;
 template <> struct RadixPlan<6>  { static constexpr int np = 2, r0 = 8,  r1 = 8,  r2 = 1; };
 template <> struct RadixPlan<7>  { static constexpr int np = 2, r0 = 16, r1 = 8,  r2 = 1; };
 template <> struct RadixPlan<8>  { static constexpr int np = 2, r0 = 16, r1 = 16, r2 = 1; };
@@ -76,25 +90,27 @@ template <> struct RadixPlan<9>  { static constexpr int np = 3, r0 = 8,  r1 = 8,
 template <> struct RadixPlan<10> { static constexpr int np = 3, r0 = 16, r1 = 16, r2 = 4; };
 template <> struct RadixPlan<11> { static constexpr int np = 3, r0 = 16, r1 = 16, r2 = 8; };
 template <> struct RadixPlan<12> { static constexpr int np = 3, r0 = 16, r1 = 16, r2 = 16; };
+template <> struct RadixPlan<9, 32>  { static constexpr int np = 2, r0 = 32, r1 = 16, r2 = 1; };
+template <> struct RadixPlan<10, 32> { static constexpr int np = 2, r0 = 32, r1 = 32, r2 = 1; };
 
 __host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
 // A tile is 2^LOGT elements = W = 2^(LOGT - LOGN) adjacent sub-FFTs, worked on by 2^LOGT / 16 threads:
 // LOGT = 11 (128 threads, 32 KB, 4 CTAs per SM) or 12 (256 threads, 64 KB, 2 CTAs per SM); sub-FFTs of
 // length 2^12 use LOGT = 13 (two per tile, so that the other pass still gets 32-byte store runs).
-template <int LOGN, int LOGT> struct FftCfg {
+template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     static_assert(LOGT >= LOGN && LOGT >= 11 && LOGT <= 13, "tile must hold at least one sub-FFT");
     static constexpr int LOGW = LOGT - LOGN;
     static constexpr int W = 1 << LOGW;
-    static constexpr int MIN_CTAS = (LOGT == 11) ? 5 : (LOGT == 12) ? 2 : 1;
+    static constexpr int MIN_CTAS = (E == 32) ? 2 : (LOGT == 11) ? 5 : (LOGT == 12) ? 2 : 1;
     static constexpr int N = 1 << LOGN;
-    static constexpr int NT = (N * W) / 16;
+    static constexpr int NT = (N * W) / E;
     // twiddle table offsets (float2 entries): pass s >= 1 holds (R_s - 1) * P_s entries, [r-1][k]
-    static constexpr int P1 = RadixPlan<LOGN>::r0;
-    static constexpr int P2 = P1 * RadixPlan<LOGN>::r1;
+    static constexpr int P1 = RadixPlan<LOGN, E>::r0;
+    static constexpr int P2 = P1 * RadixPlan<LOGN, E>::r1;
     static constexpr int OFF1 = 0;
-    static constexpr int OFF2 = (RadixPlan<LOGN>::r1 - 1) * P1;
-    static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN>::np > 2 ? (RadixPlan<LOGN>::r2 - 1) * P2 : 0);
+    static constexpr int OFF2 = (RadixPlan<LOGN, E>::r1 - 1) * P1;
+    static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN, E>::np > 2 ? (RadixPlan<LOGN, E>::r2 - 1) * P2 : 0);
     static constexpr int SMEM_BYTES = N * W * 16 + TW_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
 };
 
@@ -117,7 +133,7 @@ template <int LOGW, int LOGR0> __device__ __forceinline__ int sm_phys(int idx, i
 template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST>
 struct PassIdx {
     static constexpr int LOGR = ilog2c(R);
-    static constexpr int NB = 16 / R;                 // butterflies per thread
+    static constexpr int NB = ((1 << (LOGN + LOGW)) / NT) / R;   // butterflies per thread = register elements / R
     static constexpr int NI = (1 << LOGN) / R;        // butterflies per FFT
     __device__ __forceinline__ static void item(int bb, int &i, int &w) {
         const int g = threadIdx.x + bb * NT;
@@ -131,8 +147,8 @@ struct PassIdx {
     }
 };
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST>
-__device__ __forceinline__ void pass_compute(float2 (&a)[16], float2 (&b)[16], const float2 *__restrict__ tw) {
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int E>
+__device__ __forceinline__ void pass_compute(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
     for (int bb = 0; bb < PI::NB; ++bb) {
@@ -149,8 +165,8 @@ __device__ __forceinline__ void pass_compute(float2 (&a)[16], float2 (&b)[16], c
     }
 }
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0>
-__device__ __forceinline__ void pass_store_smem(const float2 (&a)[16], const float2 (&b)[16], float4 *sm) {
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0, int E>
+__device__ __forceinline__ void pass_store_smem(const float2 (&a)[E], const float2 (&b)[E], float4 *sm) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
     for (int bb = 0; bb < PI::NB; ++bb) {
@@ -162,8 +178,8 @@ __device__ __forceinline__ void pass_store_smem(const float2 (&a)[16], const flo
     }
 }
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0>
-__device__ __forceinline__ void pass_load_smem(float2 (&a)[16], float2 (&b)[16], const float4 *sm) {
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int LOGR0, int E>
+__device__ __forceinline__ void pass_load_smem(float2 (&a)[E], float2 (&b)[E], const float4 *sm) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
     for (int bb = 0; bb < PI::NB; ++bb) {
@@ -262,10 +278,10 @@ __device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restri
 }
 
 // Pass-0 inputs out of the staging layout (linear: element idx of lane w at idx*W + w).
-template <int LOGN, int LOGT>
-__device__ __forceinline__ void tile_take_inputs(float2 (&a)[16], float2 (&b)[16], const float4 *sm) {
-    using C = FftCfg<LOGN, LOGT>;
-    using RP = RadixPlan<LOGN>;
+template <int LOGN, int LOGT, int E>
+__device__ __forceinline__ void tile_take_inputs(float2 (&a)[E], float2 (&b)[E], const float4 *sm) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
     using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
 #pragma unroll
     for (int bb = 0; bb < PI::NB; ++bb) {
@@ -281,10 +297,10 @@ __device__ __forceinline__ void tile_take_inputs(float2 (&a)[16], float2 (&b)[16
 
 // Radix passes of one tile between "inputs of pass 0 are in registers" and "inputs of the last
 // pass are in registers and the exchange buffer is free again" (barrier included).
-template <int LOGN, int LOGT>
-__device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], float4 *sm, const float2 *__restrict__ tw) {
-    using C = FftCfg<LOGN, LOGT>;
-    using RP = RadixPlan<LOGN>;
+template <int LOGN, int LOGT, int E>
+__device__ __forceinline__ void tile_passes(float2 (&a)[E], float2 (&b)[E], float4 *sm, const float2 *__restrict__ tw) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
     constexpr int LOGW = C::LOGW, NT = C::NT, LOGR0 = ilog2c(RP::r0);
     constexpr bool LAST1 = (RP::np == 2);
     __syncthreads();                                   // every thread has taken its pass-0 inputs
@@ -302,18 +318,18 @@ __device__ __forceinline__ void tile_passes(float2 (&a)[16], float2 (&b)[16], fl
     __syncthreads();                                   // buffer free: the next tile may be prefetched
 }
 
-template <int LOGN, int LOGT>
-__device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16], const float2 *__restrict__ tw) {
-    using C = FftCfg<LOGN, LOGT>;
-    using RP = RadixPlan<LOGN>;
+template <int LOGN, int LOGT, int E>
+__device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
     if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
     else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
 }
 
 // Common kernel preamble: shared-memory carve-up, twiddles to shared memory, mbarrier init.
-#define FFT_KERNEL_PREAMBLE()                                                                     \
-    using C = FftCfg<LOGN, LOGT>;                                                                       \
-    using RP = RadixPlan<LOGN>;                                                                   \
+#define FFT_KERNEL_PREAMBLE(E)                                                                   \
+    using C = FftCfg<LOGN, LOGT, E>;                                                                       \
+    using RP = RadixPlan<LOGN, E>;                                                                   \
     constexpr int LOGW = C::LOGW, NT = C::NT;                                                     \
     extern __shared__ float4 sm[];                                                                \
     float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);                                 \
@@ -321,7 +337,7 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16],
     for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];                     \
     if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }                             \
     __syncthreads();                                                                              \
-    float2 a[16], b[16];                                                                          \
+    float2 a[E], b[E];                                                                              \
     unsigned parity = 0;                                                                          \
     int tile = blockIdx.x;                                                                        \
     if (tile >= p.n_tiles) return;                                                                \
@@ -332,10 +348,10 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[16], float2 (&b)[16],
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
 // Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
 // ---------------------------------------------------------------------------------------
-template <int LOGN, int LOGT>
-__global__ void __launch_bounds__(FftCfg<LOGN, LOGT>::NT, FftCfg<LOGN, LOGT>::MIN_CTAS)
+template <int LOGN, int LOGT, int E>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
-    FFT_KERNEL_PREAMBLE();
+    FFT_KERNEL_PREAMBLE(E);
     const uint64_t pol_S = l2_policy_evict_last(), pol_T = l2_policy_evict_first();
     TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
     tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S);
@@ -429,10 +445,12 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
 // Pass 2: row FFTs of length N2 = 2^LOGN + the 2F combination of eq. 8 (Fig. 1).
 // Persistent; tile = (template, W adjacent rows m1) = one contiguous block of T.
 // ---------------------------------------------------------------------------------------
-template <int LOGN, int LOGT>
-__global__ void __launch_bounds__(FftCfg<LOGN, LOGT>::NT, FftCfg<LOGN, LOGT>::MIN_CTAS)
+// E = register elements per thread: 16, or 32 for the two-pass radix-32 plans (sub-FFT 2^9, 2^10: one trip through
+// shared memory instead of two).
+template <int LOGN, int LOGT, int E>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
 fft_pass2_kernel(const __grid_constant__ FftArgs p) {
-    FFT_KERNEL_PREAMBLE();
+    FFT_KERNEL_PREAMBLE(E);
     const uint64_t pol_T = l2_policy_evict_first();
     int sky_next = p.tmpl[tile >> p.log_tiles].sky_slot;
     tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_T);

@@ -99,7 +99,8 @@ struct ProfScope {
 int ilog2(int64_t v) { int l = 0; while ((int64_t(1) << l) < v) ++l; return l; }
 
 // radix list of fft_kernels.cuh RadixPlan<LOGN>
-std::vector<int> radix_list(int logn) {
+std::vector<int> radix_list(int logn, int elems = 16) {
+    if (elems == 32) return logn == 9 ? std::vector<int>{32, 16} : std::vector<int>{32, 32};     // RadixPlan<9|10, 32>
     switch (logn) {
         case 6: return {8, 8};
         case 7: return {16, 8};
@@ -112,9 +113,9 @@ std::vector<int> radix_list(int logn) {
 }
 
 // Twiddles of passes s >= 1: entry [(r-1)*P + k] = exp(-2 pi i r k / (P R)).
-std::vector<float2> make_twiddles(int logn) {
+std::vector<float2> make_twiddles(int logn, int elems = 16) {
     std::vector<float2> tw;
-    const std::vector<int> rl = radix_list(logn);
+    const std::vector<int> rl = radix_list(logn, elems);
     int P = rl[0];
     for (size_t s = 1; s < rl.size(); ++s) {
         const int R = rl[s];
@@ -229,12 +230,12 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
 }
 
 // Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
-template <int LOGN, int LOGT, bool P2> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
-    using C = FftCfg<LOGN, LOGT>;
+template <int LOGN, int LOGT, bool P2, int E = 16> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
+    using C = FftCfg<LOGN, LOGT, E>;
     constexpr int SMEM = C::SMEM_BYTES;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
-    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT> : fft_pass1_kernel<LOGN, LOGT>;
+    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT, E> : fft_pass1_kernel<LOGN, LOGT, E>;
     if (configured_dev != p->device) {
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
@@ -288,7 +289,13 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     { ProfScope ps(p, 1); DISPATCH_TILE(l1, tile_log1(p), false, p, a, 1 << (l2 - p->g.log_w1), nt); }
     if (rc) return rc;
     a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
-    { ProfScope ps(p, 2); DISPATCH_TILE(l2, tile_log2(p), true, p, a, 1 << (l1 - p->g.log_w2), nt); }
+    {
+        ProfScope ps(p, 2);
+        const int tiles2 = 1 << (l1 - p->g.log_w2);
+        if (p->g.p2_elems == 32 && l2 == 10) rc = launch_pass<10, 12, true, 32>(p, a, tiles2, nt);
+        else if (p->g.p2_elems == 32 && l2 == 9) rc = launch_pass<9, 12, true, 32>(p, a, tiles2, nt);
+        else DISPATCH_TILE(l2, tile_log2(p), true, p, a, tiles2, nt);
+    }
     if (rc) return rc;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -346,9 +353,10 @@ struct OutSpec {
 // groups of 512 bins (one warp of a pass-2 tile each) per row, and how pass 2 maps them to bins
 TopkGeom topk_geom(const fstat_plan *p) {
     const int l2 = p->g.log_n2, lt = tile_log2(p);
-    const std::vector<int> rl = radix_list(l2);
+    const std::vector<int> rl = radix_list(l2, p->g.p2_elems);
     TopkGeom tg{};
-    tg.nt = (1 << lt) / 16;
+    tg.elems = p->g.p2_elems;
+    tg.nt = (1 << lt) / tg.elems;
     tg.log_w = lt - l2;
     tg.log_rl = ilog2(rl.back());
     tg.pl = 1;
@@ -619,15 +627,15 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     // n_fft = 2^log_n1 x 2^log_n2.  Pass 2 gets the shorter transform: its tile then spans more rows, which is what
     // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
     // 2^11-element tiles.  Split per size as measured on B200 (profiles/r01_v3_experiments.md, section 4).
-    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 20 ? 8 : L == 21 ? 10
-             : L - 11 <= 12 ? 11 : 12;
+    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10
+             : L == 22 ? 10 : L - 12;
     { const char *e = getenv("FSTAT_LOGN2"); if (e && atoi(e) >= 6 && atoi(e) <= 12 && L - atoi(e) >= 6 && L - atoi(e) <= 12) g.log_n2 = atoi(e); }
     g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
     {   // tile sizes of the two FFT passes (profiles/r01_v3_experiments.md): 2^11-element tiles (128 threads, 4 CTAs per
         // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
-        g.log_tile2 = (g.log_n2 == 12 || (L == 22 && 2 * n_bins > n_fft)) ? 13 : 12;   // full-band 2^22 (config 4): 4 rows per tile, 16-byte 2F runs
+        g.log_tile2 = (g.log_n2 == 12 || (L == 22 && 2 * n_bins > n_fft)) ? 13 : 12;   // full-band 2^22 (config 4): 8 rows per tile, 32-byte 2F runs
         // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
         // of a single column needs >= 4 rows per pass-2 tile
         const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
@@ -635,6 +643,12 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
         if (e1 && (atoi(e1) >= 11 && atoi(e1) <= 13) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
         if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
+    }
+    {   // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
+        // sub-FFTs of 2^9 and 2^10 points on 2^12-element tiles; FSTAT_P2_ELEMS=16 switches it off (experiments)
+        g.p2_elems = ((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) ? 32 : 16;
+        const char *e = getenv("FSTAT_P2_ELEMS");
+        if (e && atoi(e) == 16) g.p2_elems = 16;
     }
     g.log_w1 = tile_log1(p) - g.log_n1; g.log_w2 = tile_log2(p) - g.log_n2;
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
@@ -657,7 +671,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
                                   cudaMemcpyDefault, p->stream));
     SETUP_TRY(cudaMalloc(&p->d_wslot, wslot.size() * sizeof(float)));
     SETUP_TRY(cudaMemcpyAsync(p->d_wslot, wslot.data(), wslot.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-    const std::vector<float2> tw1 = make_twiddles(g.log_n1), tw2 = make_twiddles(g.log_n2);
+    const std::vector<float2> tw1 = make_twiddles(g.log_n1), tw2 = make_twiddles(g.log_n2, g.p2_elems);
     SETUP_TRY(cudaMalloc(&p->d_tw1, tw1.size() * sizeof(float2)));
     SETUP_TRY(cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
     SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));

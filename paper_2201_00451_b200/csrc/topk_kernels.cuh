@@ -28,9 +28,10 @@ __device__ __forceinline__ void block_argbest(float &v, int &i, float *s_v, int 
     __syncthreads();
 }
 
-// How FFT pass 2 lays one warp's 512 outputs ("group") over the bins of a row: element e (0..15) of
+// How FFT pass 2 lays one warp's 32 x elems outputs ("group") over the bins of a row: element e (0..15) of
 // lane l of warp wp of tile x is bin q (fft_kernels.cuh, pass-2 epilogue).
 struct TopkGeom {
+    int elems;       // register elements per thread of pass 2 (16 or 32): a group is 32 * elems bins
     int nt;          // threads per pass-2 CTA
     int log_w;       // log2(rows per tile)
     int log_rl;      // log2(last radix)
@@ -93,7 +94,7 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
             if (s_g[g0] <= kt) continue;                      // uniform per warp
             int c = 0;
 #pragma unroll 4
-            for (int e = 0; e < 16; ++e) {
+            for (int e = 0; e < tg.elems; ++e) {
                 const int64_t q = topk_group_bin(tg, g0, lane, e);
                 if (q < n_bins && row[q] > thr) ++c;
             }
@@ -145,7 +146,7 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
         for (int h = threadIdx.x >> 5; h < nhot; h += TOPK_THREADS / 32) {
             const int g = s_hot[h];
 #pragma unroll 4
-            for (int e = 0; e < 16; ++e) {
+            for (int e = 0; e < tg.elems; ++e) {
                 const int64_t q = topk_group_bin(tg, g, lane, e);
                 if (q < n_bins) {
                     const float v = row[q];
