@@ -245,3 +245,24 @@ def test_threshold_retention_matches_oracle_rule(thr, k):
         # against the oracle: bins clearly above / below the threshold are counted alike
         lo = int(np.sum(cpu[t] > thr * (1 + 2 * TOL) + 8 * TOL)); hi = int(np.sum(cpu[t] > thr * (1 - 2 * TOL) - 8 * TOL))
         assert lo <= cnt[t] <= hi
+
+
+def test_results_do_not_depend_on_templates_per_launch():
+    # chunked launches (fstat_set_inflight) and a sky-major bank larger than one launch give the same bits
+    p = synth.small_problem(seed=21, n_samples=9000, n_fft=1 << 14, n_templates=3, rho=None)
+    sky = synth.disc_sky_points(7, seed=2)
+    p.templates = np.array([(a, d, p.f_min, fd, 0.0) for (a, d) in sky for fd in (-2e-9, -1e-9, 0.0)])
+    with _plan(p) as plan:
+        full = plan.compute(p.templates)
+        val, idx = plan.compute_topk(p.templates, 6)
+        plan.sync()
+        full, val, idx = full.cpu().numpy(), val.cpu().numpy(), idx.cpu().numpy()
+        plan.set_inflight(4)
+        full2 = plan.compute(p.templates)
+        val2, idx2 = plan.compute_topk(p.templates, 6)
+        tv, ti, tc = plan.compute_threshold(p.templates, 14.0, 6)
+        plan.sync()
+        np.testing.assert_array_equal(full2.cpu().numpy(), full)
+        np.testing.assert_array_equal(val2.cpu().numpy(), val)
+        np.testing.assert_array_equal(idx2.cpu().numpy(), idx)
+        assert np.array_equal(tc.cpu().numpy(), (full > 14.0).sum(axis=1))
