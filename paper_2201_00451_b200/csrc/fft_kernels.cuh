@@ -265,21 +265,22 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // One thread starts the copy of a whole tile (contiguous in global memory thanks to the
 // tile-blocked layouts) into the exchange buffer; completion is signalled on the mbarrier.
 template <int LOGN, int LOGT>
-__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, uint64_t *bar, uint64_t policy) {
-    using C = FftCfg<LOGN, LOGT>;
-    constexpr unsigned BYTES = C::N * C::W * 16, CHUNK = 16384;
+__device__ __forceinline__ void tile_prefetch(float4 *sm, const float4 *__restrict__ src, uint64_t *bar, uint64_t policy,
+                                              unsigned n_bytes = FftCfg<LOGN, LOGT>::N * FftCfg<LOGN, LOGT>::W * 16) {
+    // n_bytes: the leading part of the tile that is copied (pass 1 skips the rows that are zero padding)
+    constexpr unsigned CHUNK = 16384;
     if (threadIdx.x == 0) {
         fence_proxy_async();                      // earlier generic-proxy reads of the buffer are ordered before the async writes
-        mbar_expect_tx(bar, BYTES);
-#pragma unroll
-        for (unsigned o = 0; o < BYTES; o += CHUNK)
-            bulk_g2s(reinterpret_cast<char *>(sm) + o, reinterpret_cast<const char *>(src) + o, CHUNK, bar, policy);
+        mbar_expect_tx(bar, n_bytes);
+        for (unsigned o = 0; o < n_bytes; o += CHUNK)
+            bulk_g2s(reinterpret_cast<char *>(sm) + o, reinterpret_cast<const char *>(src) + o, min(CHUNK, n_bytes - o), bar, policy);
     }
 }
 
 // Pass-0 inputs out of the staging layout (linear: element idx of lane w at idx*W + w).
 template <int LOGN, int LOGT, int E>
-__device__ __forceinline__ void tile_take_inputs(float2 (&a)[E], float2 (&b)[E], const float4 *sm) {
+__device__ __forceinline__ void tile_take_inputs(float2 (&a)[E], float2 (&b)[E], const float4 *sm, int r_nz = 32) {
+    // r_nz: inputs r >= r_nz of every butterfly are zero padding (not staged, not read)
     using C = FftCfg<LOGN, LOGT, E>;
     using RP = RadixPlan<LOGN, E>;
     using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
@@ -288,7 +289,7 @@ __device__ __forceinline__ void tile_take_inputs(float2 (&a)[E], float2 (&b)[E],
         const int g = threadIdx.x + bb * C::NT;   // = i*W + w
 #pragma unroll
         for (int r = 0; r < RP::r0; ++r) {
-            const float4 v = sm[g + ((r * PI::NI) << C::LOGW)];
+            const float4 v = (r < r_nz) ? sm[g + ((r * PI::NI) << C::LOGW)] : make_float4(0.f, 0.f, 0.f, 0.f);
             a[bb * RP::r0 + r] = make_float2(v.x, v.y);
             b[bb * RP::r0 + r] = make_float2(v.z, v.w);
         }
@@ -348,13 +349,19 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], c
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
 // Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
 // ---------------------------------------------------------------------------------------
-template <int LOGN, int LOGT, int E>
+// SKIPZ: do not stage or touch the zero padding (pays when at least half of every column is padding, as in config 4).
+template <int LOGN, int LOGT, int E, bool SKIPZ>
 __global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
     FFT_KERNEL_PREAMBLE(E);
     const uint64_t pol_S = l2_policy_evict_last(), pol_T = l2_policy_evict_first();
     TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
-    tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S);
+    // zero padding: rows k1 >= ceil(n_src / N2) of every column are zero, i.e. the inputs r >= r_nz of every first-pass
+    // butterfly (k1 = i + r*NI): they are neither staged nor multiplied by the spin-down factor
+    const int r_nz = !SKIPZ ? (int)RP::r0
+        : min((int)RP::r0, (int)((((p.n_src + ((int64_t)1 << p.log_other) - 1) >> p.log_other) + (C::N / RP::r0) - 1) / (C::N / RP::r0)));
+    const unsigned stage_bytes = (unsigned)min(r_nz * (C::N / RP::r0), (int)C::N) * C::W * 16u;
+    tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
     for (; tile < p.n_tiles; tile += gridDim.x) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const TmplDesc td = td_next;
@@ -363,7 +370,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
         if (nxt < p.n_tiles) td_next = p.tmpl[nxt >> p.log_tiles];
         mbar_wait(bar, parity);
         parity ^= 1;
-        tile_take_inputs<LOGN, LOGT>(a, b, sm);
+        tile_take_inputs<LOGN, LOGT>(a, b, sm, SKIPZ ? r_nz : 32);
         {   // times exp(-i Phi_s) (S9).  The r0 inputs of one butterfly sit on an
             // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic
             // phi(tau) = tau^2 (c1 + c2 tau): its forward differences D1, D2 and the constant D3 are
@@ -387,6 +394,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
                 float2 q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
 #pragma unroll
                 for (int r = 0; r < RP::r0; ++r) {
+                    if (SKIPZ && r >= r_nz) break;
                     pcmul(a[bb * RP::r0 + r], b[bb * RP::r0 + r], e);
                     if (r + 1 < RP::r0) {
                         e = cmul(e, d);
@@ -398,7 +406,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
         }
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < p.n_tiles)
-            tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S);
+            tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
         tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
         {   // outputs m1 = i + r*NI of column k2 = k2_0 + w, times the four-step twiddle
             // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r (two exact sincospif per butterfly, powers by

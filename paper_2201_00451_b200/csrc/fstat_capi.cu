@@ -230,12 +230,12 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
 }
 
 // Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
-template <int LOGN, int LOGT, bool P2, int E = 16> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
+template <int LOGN, int LOGT, bool P2, int E = 16, bool SKIPZ = false> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN, LOGT, E>;
     constexpr int SMEM = C::SMEM_BYTES;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
-    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT, E> : fft_pass1_kernel<LOGN, LOGT, E>;
+    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT, E> : fft_pass1_kernel<LOGN, LOGT, E, SKIPZ>;
     if (configured_dev != p->device) {
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
         CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
@@ -286,7 +286,18 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     int rc = FSTAT_OK;
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
     a.tw = p->d_tw1; a.log_other = l2; a.log_w_other = p->g.log_w2;
-    { ProfScope ps(p, 1); DISPATCH_TILE(l1, tile_log1(p), false, p, a, 1 << (l2 - p->g.log_w1), nt); }
+    {
+        ProfScope ps(p, 1);
+        const int tiles1 = 1 << (l2 - p->g.log_w1), lt1 = tile_log1(p);
+        // columns that are at least half zero padding: the variant that neither stages nor touches the padding
+        const bool skipz = 2 * p->g.n_src <= p->g.n_fft;
+        if (skipz && l1 == 12 && lt1 == 12) rc = launch_pass<12, 12, false, 16, true>(p, a, tiles1, nt);
+        else if (skipz && l1 == 12 && lt1 == 13) rc = launch_pass<12, 13, false, 16, true>(p, a, tiles1, nt);
+        else if (skipz && l1 == 11 && lt1 == 11) rc = launch_pass<11, 11, false, 16, true>(p, a, tiles1, nt);
+        else if (skipz && l1 == 11 && lt1 == 12) rc = launch_pass<11, 12, false, 16, true>(p, a, tiles1, nt);
+        else if (skipz && l1 == 10 && lt1 == 11) rc = launch_pass<10, 11, false, 16, true>(p, a, tiles1, nt);
+        else DISPATCH_TILE(l1, lt1, false, p, a, tiles1, nt);
+    }
     if (rc) return rc;
     a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
     {
