@@ -266,3 +266,30 @@ def test_results_do_not_depend_on_templates_per_launch():
         np.testing.assert_array_equal(val2.cpu().numpy(), val)
         np.testing.assert_array_equal(idx2.cpu().numpy(), idx)
         assert np.array_equal(tc.cpu().numpy(), (full > 14.0).sum(axis=1))
+
+
+@pytest.mark.parametrize("case", range(10))
+def test_parity_random_geometries(case):
+    # unusual plans: Dterms 1..32, sample intervals that are not powers of two, narrow bands off the heterodyne
+    # frequency, 1-3 detectors, heavy gaps, second spin-down
+    rng = np.random.default_rng(1000 + case)
+    dt = float(rng.choice([0.25, 0.5, 0.7, 1.0, 3.0]))
+    log_nfft = int(rng.integers(12, 17))
+    km2 = 2 * int(np.ceil(512.0 / dt))
+    while (1 << log_nfft) < 2 * km2:               # room for data beside the 2 x 512 s margins
+        log_nfft += 1
+    n_samples = int(rng.uniform(0.35, 0.95) * ((1 << log_nfft) - km2))
+    if n_samples * dt < 2 * 1800.0:                # at least two 1800 s slots of data
+        n_samples = int(min(((1 << log_nfft) - km2), 2.5 * 1800.0 / dt))
+    band = float(rng.choice([1.0, 0.5, 0.25, 0.1])) / dt
+    p = synth.small_problem(seed=2000 + case, n_det=int(rng.integers(1, 4)), n_samples=n_samples, dt=dt, n_fft=1 << log_nfft,
+                            dterms=int(rng.choice([1, 3, 8, 20, 32])), n_templates=3, gap_frac=0.0,
+                            weights=bool(rng.integers(0, 2)), rho=float(rng.choice([6.0, 15.0])), f_min=float(rng.uniform(20.0, 900.0)),
+                            band=band, fddot=float(rng.choice([0.0, 3e-15])))
+    # heterodyne frequency away from the band centre (the plan shifts the band to FFT bin 0)
+    p.f_het = p.f_min + float(rng.uniform(0.0, 1.0)) * band
+    gap = 0.3 if n_samples * dt >= 8 * 1800.0 else 0.0          # keep at least a few data slots
+    p = synth.make_problem(p.name, p.detectors, p.n_samples, p.dt, p.f_min, p.band, p.f_het, p.n_fft, p.dterms, p.templates,
+                           seed=p.seed, gap_frac=gap, weight_range=(0.5, 2.0), injection=p.injection,
+                           injection_template=p.injection_template, snap_injection_to_bin=True)
+    _check_bank(p)
