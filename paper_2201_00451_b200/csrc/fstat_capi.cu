@@ -28,6 +28,8 @@ struct HostRing {            // device row buffers for the *_host variants
 
 }  // namespace
 
+#define STAGE_SLOTS 4
+
 struct fstat_plan {
     PlanGeom g{};
     cudaStream_t stream = nullptr;
@@ -56,7 +58,10 @@ struct fstat_plan {
     float *d_topk_v = nullptr; int *d_topk_i = nullptr; size_t topk_cap = 0;
     // pinned staging
     SkyConst *h_sky = nullptr; TmplDesc *h_tmpl = nullptr;
-    cudaEvent_t staging_ev = nullptr; cudaEvent_t chunk_ev = nullptr;
+    // pinned staging comes in STAGE_SLOTS rotating slots (each of capacity tmpl_cap / sky_cap), so that a call does not
+    // have to wait for the previous call's GPU work before it can prepare its descriptors
+    cudaEvent_t staging_ev[4] = {nullptr, nullptr, nullptr, nullptr}; int stage_slot = 0;
+    cudaEvent_t chunk_ev = nullptr;
     int64_t launches = 0;
     std::string err;
     // optional per-kernel-class timing (fstat_set_profile)
@@ -324,13 +329,14 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) 
 }
 
 int ensure_tmpl_capacity(fstat_plan *p, size_t n_tmpl, size_t n_groups) {
+    if (n_tmpl > p->tmpl_cap || n_groups > p->sky_cap) CUDA_TRY(p, cudaStreamSynchronize(p->stream));   // staging in flight
     if (n_tmpl > p->tmpl_cap) {
         if (p->d_tmpl) cudaFree(p->d_tmpl);
         if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
         p->d_tmpl = nullptr; p->h_tmpl = nullptr; p->tmpl_cap = 0;
         const size_t cap = n_tmpl + n_tmpl / 2 + 16;
         CUDA_TRY(p, cudaMalloc(&p->d_tmpl, cap * sizeof(TmplDesc)));
-        CUDA_TRY(p, cudaMallocHost(&p->h_tmpl, cap * sizeof(TmplDesc)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_tmpl, STAGE_SLOTS * cap * sizeof(TmplDesc)));
         p->tmpl_cap = cap;
     }
     if (n_groups > p->sky_cap) {
@@ -341,9 +347,9 @@ int ensure_tmpl_capacity(fstat_plan *p, size_t n_tmpl, size_t n_groups) {
         p->d_sky = nullptr; p->h_sky = nullptr; p->d_abcd = nullptr; p->h_abcd = nullptr; p->sky_cap = 0;
         const size_t cap = n_groups + n_groups / 2 + 16;
         CUDA_TRY(p, cudaMalloc(&p->d_sky, cap * sizeof(SkyConst)));
-        CUDA_TRY(p, cudaMallocHost(&p->h_sky, cap * sizeof(SkyConst)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_sky, STAGE_SLOTS * cap * sizeof(SkyConst)));
         CUDA_TRY(p, cudaMalloc(&p->d_abcd, cap * sizeof(SkyABCD)));
-        CUDA_TRY(p, cudaMallocHost(&p->h_abcd, cap * sizeof(SkyABCD)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_abcd, STAGE_SLOTS * cap * sizeof(SkyABCD)));
         p->sky_cap = cap;
     }
     return FSTAT_OK;
@@ -428,22 +434,27 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     rc = ensure_sky_slots(p, groups.size());
     if (rc) return rc;
     // staging buffers are reused between calls: wait until the previous upload has been consumed
-    CUDA_TRY(p, cudaEventSynchronize(p->staging_ev));
+    const int slot = p->stage_slot;
+    p->stage_slot = (slot + 1) % STAGE_SLOTS;
+    CUDA_TRY(p, cudaEventSynchronize(p->staging_ev[slot]));
+    SkyConst *h_sky = p->h_sky + (size_t)slot * p->sky_cap;
+    SkyABCD *h_abcd = p->h_abcd + (size_t)slot * p->sky_cap;
+    TmplDesc *h_tmpl = p->h_tmpl + (size_t)slot * p->tmpl_cap;
     for (size_t gi = 0; gi < groups.size(); ++gi) {
-        fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &p->h_sky[gi]);
-        sky_abcd(p, groups[gi].alpha, groups[gi].delta, &p->h_abcd[gi]);
-        if (p->h_abcd[gi].bad) p->pending_edom = true;
+        fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &h_sky[gi]);
+        sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi]);
+        if (h_abcd[gi].bad) p->pending_edom = true;
         for (int t = groups[gi].first; t < groups[gi].first + groups[gi].count; ++t) {
-            p->h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
-            p->h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
-            p->h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
-            p->h_tmpl[t].pad = 0;
+            h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
+            h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
+            h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
+            h_tmpl[t].pad = 0;
         }
     }
-    CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, p->h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
-    CUDA_TRY(p, cudaMemcpyAsync(p->d_abcd, p->h_abcd, groups.size() * sizeof(SkyABCD), cudaMemcpyHostToDevice, p->stream));
-    CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
-    CUDA_TRY(p, cudaEventRecord(p->staging_ev, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_abcd, h_abcd, groups.size() * sizeof(SkyABCD), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaEventRecord(p->staging_ev[slot], p->stream));
 
     if (out.mode == OUT_TOPK) { rc = ensure_topk_scratch(p); if (rc) return rc; }
     if (out.mode == OUT_HOST_ROWS) { rc = ensure_host_ring(p); if (rc) return rc; }
@@ -513,7 +524,7 @@ void destroy_impl(fstat_plan *p) {
     if (p->h_sky) cudaFreeHost(p->h_sky);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
     if (p->h_abcd) cudaFreeHost(p->h_abcd);
-    if (p->staging_ev) cudaEventDestroy(p->staging_ev);
+    for (int i = 0; i < STAGE_SLOTS; ++i) if (p->staging_ev[i]) cudaEventDestroy(p->staging_ev[i]);
     if (p->chunk_ev) cudaEventDestroy(p->chunk_ev);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
@@ -673,7 +684,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     for (int X = 0; X < n_det; ++X) p->det[X] = det[X];
 
     SETUP_TRY(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
-    SETUP_TRY(cudaEventCreateWithFlags(&p->staging_ev, cudaEventDisableTiming));
+    for (int i = 0; i < STAGE_SLOTS; ++i) SETUP_TRY(cudaEventCreateWithFlags(&p->staging_ev[i], cudaEventDisableTiming));
     SETUP_TRY(cudaEventCreateWithFlags(&p->chunk_ev, cudaEventDisableTiming));
     SETUP_TRY(cudaMalloc(&p->d_series, (size_t)n_det * g.series_stride * sizeof(float2)));
     SETUP_TRY(cudaMemsetAsync(p->d_series, 0, (size_t)n_det * g.series_stride * sizeof(float2), p->stream));
@@ -729,7 +740,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
                 p->mom[X][q] = t;
             }
     }
-    SETUP_TRY(cudaEventRecord(p->staging_ev, p->stream));
+    for (int i = 0; i < STAGE_SLOTS; ++i) SETUP_TRY(cudaEventRecord(p->staging_ev[i], p->stream));
     // the caller may free its buffers when we return
     SETUP_TRY(cudaStreamSynchronize(p->stream));
 #undef SETUP_TRY
@@ -796,10 +807,13 @@ int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta, float *S_
     CUDA_TRY(plan, cudaSetDevice(plan->device));
     int rc = ensure_tmpl_capacity(plan, 1, 1);
     if (rc) return rc;
-    CUDA_TRY(plan, cudaEventSynchronize(plan->staging_ev));
-    fill_sky_const(plan, alpha, delta, &plan->h_sky[0]);
-    CUDA_TRY(plan, cudaMemcpyAsync(plan->d_sky, plan->h_sky, sizeof(SkyConst), cudaMemcpyHostToDevice, plan->stream));
-    CUDA_TRY(plan, cudaEventRecord(plan->staging_ev, plan->stream));
+    const int slot = plan->stage_slot;
+    plan->stage_slot = (slot + 1) % STAGE_SLOTS;
+    CUDA_TRY(plan, cudaEventSynchronize(plan->staging_ev[slot]));
+    SkyConst *h_sky = plan->h_sky + (size_t)slot * plan->sky_cap;
+    fill_sky_const(plan, alpha, delta, h_sky);
+    CUDA_TRY(plan, cudaMemcpyAsync(plan->d_sky, h_sky, sizeof(SkyConst), cudaMemcpyHostToDevice, plan->stream));
+    CUDA_TRY(plan, cudaEventRecord(plan->staging_ev[slot], plan->stream));
     CUDA_TRY(plan, cudaMemsetAsync(S_dev, 0, (size_t)plan->g.n_fft * sizeof(float4), plan->stream));
     rc = launch_sky_batch(plan, 0, 1, (float4 *)S_dev, 0);
     if (rc) return rc;
