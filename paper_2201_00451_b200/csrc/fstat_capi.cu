@@ -308,7 +308,8 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     {
         ProfScope ps(p, 2);
         const int tiles2 = 1 << (l1 - p->g.log_w2);
-        if (p->g.p2_elems == 32 && l2 == 10) rc = launch_pass<10, 12, true, 32>(p, a, tiles2, nt);
+        if (p->g.p2_elems == 32 && l2 == 10 && tile_log2(p) == 13) rc = launch_pass<10, 13, true, 32>(p, a, tiles2, nt);
+        else if (p->g.p2_elems == 32 && l2 == 10) rc = launch_pass<10, 12, true, 32>(p, a, tiles2, nt);
         else if (p->g.p2_elems == 32 && l2 == 9) rc = launch_pass<9, 12, true, 32>(p, a, tiles2, nt);
         else DISPATCH_TILE(l2, tile_log2(p), true, p, a, tiles2, nt);
     }
@@ -667,8 +668,8 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
     }
     {   // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
-        // sub-FFTs of 2^9 and 2^10 points on 2^12-element tiles; FSTAT_P2_ELEMS=16 switches it off (experiments)
-        g.p2_elems = ((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) ? 32 : 16;
+        // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles; FSTAT_P2_ELEMS=16 switches it off (experiments)
+        g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
         const char *e = getenv("FSTAT_P2_ELEMS");
         if (e && atoi(e) == 16) g.p2_elems = 16;
     }
