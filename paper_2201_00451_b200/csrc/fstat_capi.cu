@@ -659,8 +659,9 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
         // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
         // pass 2: 2^12-element tiles; 2^13 (8 rows of 2^10 points: 128-byte runs in pass 1's transposed store, 32-byte
-        // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2
-        g.log_tile2 = (g.log_n2 == 12 || (g.log_n2 == 10 && L >= 21)) ? 13 : 12;
+        // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2; likewise 4 rows
+        // of 2^11 points at 2^23, which lets pass 1 run one 2^12-point column per 2^12-element tile
+        g.log_tile2 = (g.log_n2 == 12 || (g.log_n2 == 10 && L >= 21) || (g.log_n2 == 11 && L == 23)) ? 13 : 12;
         // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
         // of a single column needs >= 4 rows per pass-2 tile
         const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
