@@ -41,6 +41,7 @@ struct fstat_plan {
     int n_sm = 148;
     // device memory
     float2 *d_series = nullptr;
+    void *d_tmp[3] = {nullptr, nullptr, nullptr};   // setup-time scratch (freed by destroy_impl if setup fails half-way)
     double4 *d_base = nullptr;        // [n_src] trigonometric base of the timing model per SSB grid point
     float2 *d_farrow = nullptr;       // [n_det][FARROW_NC/2][N+1] float4: Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
@@ -517,7 +518,8 @@ void destroy_impl(fstat_plan *p) {
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_base); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
+    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_base);
+    for (void *t : p->d_tmp) cudaFree(t); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
     cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
@@ -709,7 +711,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
     {   // Farrow-filtered copies of the series (sky_kernels.cuh), once per plan
         const std::vector<float> fc = farrow_coefficients(dterms);
-        float *d_fc = nullptr;
+        float *&d_fc = reinterpret_cast<float *&>(p->d_tmp[0]);
         SETUP_TRY(cudaMalloc(&d_fc, fc.size() * sizeof(float)));
         SETUP_TRY(cudaMemcpyAsync(d_fc, fc.data(), fc.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
         SETUP_TRY(cudaMalloc(&p->d_farrow, (size_t)n_det * (n_samples + 1) * FARROW_NC * sizeof(float2)));
@@ -722,11 +724,11 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         ++p->launches;
         SETUP_TRY(cudaGetLastError());
         SETUP_TRY(cudaStreamSynchronize(p->stream));
-        cudaFree(d_fc);
+        cudaFree(d_fc); d_fc = nullptr;
     }
     {   // antenna moment matrices M_X (sky_kernels.cuh), once per plan
         const int nblk = (int)((n_samples + MOM_THREADS * MOM_PER_THREAD - 1) / (MOM_THREADS * MOM_PER_THREAD));
-        double *d_part = nullptr, *d_lon = nullptr;
+        double *&d_part = reinterpret_cast<double *&>(p->d_tmp[1]), *&d_lon = reinterpret_cast<double *&>(p->d_tmp[2]);
         std::vector<double> lon(n_det), part((size_t)n_det * nblk * MOM_TERMS);
         for (int X = 0; X < n_det; ++X) lon[X] = det[X].lon_east_rad;
         SETUP_TRY(cudaMalloc(&d_part, part.size() * sizeof(double)));
@@ -737,7 +739,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         SETUP_TRY(cudaGetLastError());
         SETUP_TRY(cudaMemcpyAsync(part.data(), d_part, part.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
         SETUP_TRY(cudaStreamSynchronize(p->stream));
-        cudaFree(d_part); cudaFree(d_lon);
+        cudaFree(d_part); cudaFree(d_lon); d_part = nullptr; d_lon = nullptr;
         for (int X = 0; X < n_det; ++X)
             for (int q = 0; q < MOM_TERMS; ++q) {
                 double t = 0.0;
