@@ -6,13 +6,13 @@
 //   pass 2 (one CTA = W adjacent rows   m1):    X[m1 + N1 m2] = sum_k2 T[k2][m1] W_N2^{k2 m2}
 //
 // An element is a float4 = (Re Fa, Re Fb, Im Fa, Im Fb): both transforms run in lock step and
-// share every twiddle.  Each thread keeps 16 elements in registers; shared memory is the exchange
-// buffer between radix passes (one buffer, two barriers per exchange).  CTAs are persistent: each
-// loops over tiles, and as soon as the last radix pass of a tile has pulled its inputs out of
-// the buffer, the NEXT tile's global loads are started into it with cp.async (L2 -> shared, no
-// registers), so they fly while the last pass, the twiddle/2F epilogue and the global stores of
-// the current tile execute.  Each thread prefetches exactly the elements it will itself read in
-// pass 0, so the hand-over needs cp.async.wait_group only, no extra barrier.
+// share every twiddle.  Each thread keeps E = 16 elements in registers (32 in the two-pass radix-32
+// plans of pass 2); shared memory is the exchange buffer between radix passes (one buffer, two
+// barriers per exchange).  CTAs are persistent: each loops over tiles, and as soon as the last radix
+// pass of a tile has pulled its inputs out of the buffer, the NEXT tile -- one contiguous block of
+// global memory thanks to the tile-blocked layouts of S and T -- is copied into it by one thread with
+// 1-D bulk TMA (cp.async.bulk + mbarrier; no registers), so the copy flies while the last pass, the
+// twiddle / 2F epilogue and the global stores of the current tile execute.
 #pragma once
 #include "fstat_common.cuh"
 
@@ -128,7 +128,7 @@ template <int LOGW, int LOGR0> __device__ __forceinline__ int sm_phys(int idx, i
     return ((idx ^ hi) << LOGW) + (w ^ lo);
 }
 
-// One radix-R Stockham pass on the 16 register elements: twiddle (if P > 1) and DFT.
+// One radix-R Stockham pass on the E register elements: twiddle (if P > 1) and DFT.
 // Work item bb of this thread is butterfly i = item_i(bb); inputs sit in slots bb*R + r.
 template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST>
 struct PassIdx {
