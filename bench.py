@@ -301,6 +301,8 @@ def run_ours(args):
         roofline = {"bound": "hbm", "kernel": dom + "_kernel", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                     "fft_pair_achieved": both, "fft_pair_frac": both / peak,
+                    # SURVEY.md 8(d) R_min: compulsory traffic only (raw series in, 2F out) over the whole step
+                    "r_min_frac": (8 * p.n_samples * p.n_det + 4 * nb) * n_t * args.steps / (total_ms * 1e-3) / 1e9 / peak,
                     "alu_tflops": flops / (fft_ms * 1e-3) / 1e12, "alu_peak_tflops": alu_peak,
                     "alu_frac": flops / (fft_ms * 1e-3) / 1e12 / alu_peak,
                     "share_of_step": prof[dom][0] / total_ms if world == 1 else None}
