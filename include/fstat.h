@@ -107,8 +107,9 @@ typedef struct fstat_plan fstat_plan_t;   /* opaque */
  *
  * Device memory owned by the plan: the series (8 B per sample and detector), its Farrow-filtered
  * copies (80 B per sample and detector: the interpolation taps folded once), 32 B per
- * SSB grid point of timing-model constants, 16 B x n_fft per sky slot (<= 64 MB in total) and up to
- * 2 GB of FFT intermediates; scratch rows for the top-k and host-output modes on first use.
+ * SSB grid point of timing-model constants, 16 B x n_fft per sky position of a batch (grown on demand, <= 1 GB) and up to
+ * 4 GB of FFT intermediates (16 B x n_fft per template of a launch, grown on demand); scratch rows for the top-k and
+ * host-output modes on first use.
  */
 FSTAT_API int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det,
                 const void *const *series_c64, int64_t n_samples, double t_start, double dt, double f_het,

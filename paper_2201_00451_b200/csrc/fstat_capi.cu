@@ -47,7 +47,8 @@ struct fstat_plan {
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
     float4 *d_S = nullptr;   int n_sky_slots = 0, max_sky_slots = 1;   // S buffers: allocated / allowed (grown on demand)
-    float4 *d_T = nullptr;   int n_inflight = 0;
+    float4 *d_T = nullptr;   int n_inflight = 0;   // four-step intermediates of the templates of one launch
+    int t_cap = 0;                                 // templates d_T currently holds (grown on demand up to n_inflight)
     SkyConst *d_sky = nullptr; size_t sky_cap = 0;
     SkyABCD *d_abcd = nullptr; SkyABCD *h_abcd = nullptr;   // per sky group of the current call (capacity sky_cap)
     double mom[FSTAT_MAX_DET][MOM_TERMS];                   // antenna moment matrices M_X (sky_kernels.cuh)
@@ -284,6 +285,12 @@ int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
 int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
+    if (nt > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
+        CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        cudaFree(p->d_T); p->d_T = nullptr; p->t_cap = 0;
+        if (cudaMalloc(&p->d_T, (size_t)nt * p->g.n_fft * sizeof(float4)) != cudaSuccess) { cudaGetLastError(); return fail(p, FSTAT_ENOMEM, "device allocation of the FFT intermediates failed"); }
+        p->t_cap = nt;
+    }
     FftArgs a{};
     a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd + g0;
     a.twoF = rows; a.twoF_stride = row_stride; a.gmax = gmax;
@@ -708,7 +715,6 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     p->n_inflight = default_inflight(n_fft, g.log_tile2);
     p->max_sky_slots = max_sky_slots_for(n_fft);
     if (ensure_sky_slots(p, 1) != FSTAT_OK) return bail(FSTAT_ENOMEM);
-    SETUP_TRY(cudaMalloc(&p->d_T, (size_t)p->n_inflight * n_fft * sizeof(float4)));
     {   // Farrow-filtered copies of the series (sky_kernels.cuh), once per plan
         const std::vector<float> fc = farrow_coefficients(dterms);
         float *&d_fc = reinterpret_cast<float *&>(p->d_tmp[0]);
@@ -852,13 +858,12 @@ int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight) {
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
     const int tb = n_inflight == 0 ? default_inflight(plan->g.n_fft, plan->g.log_tile2) : n_inflight;
     if (tb == plan->n_inflight) return FSTAT_OK;
-    cudaFree(plan->d_T); plan->d_T = nullptr;
+    cudaFree(plan->d_T); plan->d_T = nullptr; plan->t_cap = 0;
     cudaFree(plan->d_rows); plan->d_rows = nullptr;
     cudaFree(plan->d_gmax); plan->d_gmax = nullptr;
     for (int i = 0; i < 2; ++i) { cudaFree(plan->ring.buf[i]); plan->ring.buf[i] = nullptr; if (plan->ring.done[i]) cudaEventDestroy(plan->ring.done[i]); plan->ring.done[i] = nullptr; }
     plan->ring.rows = 0;
     plan->n_inflight = tb;
-    CUDA_TRY(plan, cudaMalloc(&plan->d_T, (size_t)tb * plan->g.n_fft * sizeof(float4)));
     return FSTAT_OK;
 }
 
