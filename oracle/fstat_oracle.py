@@ -21,7 +21,9 @@ P2 noise-free 2F = rho^2, P3 E[2F]=4+rho^2, P4 brute-force detector-frame sum
 (eq. 4-5) on tiny inputs, P5 antenna closed form vs tensor form, P6
 invariances, P7 zero-delay special case = plain zero-padded numpy FFT, P8 the
 chi^2_4 tail against the paper's printed false-alarm figure,
-Fig. 1's code formula with E=0 against eq. 8.
+Fig. 1's code formula with E=0 against eq. 8; eq. 9-10 metrics on hand-computed
+vectors; the semi-coherent sum (chi^2 with 4 N_seg dof, sum of rho^2_seg); the
+single-detector statistic (sum_X rho_X^2 = rho^2).  No function is unpinned.
 """
 from __future__ import annotations
 
@@ -160,9 +162,13 @@ def per_sky(prob, alpha: float, delta: float) -> Dict[str, object]:
 # Steps 5-8 (per template): phases, Fa(t), Fb(t), FFTs, 2F.  PAPER.md:81, :84-85,
 # eq. 8 in the unit-free normalisation of DESIGN.md G5.
 # ---------------------------------------------------------------------------
-def bin_shift(prob) -> int:
-    """FFT index of output bin 0: round((f_min - f_het)/df)."""
-    return int(round((prob.f_min - prob.f_het) * prob.n_fft * prob.dt))
+def band_shift_cycles(prob, k: np.ndarray) -> np.ndarray:
+    """Phase ramp (cycles, reduced mod 1) that places output bin 0 exactly at f_min: FFT index m of the
+    series sampled at (k - K_m) dt is frequency f_het + m df, so Fa(f_min + q df) = sum_k Ya_k
+    exp(-2 pi i [(f_min - f_het) dt k + q k / n_fft])  ("Fa(f - f_h)"; S13).  When
+    (f_min - f_het)/df is an integer s this is the index shift q -> (q + s) mod n_fft of the plain FFT."""
+    x = (prob.f_min - prob.f_het) * prob.dt * np.asarray(k, dtype=np.float64)
+    return x - np.floor(x)
 
 
 def validate(prob) -> None:
@@ -193,10 +199,12 @@ def fstat_FaFb(prob, template, sky: Optional[dict] = None):
         y = s["z"] * np.exp(-2j * math.pi * cyc)
         Ya[:n_src] += s["wk"] * s["a"] * y
         Yb[:n_src] += s["wk"] * s["b"] * y
+    ramp = np.exp(-2j * math.pi * band_shift_cycles(prob, np.arange(n_src)))     # step 7: bin 0 at f_min (S13)
+    Ya[:n_src] *= ramp
+    Yb[:n_src] *= ramp
     Fa = np.fft.fft(Ya)
     Fb = np.fft.fft(Yb)
-    idx = (np.arange(prob.n_bins) + bin_shift(prob)) % prob.n_fft
-    return Fa[idx], Fb[idx], sky["ABCD"]
+    return Fa[:prob.n_bins], Fb[:prob.n_bins], sky["ABCD"]
 
 
 def twoF_from_FaFb(Fa, Fb, A, B, C, D):
@@ -224,6 +232,58 @@ def fstat_2F_bank(prob, template_indices=None) -> np.ndarray:
             cache_key, cache = key, per_sky(prob, key[0], key[1])
         out[r] = fstat_2F(prob, t, cache)
     return out
+
+
+# ---------------------------------------------------------------------------
+# Single-detector statistic and the semi-coherent sum over segments
+# ---------------------------------------------------------------------------
+def single_detector_view(prob, X: int):
+    """The same problem restricted to detector X (a shallow copy with one-element lists)."""
+    import copy
+    q = copy.copy(prob)
+    q.detectors = [prob.detectors[X]]
+    q.series = [prob.series[X]]
+    q.timestamps = [prob.timestamps[X]]
+    q.weights = [prob.weights[X]]
+    return q
+
+
+def fstat_2F_per_detector(prob, template) -> np.ndarray:
+    """2F_X[n_det][n_bins]: eq. 8 with every sum over detector X only -- the per-detector
+    quantity the paper's accuracy tooling compares.  By definition: the whole path on the
+    one-detector problem."""
+    return np.stack([fstat_2F(single_detector_view(prob, X), template) for X in range(prob.n_det)])
+
+
+def fstat_2F_semicoherent(probs, templates, bin_offsets=None) -> np.ndarray:
+    """Semi-coherent statistic (section 6: "each segment is searched using the F-statistic, and
+    results from all segments are summed"): out[q] = sum_s 2F_s[q + off_s], where segment s has its own problem
+    (data, t_start = its reference time), its own template (the signal's parameters at that reference time) and a
+    bin offset off_s (the signal's frequency drift since the search's reference time, in bins; default 0).
+    Bins that fall outside a segment's band add nothing."""
+    n_bins = probs[0].n_bins
+    out = np.zeros(n_bins)
+    for s, (prob, tmpl) in enumerate(zip(probs, templates)):
+        assert prob.n_bins == n_bins
+        row = fstat_2F(prob, tmpl)
+        off = 0 if bin_offsets is None else int(bin_offsets[s])
+        q = np.arange(n_bins)
+        src = q + off
+        ok = (src >= 0) & (src < n_bins)
+        out[ok] += row[src[ok]]
+    return out
+
+
+def chi2_sf(x, dof: int):
+    """Pr(chi^2_dof > x) for even dof: e^{-x/2} sum_{j < dof/2} (x/2)^j / j!  (dof = 4: chi2_4_sf)."""
+    assert dof % 2 == 0 and dof > 0
+    x = np.asarray(x, dtype=np.float64)
+    term = np.ones_like(x)
+    acc = np.ones_like(x)
+    for j in range(1, dof // 2):
+        term = term * (0.5 * x) / j
+        acc = acc + term
+    return np.exp(-0.5 * x) * acc
 
 
 # ---------------------------------------------------------------------------
@@ -291,8 +351,12 @@ def threshold_candidates(twoF_row: np.ndarray, threshold: float, k: int):
 
 
 def comparison_metrics(x: np.ndarray, y: np.ndarray):
-    """r_1, r_2 of eq. 9 and the angle of eq. 10."""
+    """The paper's vector comparison metrics: relative errors
+    r_p(x, y) = 2 ||x - y||_p / (||x||_p + ||y||_p) for p = 1, 2 (eq. 9) and the angle
+    theta = arccos( Re(x^* . y) / (||x||_2 ||y||_2) ) (eq. 10), for real or complex vectors."""
+    x = np.asarray(x).ravel()
+    y = np.asarray(y).ravel()
     r1 = 2.0 * np.sum(np.abs(x - y)) / (np.sum(np.abs(x)) + np.sum(np.abs(y)))
     r2 = 2.0 * np.linalg.norm(x - y) / (np.linalg.norm(x) + np.linalg.norm(y))
     c = np.real(np.vdot(x, y)) / (np.linalg.norm(x) * np.linalg.norm(y))
-    return r1, r2, math.acos(min(1.0, max(-1.0, c)))
+    return float(r1), float(r2), math.acos(min(1.0, max(-1.0, c)))

@@ -342,7 +342,7 @@ def small_problem(seed: int = 7, n_det: int = 2, n_samples: int = 20000, dt: flo
                   n_fft: int = 1 << 15, dterms: int = 8, n_templates: int = 4, gap_frac: float = 0.3,
                   weights: bool = True, rho: Optional[float] = 12.0, noise: bool = True,
                   f_min: float = 120.0, band: Optional[float] = None, fddot: float = 0.0,
-                  ephem: Optional[dict] = None) -> Problem:
+                  ephem: Optional[dict] = None, f_het: Optional[float] = None) -> Problem:
     """A seconds-scale problem with the structure of config 2 (ragged length,
     gaps, weights, two detectors) used by the parity tests and smoke()."""
     band = 0.5 / dt if band is None else band
@@ -354,7 +354,7 @@ def small_problem(seed: int = 7, n_det: int = 2, n_samples: int = 20000, dt: flo
                         fddot=fddot, alpha=SKY0[0], delta=SKY0[1])
     tm = _fdot_bank(SKY0[0], SKY0[1], f_min, fdots, (fddot,))
     dets = [H1, L1, V1][:n_det]
-    return make_problem(f"small_s{seed}", dets, n_samples, dt, f_min, band, f_min + band / 2, n_fft, dterms, tm,
+    return make_problem(f"small_s{seed}", dets, n_samples, dt, f_min, band, f_min + band / 2 if f_het is None else f_het, n_fft, dterms, tm,
                         seed=seed, gap_frac=gap_frac, weight_range=(0.5, 2.0) if weights else None,
                         injection=inj, injection_template=it if inj else None, noise=noise, ephem=ephem,
                         snap_injection_to_bin=True)

@@ -110,6 +110,21 @@ def test_noise_free_single_detector_no_gaps():
     assert abs(twoF[0].max() / 400.0 - 1.0) < 2e-3
 
 
+# -- S13 (exact band placement): bin q is f_min + q df whatever f_het.  With the heterodyne frequency off the
+# bin grid a noise-free injection placed exactly on a labelled bin must still give 2F = rho^2 there (rounding the
+# shift to whole FFT bins would leave the signal up to df/2 off the bin: 2F drops by up to ~36 %)
+@pytest.mark.parametrize("off", [0.45, -0.3, 0.0])
+def test_bins_are_labelled_exactly_with_off_grid_heterodyne(off):
+    q = synth.small_problem(noise=False, rho=12.0, n_templates=3, n_samples=20000, n_fft=1 << 15)
+    p = synth.small_problem(noise=False, rho=12.0, n_templates=3, n_samples=20000, n_fft=1 << 15,
+                            f_het=q.f_het + off * q.df)
+    inj_bin = int(round((p.injection.f - p.f_min) / p.df))
+    assert abs(p.injection.f - (p.f_min + inj_bin * p.df)) < 1e-9 * p.df * p.n_fft
+    twoF = O.fstat_2F(p, p.templates[p.injection_template])
+    assert twoF.argmax() == inj_bin
+    assert abs(twoF[inj_bin] / 144.0 - 1.0) < 2e-3
+
+
 # -- P1: pure noise => chi^2_4 (mean 4, var 8) over the central bins
 def test_pure_noise_is_chi2_4():
     p = synth.small_problem(seed=11, rho=None, n_samples=200000, n_fft=1 << 18, n_templates=2, gap_frac=0.5)
@@ -202,7 +217,9 @@ def test_frozen_earth_is_a_fixed_fir_filter():
     dl = shift_samples - n0
     taps = {mm: np.sinc(dl - mm) * (0.54 + 0.46 * math.cos(math.pi * (dl - mm) / (D + 0.5))) for mm in range(-D, D + 1)}
     bins = np.array([0, 3, 100, p.n_bins // 2, p.n_bins - 2])
-    m = (bins + O.bin_shift(p)) % p.n_fft
+    s_bins = (p.f_min - p.f_het) * p.n_fft * p.dt                  # f_het on the bin grid here: an integer shift
+    assert s_bins == round(s_bins)
+    m = (bins + int(s_bins)) % p.n_fft
     x = p.series[0].astype(np.complex128)
     j = np.arange(p.n_samples)
     out = []
@@ -255,7 +272,9 @@ def test_zero_delay_special_case_is_plain_fft():
     # explicit DFT matrix on a subset of bins (not numpy.fft), shifted by K_m samples
     km = O.k_margin(p)
     bins = np.array([0, 1, 17, p.n_bins // 2, p.n_bins - 1])
-    m = (bins + O.bin_shift(p)) % p.n_fft
+    s_bins = (p.f_min - p.f_het) * p.n_fft * p.dt                  # f_het on the bin grid here: an integer shift
+    assert s_bins == round(s_bins)
+    m = (bins + int(s_bins)) % p.n_fft
     k = np.arange(p.n_fft)
     Wm = np.exp(-2j * np.pi * np.outer(m, k) / p.n_fft)
     shift = np.exp(-2j * np.pi * m * km / p.n_fft)
@@ -295,3 +314,84 @@ def test_threshold_candidates_brute_force():
     assert np.all(v == row[i]) and np.all(v > 9.0)
     v, i, c = O.threshold_candidates(row, 1e9, 6)
     assert c == 0 and len(i) == 0
+
+
+# -- eq. 9-10: hand-computed cases
+def test_comparison_metrics_hand_computed():
+    x = np.array([3.0, 4.0])
+    y = np.array([4.0, 3.0])
+    r1, r2, th = O.comparison_metrics(x, y)
+    # |x-y|_1 = 2, |x|_1 = |y|_1 = 7 -> 2*2/14; |x-y|_2 = sqrt 2, |x|_2 = |y|_2 = 5 -> 2 sqrt2 / 10; cos = 24/25
+    assert abs(r1 - 4.0 / 14.0) < 1e-15 and abs(r2 - 2.0 * math.sqrt(2.0) / 10.0) < 1e-15
+    assert abs(th - math.acos(24.0 / 25.0)) < 1e-15
+    assert O.comparison_metrics(x, x) == (0.0, 0.0, 0.0)
+    assert abs(O.comparison_metrics(np.array([1.0, 0.0]), np.array([0.0, 2.0]))[2] - math.pi / 2) < 1e-15
+    # y = 2x: r1 = r2 = 2|x|/(3|x|) = 2/3 whatever the norm, angle 0
+    r1, r2, th = O.comparison_metrics(x, 2 * x)
+    assert abs(r1 - 2.0 / 3.0) < 1e-15 and abs(r2 - 2.0 / 3.0) < 1e-15 and th < 1e-7
+    # complex vectors: x^* . y conjugates x; a global phase i turns the vectors "orthogonal" in the sense of eq. 10
+    z = np.array([1.0 + 1.0j, 2.0 - 1.0j])
+    r1, r2, th = O.comparison_metrics(z, 1j * z)
+    assert abs(th - math.pi / 2) < 1e-15 and abs(r2 - math.sqrt(2.0)) < 1e-15
+    assert abs(O.comparison_metrics(z, -z)[2] - math.pi) < 1e-7
+
+
+# -- single-detector statistic: for noise-free data 2F_X = rho_X^2 at the injected bin, and the rho_X^2 add up to
+# the coherent rho^2 (A = sum_X A_X etc. and the same amplitudes in every detector)
+def test_per_detector_statistic_noise_free():
+    p = synth.small_problem(seed=8, noise=False, rho=15.0, n_templates=3, n_samples=30000, n_fft=1 << 15)
+    t = p.templates[p.injection_template]
+    per = O.fstat_2F_per_detector(p, t)
+    assert per.shape == (2, p.n_bins)
+    inj_bin = int(round((p.injection.f - p.f_min) / p.df))
+    assert per[0].argmax() == inj_bin and per[1].argmax() == inj_bin
+    assert abs((per[0, inj_bin] + per[1, inj_bin]) / 225.0 - 1.0) < 2e-3
+    # expected split from the generator's own (geometric) antenna functions and weights
+    inj = p.injection
+    a1, a2, a3, a4 = synth._jks_amplitudes(1.0, inj.cosi, inj.psi, inj.phi0)
+    aa, ab = complex(a1, -a3), complex(a2, -a4)
+    tp = np.arange(p.n_samples) * p.dt
+    rho2 = []
+    for X, det in enumerate(p.detectors):
+        a, b = synth.geometric_antenna(det, p.ephem, inj.alpha, inj.delta, tp)
+        w = O.slot_weights(p, X)[np.minimum((tp / p.t_sft).astype(int), 10 ** 9)]
+        A, B, C = np.sum(w * a * a), np.sum(w * b * b), np.sum(w * a * b)
+        rho2.append(A * abs(aa) ** 2 + B * abs(ab) ** 2 + 2 * C * (aa * ab.conjugate()).real)
+    frac = np.array(rho2) / sum(rho2)
+    np.testing.assert_allclose(per[:, inj_bin] / 225.0, frac, rtol=3e-3)
+    # coherent statistic of the two-detector problem is NOT the sum of the per-detector ones off the peak (G6)
+    coh = O.fstat_2F(p, t)
+    assert abs(coh[inj_bin] / 225.0 - 1.0) < 2e-3
+    assert np.abs(coh - per.sum(axis=0)).max() > 1e-3
+
+
+# -- semi-coherent sum: pure noise -> chi^2 with 4 N_seg dof; noise-free injections -> sum of rho_seg^2
+def test_semicoherent_sum_noise_statistics_and_injection():
+    n_seg = 3
+    probs = [synth.small_problem(seed=70 + s, rho=None, n_samples=100000, n_fft=1 << 17, n_templates=1, gap_frac=0.3)
+             for s in range(n_seg)]
+    tm = [q.templates[0] for q in probs]
+    tot = O.fstat_2F_semicoherent(probs, tm)
+    nb = probs[0].n_bins
+    central = tot[nb // 4: 3 * nb // 4]
+    assert central.size >= 30000
+    assert abs(central.mean() - 4.0 * n_seg) < 0.15
+    assert abs(central.var() - 8.0 * n_seg) < 1.5
+    for thr in (16.0, 24.0):
+        assert abs((central > thr).mean() / float(O.chi2_sf(thr, 4 * n_seg)) - 1.0) < 0.15
+    assert abs(float(O.chi2_sf(7.3, 4)) - float(O.chi2_4_sf(7.3))) < 1e-15
+    # noise-free: each segment carries its own rho; with offsets the peaks are brought onto one bin
+    rhos = (6.0, 9.0, 12.0)
+    probs = [synth.small_problem(seed=80 + s, noise=False, rho=rhos[s], n_samples=20000, n_fft=1 << 15, n_templates=3)
+             for s in range(n_seg)]
+    tm = [q.templates[q.injection_template] for q in probs]
+    inj_bin = int(round((probs[0].injection.f - probs[0].f_min) / probs[0].df))
+    tot = O.fstat_2F_semicoherent(probs, tm)
+    assert tot.argmax() == inj_bin
+    assert abs(tot[inj_bin] / sum(r * r for r in rhos) - 1.0) < 2e-3
+    offs = [0, 5, -7]                       # segment s is read at bin q + off_s: its peak appears at inj_bin - off_s
+    tot2 = O.fstat_2F_semicoherent(probs, tm, offs)
+    rows = [O.fstat_2F(q, t) for q, t in zip(probs, tm)]
+    q0 = 1000
+    assert abs(tot2[q0] - (rows[0][q0] + rows[1][q0 + 5] + rows[2][q0 - 7])) < 1e-12
+    assert abs(tot2[2] - (rows[0][2] + rows[1][7])) < 1e-12          # bin 2 - 7 < 0 of segment 2 adds nothing
