@@ -7,6 +7,10 @@ A "step" is one pass of the whole hot path (sky-dependent kernels, fused FFT pas
 one batch of synthetic input: `fstat_compute` on the full template bank of the workload
 (default: BASELINE.json configs[1] -- 2 detectors, 10 d at 2 Hz, 30 % gaps, 1024 fdot templates,
 FFT 2^21).  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+
+Workloads: config1 | config2[:n_templates] | config3:<days>:<band> | config4:<target>[:n_fdot] |
+config5[:n_sky] | sky100:<days>:<band> (the paper's timing protocol: 100 sky positions x one
+spin-down template on a config-3 cell) | small.
 """
 from __future__ import annotations
 
@@ -28,6 +32,9 @@ from paper_2201_00451_b200 import synth  # noqa: E402
 
 METRIC = "2F_bins_per_s"
 UNIT = "2F-bins/s"
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # plain fp32 FMA peak (SMs x lanes x 2 flop x max SM clock)
+# config-3 cells of the bounded sweep carried by the default line: one per FFT length 2^15 .. 2^23
+CONFIG3_SWEEP = [(1, 0.1), (2, 0.1), (1, 0.5), (1, 1.0), (1, 2.0), (2, 2.0), (5, 2.0), (10, 2.0), (20, 2.0)]
 
 
 def make_workload(name: str, rank: int = 0):
@@ -39,6 +46,13 @@ def make_workload(name: str, rank: int = 0):
     elif name.startswith("config3"):          # config3:<days>:<band>
         _, d, b = name.split(":")
         p = synth.config3(float(d) if "." in d else int(d), float(b))
+    elif name.startswith("sky100"):           # sky100:<days>:<band>[:n_sky]
+        parts = name.split(":")
+        d, b = parts[1], parts[2]
+        p = synth.config3(float(d) if "." in d else int(d), float(b), n_templates=1)
+        sky = synth.disc_sky_points(int(parts[3]) if len(parts) > 3 else 100, seed=77, radius=0.3)
+        p.templates = np.array([(a, dl, p.f_min, -5e-10, 0.0) for (a, dl) in sky], dtype=np.float64)
+        p.name = name
     elif name.startswith("config4"):          # config4:<target>[:n_fdot]
         parts = name.split(":")
         p = synth.config4(int(parts[1]), n_fdot=int(parts[2]) if len(parts) > 2 else 256)
@@ -78,30 +92,30 @@ def aggregate_ranks(total_ms: float, units: int, steps: int, dist=None, device=N
 
 
 def algorithmic_bytes(p):
-    """Per-template algorithmic bytes of the two FFT passes (DESIGN.md 'Roofline'):
-    pass 1 reads the detector-summed resampled series (16 B x n_src) and writes the four-step
-    intermediate (16 B x n_fft); pass 2 reads it back and writes 2F (4 B x n_bins).  Their sum is
-    SURVEY.md 8(d)'s B_2pass."""
+    """Per-template algorithmic bytes of the two FFT passes (DESIGN.md 5):
+    pass 1 reads the detector-summed resampled series S (16 B x n_src; served by L2 after the first template of a
+    sky position) and writes the four-step intermediate T (16 B x n_fft); pass 2 reads T back and writes 2F
+    (4 B x n_bins).  Their sum is SURVEY.md 8(d)'s B_2pass."""
     n_src = p.n_samples + 2 * int(np.ceil(512.0 / p.dt))
-    b1 = 16 * n_src + 16 * p.n_fft
-    b2 = 16 * p.n_fft + 4 * p.n_bins
-    return b1, b2
+    return {"S_read": 16 * n_src, "T_write": 16 * p.n_fft, "T_read": 16 * p.n_fft, "twoF_write": 4 * p.n_bins}
 
 
-def ncu_traffic(cls: str, n_fft: int, launches: int, templates: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of this kernel class from the committed
-    `ncu --set full` capture (profiles/r01_traffic.csv holds bytes per template; a launch of the timed run
-    processes templates/launches of them).  None when no capture exists for this FFT length."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+def ncu_traffic_table():
+    """{(class, n_fft): dram bytes per template} from the newest committed `profiles/r*_traffic.csv`
+    (ncu dram__bytes_read.sum + dram__bytes_write.sum per launch / templates per launch)."""
+    pdir = os.path.join(ROOT, "profiles")
     try:
-        for line in open(path):
-            f = [c.strip() for c in line.split(",")]
-            if len(f) >= 4 and f[0] == cls and f[1].isdigit() and int(f[1]) == n_fft:
-                per_t = float(f[2]) + float(f[3])
-                return per_t * templates / max(launches, 1), "profiles/r01_traffic.csv (ncu --set full, per template x templates per launch)"
+        files = sorted(f for f in os.listdir(pdir) if f.endswith("_traffic.csv"))
     except OSError:
-        pass
-    return None, None
+        return {}, None
+    if not files:
+        return {}, None
+    tab = {}
+    for line in open(os.path.join(pdir, files[-1])):
+        f = [c.strip() for c in line.split(",")]
+        if len(f) >= 4 and f[1].isdigit():
+            tab[(f[0], int(f[1]))] = float(f[2]) + float(f[3])
+    return tab, "profiles/" + files[-1]
 
 
 def measured_peaks():
@@ -152,29 +166,79 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------
-# CPU oracle legs (the only places bench.py touches oracle/)
+# CPU oracle legs (the only places bench.py touches oracle/).  ONE protocol for `cpu_baseline` and for
+# `--impl reference`: the sky-dependent preparation once (one core; it is amortised over the bank exactly as the
+# GPU path amortises it), then a bounded sample of templates spread over all host cores by a process pool.
 # ------------------------------------------------------------------------------------------
-def oracle_step(p, n_templates: int):
-    """One bounded oracle sample: the sky-dependent work once, then n_templates templates."""
+_ORACLE_STATE = {}
+
+
+def _oracle_worker(i):
     from oracle import fstat_oracle as O
-    t0 = time.perf_counter()
-    sky = O.per_sky(p, float(p.templates[0, 0]), float(p.templates[0, 1]))
-    t1 = time.perf_counter()
-    for i in range(n_templates):
-        O.fstat_2F(p, p.templates[i], sky)
-    t2 = time.perf_counter()
-    return t1 - t0, (t2 - t1) / n_templates
+    p, sky = _ORACLE_STATE["p"], _ORACLE_STATE["sky"]
+    t = p.templates[i]
+    if sky is None or (float(t[0]), float(t[1])) != _ORACLE_STATE["sky_key"]:
+        return float(O.fstat_2F(p, t).max())           # sky-varying bank: the per-sky work belongs to the template
+    return float(O.fstat_2F(p, t, sky).max())
 
 
-def cpu_baseline(p, n_templates: int = 8):
-    t_sky, t_tmpl = oracle_step(p, n_templates)
-    n_groups = len({(float(a), float(d)) for a, d in p.templates[:, :2]})
-    n_t = len(p.templates)
-    full = n_groups * t_sky + n_t * t_tmpl             # extrapolated to the whole bank
-    return {"value": n_t * p.n_bins / full, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "templates_per_s": n_t / full,
-            "sample": f"numpy fp64 oracle, 1 sky preparation ({t_sky:.2f} s) + {n_templates} of {n_t} templates "
-                      f"({t_tmpl:.3f} s each), extrapolated to the bank ({n_groups} sky position(s))"}
+class OraclePool:
+    """Fork pool over the host cores; the problem and the per-sky cache are inherited copy-on-write.  Must be created
+    before CUDA is initialised in this process (fork)."""
+
+    def __init__(self, p):
+        import multiprocessing as mp
+        from oracle import fstat_oracle as O
+        self.p = p
+        self.cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+        groups = {(float(a), float(d)) for a, d in p.templates[:, :2]}
+        self.n_groups = len(groups)
+        self.sky_varying = self.n_groups > 1
+        t0 = time.perf_counter()
+        sky = O.per_sky(p, float(p.templates[0, 0]), float(p.templates[0, 1]))
+        self.t_sky = time.perf_counter() - t0
+        _ORACLE_STATE.update(p=p, sky=sky, sky_key=(float(p.templates[0, 0]), float(p.templates[0, 1])))
+        self.pool = mp.get_context("fork").Pool(self.cores)
+        self.pool.map(_oracle_worker, [0] * self.cores)             # start the workers (untimed)
+
+    def step(self, idxs):
+        """Wall seconds for the oracle to compute the 2F rows of templates idxs on all cores."""
+        t0 = time.perf_counter()
+        self.pool.map(_oracle_worker, list(idxs), chunksize=1)
+        return time.perf_counter() - t0
+
+    def sample_indices(self, per_core: int):
+        n_t = len(self.p.templates)
+        n = min(n_t, per_core * self.cores)
+        return [int(i) for i in np.linspace(0, n_t - 1, n).astype(int)]
+
+    def rate(self, idxs, t_pool: float):
+        """2F-bins/s and templates/s of the whole bank extrapolated from the sample: per-template pool time x
+        templates + one sky preparation per sky position (already inside the template cost for sky-varying banks)."""
+        n_t = len(self.p.templates)
+        full = n_t * t_pool / len(idxs) + (0.0 if self.sky_varying else self.n_groups * self.t_sky)
+        return n_t * self.p.n_bins / full, n_t / full
+
+    def describe(self, idxs, t_pool):
+        return (f"numpy fp64 oracle on {self.cores} cores (process pool over templates): 1 sky preparation "
+                f"({self.t_sky:.2f} s, one core) + {len(idxs)} of {len(self.p.templates)} templates in {t_pool:.2f} s wall, "
+                f"extrapolated to the bank ({self.n_groups} sky position(s))")
+
+    def close(self):
+        self.pool.close()
+        self.pool.join()
+
+
+def cpu_baseline(p, per_core: int = 2):
+    pool = OraclePool(p)
+    try:
+        idxs = pool.sample_indices(per_core)
+        t_pool = pool.step(idxs)
+        value, tps = pool.rate(idxs, t_pool)
+        return {"value": value, "unit": UNIT, "cores": pool.cores, "kind": "oracle", "templates_per_s": tps,
+                "sample": pool.describe(idxs, t_pool)}
+    finally:
+        pool.close()
 
 
 def run_reference(args):
@@ -182,130 +246,265 @@ def run_reference(args):
     if rank != 0:
         return
     p = make_workload(args.workload)
-    n_per_step = 2
-    times = []
-    for s in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        oracle_step(p, n_per_step)
-        dt = time.perf_counter() - t0
-        if s >= args.warmup:
-            times.append(dt)
-    ms = 1e3 * float(np.mean(times))
-    value = n_per_step * p.n_bins / (ms * 1e-3)
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_det": p.n_det, "n_samples": p.n_samples, "n_fft": p.n_fft,
-                       "n_bins": p.n_bins, "templates_per_step": n_per_step,
-                       "note": "CPU oracle (numpy fp64) on a bounded sample: one sky preparation + 2 templates per step"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                             "sample": f"{n_per_step} templates + 1 sky preparation per step"},
-            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
-    print(json.dumps(line))
+    pool = OraclePool(p)
+    try:
+        idxs = pool.sample_indices(1)                   # one template per core and step
+        times = []
+        for s in range(args.warmup + args.steps):
+            dt = pool.step(idxs)
+            if s >= args.warmup:
+                times.append(dt)
+        t_pool = float(np.mean(times))
+        value, tps = pool.rate(idxs, t_pool)
+        sample = pool.describe(idxs, t_pool) + f"; mean of {args.steps} steps"
+        line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * t_pool, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "templates_per_s": tps,
+                "config": {"workload": args.workload, "n_det": p.n_det, "n_samples": p.n_samples, "dt": p.dt, "n_fft": p.n_fft,
+                           "n_bins": p.n_bins, "n_templates": len(p.templates), "dterms": p.dterms,
+                           "templates_per_step": len(idxs),
+                           "note": "CPU oracle (numpy fp64) on a bounded sample per step; value = whole-bank rate extrapolated "
+                                   "from it with the sky preparation amortised over the bank as the GPU path does"},
+                "cpu_baseline": {"value": value, "unit": UNIT, "cores": pool.cores, "kind": "oracle", "sample": sample},
+                "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+    finally:
+        pool.close()
 
 
 # ------------------------------------------------------------------------------------------
 # Our arm
 # ------------------------------------------------------------------------------------------
-def run_ours(args):
+def time_bank(plan, p, steps, warmup, topk, k, flush, barrier=None, sampler=None):
+    """W warm-up steps, then K timed steps of the whole bank (CUDA events on the plan's stream, L2 flushed between
+    steps, per-kernel-class events inside the library).  Returns (per-step ms, class profile, launches, clocks)."""
     import torch
-    import torch.distributed as dist
-    from paper_2201_00451_b200.binding import FstatPlan
+    n_t, nb = len(p.templates), plan.n_bins
+    if topk:
+        out = (torch.empty((n_t, k), dtype=torch.float32, device="cuda"), torch.empty((n_t, k), dtype=torch.int32, device="cuda"))
+    else:
+        out = torch.empty((n_t, nb), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
 
+    def step():
+        if topk:
+            plan.compute_topk(p.templates, k, out=out)
+        else:
+            plan.compute(p.templates, out=out)
+
+    for _ in range(warmup):
+        step()
+    plan.sync()
+    plan.set_profile(True)
+    l0 = plan.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    if barrier:
+        barrier()
+    if sampler:
+        sampler.start()
+    t_wall0 = time.time()
+    for s in range(steps):
+        flush.zero_()
+        ev[s][0].record(stream)
+        step()
+        ev[s][1].record(stream)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    prof = plan.get_profile()
+    plan.set_profile(False)
+    launches = plan.launch_count() - l0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    del out
+    return step_ms, prof, launches, clocks
+
+
+def roofline_report(p, prof, total_ms, steps, n_t, world, traffic_tab, traffic_src, peak, peak_src):
+    """Roofline of the dominant FFT kernel and of the pair, on SURVEY.md 8(d)'s algorithmic bytes, plus the DRAM-only
+    view: which of those bytes are served by HBM and which by L2 (the resampled series S is re-read by every template
+    of a sky position out of L2), and the fraction of the measured HBM peak that the ncu-measured DRAM traffic makes."""
+    ab = algorithmic_bytes(p)
+    b1, b2 = ab["S_read"] + ab["T_write"], ab["T_read"] + ab["twoF_write"]
+    kernels = {}
+    single = prof["fft_single"][1] > 0
+    fused = prof["fused_sky_pass1"][1] > 0
+    classes = [("fft_single", b1 + b2 - ab["T_write"] - ab["T_read"])] if single else \
+        [("fused_sky_pass1" if fused else "fft_pass1", b1), ("fft_pass2", b2)]
+    for cls, bytes_per_t in classes:
+        ms, n = prof[cls]
+        kernels[cls] = {"ms_total": ms, "launches": n, "avg_launch_us": 1e3 * ms / max(n, 1),
+                        "algorithmic_bytes_per_template": bytes_per_t,
+                        "achieved_gbs": bytes_per_t * n_t * steps / (ms * 1e-3) / 1e9 if ms > 0 else None}
+    for cls in ("sky", "topk"):
+        kernels[cls] = {"ms_total": prof[cls][0], "launches": prof[cls][1]}
+    fft_ms = sum(prof[c][0] for c, _ in classes)
+    dom = max((c for c, _ in classes), key=lambda c: prof[c][0])
+    ach = kernels[dom]["achieved_gbs"]
+    # the pair always against B_2pass (SURVEY.md 8(d) convention), also when the intermediate never leaves the chip
+    pair = (b1 + b2) * n_t * steps / (fft_ms * 1e-3) / 1e9
+    flops = 2 * 5.0 * p.n_fft * float(np.log2(p.n_fft)) * n_t * steps
+    per_launch = n_t * steps / max(kernels[dom]["launches"], 1)
+    tr = traffic_tab.get((dom, p.n_fft))
+    dram_pair = None
+    if all((c, p.n_fft) in traffic_tab for c, _ in classes):
+        dram_pair = sum(traffic_tab[(c, p.n_fft)] for c, _ in classes)
+    n_groups = len({(float(a), float(d)) for a, d in p.templates[:, :2]})
+    s_from_hbm = ab["S_read"] * n_groups / n_t            # S is read from HBM once per sky position, then from L2
+    hbm_alg = s_from_hbm + (0 if single else ab["T_write"] + ab["T_read"]) + ab["twoF_write"]
+    return {"bound": "hbm", "kernel": dom + "_kernel", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": tr * per_launch if tr is not None else None,
+            "traffic_source": ((traffic_src or "") + " (ncu dram__bytes_read.sum + dram__bytes_write.sum per template x templates per launch)") if tr is not None else None,
+            "peak_source": peak_src,
+            "fft_pair_achieved": pair, "fft_pair_frac": pair / peak,
+            # which of the algorithmic bytes are HBM traffic and which are L2 hits (per template)
+            "algorithmic_bytes_per_template": {"total_B_2pass": b1 + b2, "hbm": hbm_alg, "l2_served_S_reread": ab["S_read"] - s_from_hbm,
+                                               "on_chip_T": (ab["T_write"] + ab["T_read"]) if single else 0},
+            "hbm_algorithmic_frac": hbm_alg * n_t * steps / (fft_ms * 1e-3) / 1e9 / peak,
+            # measured: ncu DRAM bytes of the FFT kernels per template / their CUDA-event time / measured peak
+            "dram_frac": dram_pair * n_t * steps / (fft_ms * 1e-3) / 1e9 / peak if dram_pair is not None else None,
+            "dram_bytes_per_template": dram_pair,
+            # SURVEY.md 8(d) R_min: compulsory traffic only (raw series in, 2F out) over the whole step
+            "r_min_frac": (8 * p.n_samples * p.n_det + 4 * p.n_bins) * n_t * steps / (total_ms * 1e-3) / 1e9 / peak,
+            "alu_tflops": flops / (fft_ms * 1e-3) / 1e12, "alu_peak_tflops": ALU_PEAK_TFLOPS,
+            "alu_frac": flops / (fft_ms * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+            "share_of_step": prof[dom][0] / total_ms if world == 1 else None}, kernels
+
+
+def cufft_variant(plan, p, ours_us_per_template):
+    """Comparison baseline only (north_star (3); "FFTs are computed using the cuFFT library"): the paper's
+    structure on this GPU -- the same resampled series S from our sky kernel, then separate library kernels per step:
+    spin-down phase factor, two cuFFT transforms (torch.fft.fft), the 2F map (torch expression).  Never on the product
+    path.  Returns timing per template and the agreement with fstat_compute on the same templates."""
+    import torch
+    al, de = float(p.templates[0, 0]), float(p.templates[0, 1])
+    S, abcd = plan.resample_sky(al, de)
+    ya = torch.complex(S[:, 0], S[:, 1]).contiguous()
+    yb = torch.complex(S[:, 2], S[:, 3]).contiguous()
+    A, B, C, D = [float(v) for v in abcd]
+    n_b = max(1, min(16, (1 << 26) // p.n_fft))
+    same_sky = [i for i in range(len(p.templates)) if float(p.templates[i, 0]) == al and float(p.templates[i, 1]) == de][:n_b]
+    tm = torch.tensor(p.templates[same_sky], dtype=torch.float64, device="cuda")
+    km = int(np.ceil(512.0 / p.dt))
+    tau = (torch.arange(p.n_fft, dtype=torch.float64, device="cuda") - km) * p.dt
+    nb = plan.n_bins
+
+    def path():
+        cyc = 0.5 * tm[:, 3:4] * tau * tau + tm[:, 4:5] * tau * tau * tau / 6.0            # [n_b, n_fft] fp64 cycles
+        ang = (-2.0 * np.pi) * (cyc - torch.floor(cyc)).to(torch.float32)
+        rot = torch.complex(torch.cos(ang), torch.sin(ang))
+        fa = torch.fft.fft(ya * rot)[:, :nb]
+        fb = torch.fft.fft(yb * rot)[:, :nb]
+        return (B * (fa.real ** 2 + fa.imag ** 2) + A * (fb.real ** 2 + fb.imag ** 2)
+                - 2.0 * C * (fa.real * fb.real + fa.imag * fb.imag)) / D
+
+    for _ in range(2):
+        ref = path()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        ref = path()
+    e1.record()
+    torch.cuda.synchronize()
+    us_path = 1e3 * e0.elapsed_time(e1) / 5 / len(same_sky)
+    x = (ya * 1.0).unsqueeze(0).repeat(2 * len(same_sky), 1)
+    for _ in range(2):
+        torch.fft.fft(x)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        torch.fft.fft(x)
+    e1.record()
+    torch.cuda.synchronize()
+    us_fft = 1e3 * e0.elapsed_time(e1) / 5 / len(same_sky)
+    ours = plan.compute(p.templates[same_sky])
+    plan.sync()
+    dev = float(((ours - ref).abs() / torch.clamp(ref, min=4.0)).max().item())
+    return {"us_per_template_cufft_path": us_path, "us_per_template_two_ffts_only": us_fft,
+            "ours_us_per_template_whole_path": ours_us_per_template,
+            "speedup_vs_cufft_path": us_path / ours_us_per_template,
+            "max_rel_dev_ours_vs_cufft_path": dev, "templates": len(same_sky),
+            "note": "comparison baseline only, never on the product path: our resampled series S, then torch ops per step "
+                    "(fp64 spin-down phase -> complex64 factor, two torch.fft.fft = cuFFT, 2F expression); the sky-dependent "
+                    "work is excluded from both sides' per-template figure"}
+
+
+def config3_block(args, flush, traffic_tab, peak):
+    """Bounded config-3 sweep carried by the default line: one cell per FFT length 2^15 .. 2^23 (256 fdot templates,
+    W warm-up + 3 timed steps each), with the pair / dominant-kernel / DRAM fractions per cell."""
+    from paper_2201_00451_b200.binding import FstatPlan
+    cells = []
+    for days, band in CONFIG3_SWEEP:
+        p = synth.config3(days, band)
+        with FstatPlan(p) as plan:
+            step_ms, prof, launches, _ = time_bank(plan, p, 3, max(3, args.warmup), False, 0, flush)
+        n_t = len(p.templates)
+        total_ms = float(sum(step_ms))
+        roof, kern = roofline_report(p, prof, total_ms, 3, n_t, 1, traffic_tab, None, peak, None)
+        cells.append({"days": days, "band_hz": band, "log2_n_fft": int(np.log2(p.n_fft)), "n_templates": n_t,
+                      "ms_per_step": total_ms / 3, "bins_per_s": n_t * p.n_bins / (total_ms / 3 * 1e-3),
+                      "pair_frac": roof["fft_pair_frac"], "dom_kernel": roof["kernel"], "dom_frac": roof["frac"],
+                      "hbm_algorithmic_frac": roof["hbm_algorithmic_frac"], "dram_frac": roof["dram_frac"],
+                      "launches_per_step": launches // 3,
+                      "class_ms_per_step": {c: prof[c][0] / 3 for c in prof if prof[c][1] > 0}})
+        del p
+    return {"cells": cells, "min_pair_frac": min(c["pair_frac"] for c in cells),
+            "min_pair_cell": min(cells, key=lambda c: c["pair_frac"])["log2_n_fft"],
+            "note": "config 3 (2 detectors, 50 % gaps, 256 fdot templates, full 2F output), one cell per FFT length; "
+                    "pair_frac = B_2pass / (FFT kernel time) / measured HBM peak (SURVEY.md 8(d) R_hbm)"}
+
+
+def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    p = make_workload(args.workload, rank)
+
+    # the oracle leg forks a process pool: before CUDA is initialised in this process
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(p, args.cpu_templates_per_core)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2201_00451_b200.binding import FstatPlan
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
+    nccl = None
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")               # the communicator lines go to stderr, stdout stays one JSON line
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        nccl = {"backend": "nccl", "version": ".".join(str(v) for v in torch.cuda.nccl.version()),
+                "collectives": "all_reduce(MAX) of the device time (1 per timed region); no data-path collective (replicas only)"}
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    p = make_workload(args.workload, rank)
     plan = FstatPlan(p)
     if args.inflight:
         plan.set_inflight(args.inflight)
+    if args.paths:
+        plan.debug_set_paths(*[int(v) for v in args.paths.split(",")])
     n_t, nb = len(p.templates), plan.n_bins
     topk = args.mode == "topk"
-    if topk:                      # config-4 style: only the k loudest bins of every template leave the GPU
-        out = (torch.empty((n_t, args.k), dtype=torch.float32, device="cuda"),
-               torch.empty((n_t, args.k), dtype=torch.int32, device="cuda"))
-    else:
-        out = torch.empty((n_t, nb), dtype=torch.float32, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    stream = torch.cuda.current_stream()
-
-    def step():
-        if topk:
-            plan.compute_topk(p.templates, args.k, out=out)
-        else:
-            plan.compute(p.templates, out=out)
-
-    for _ in range(args.warmup):
-        step()
-    plan.sync()
-    # ---- timed region: K steps, per-step CUDA events on the plan's stream, L2 flushed between steps
-    plan.set_profile(not args.no_kernel_events)
-    l0 = plan.launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    barrier()
-    sampler.start()
-    t_wall0 = time.time()
-    for s in range(args.steps):
-        flush.zero_()
-        ev[s][0].record(stream)
-        step()
-        ev[s][1].record(stream)
-    barrier()
-    t_wall1 = time.time()
-    clocks = sampler.stop(t_wall0, t_wall1)
-    prof = plan.get_profile() if not args.no_kernel_events else None
-    plan.set_profile(False)
-    launches = plan.launch_count() - l0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms, prof, launches, clocks = time_bank(plan, p, args.steps, args.warmup, topk, args.k, flush, barrier, ClockSampler(local))
     total_ms = float(sum(step_ms))
     value, ms_per_step = aggregate_ranks(total_ms, n_t * nb, args.steps, dist if world > 1 else None, "cuda")
     total_ms = ms_per_step * args.steps
 
-    # ---- roofline of the dominant kernel class (CUDA events inside the library, same timed steps)
-    roofline = None
-    kernels = None
-    if prof is not None:
-        b1, b2 = algorithmic_bytes(p)
-        peak, peak_src = measured_peaks()
-        per_launch_t = plan_inflight = None
-        kernels = {}
-        for cls, bytes_per_t in (("fft_pass1", b1), ("fft_pass2", b2)):
-            ms, n = prof[cls]
-            tot_bytes = bytes_per_t * n_t * args.steps
-            kernels[cls] = {"ms_total": ms, "launches": n, "avg_launch_us": 1e3 * ms / max(n, 1),
-                            "algorithmic_bytes_per_template": bytes_per_t,
-                            "achieved_gbs": tot_bytes / (ms * 1e-3) / 1e9 if ms > 0 else None}
-        kernels["sky"] = {"ms_total": prof["sky"][0], "launches": prof["sky"][1]}
-        kernels["topk"] = {"ms_total": prof["topk"][0], "launches": prof["topk"][1]}
-        dom = max(("fft_pass1", "fft_pass2"), key=lambda c: prof[c][0])
-        ach = kernels[dom]["achieved_gbs"]
-        both = (b1 + b2) * n_t * args.steps / ((prof["fft_pass1"][0] + prof["fft_pass2"][0]) * 1e-3) / 1e9
-        # fp32 work of the two FFTs of a template (2 x 5 N log2 N flop) against the plain-FMA peak
-        fft_ms = prof["fft_pass1"][0] + prof["fft_pass2"][0]
-        flops = 2 * 5.0 * p.n_fft * float(np.log2(p.n_fft)) * n_t * args.steps
-        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        traffic, traffic_src = ncu_traffic(dom, p.n_fft, kernels[dom]["launches"], n_t * args.steps)
-        roofline = {"bound": "hbm", "kernel": dom + "_kernel", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                    "fft_pair_achieved": both, "fft_pair_frac": both / peak,
-                    # SURVEY.md 8(d) R_min: compulsory traffic only (raw series in, 2F out) over the whole step
-                    "r_min_frac": (8 * p.n_samples * p.n_det + 4 * nb) * n_t * args.steps / (total_ms * 1e-3) / 1e9 / peak,
-                    "alu_tflops": flops / (fft_ms * 1e-3) / 1e12, "alu_peak_tflops": alu_peak,
-                    "alu_frac": flops / (fft_ms * 1e-3) / 1e12 / alu_peak,
-                    "share_of_step": prof[dom][0] / total_ms if world == 1 else None}
+    peak, peak_src = measured_peaks()
+    traffic_tab, traffic_src = ncu_traffic_table()
+    roofline, kernels = roofline_report(p, prof, total_ms, args.steps, n_t, world, traffic_tab, traffic_src or "", peak, peak_src)
 
     # ---- end to end through the host-buffer entry point (pinned host 2F, D2H inside the timed region)
     e2e = None
@@ -337,33 +536,23 @@ def run_ours(args):
         e2e = {"value": world * n_t * nb / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": n_e2e,
                "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(d2h),
                "api": api + "; the series is uploaded once by fstat_setup (PAPER.md:93) and is not part of a step"}
+        if not topk:
+            del host_out
 
-    # ---- context only: the library FFT alone (cuFFT through torch.fft) on the same shape: two batched complex64
-    # transforms of n_fft points per template, nothing else of the path (no resampling, phases or 2F)
     cufft = None
-    if args.cufft_compare and rank == 0:
-        nb_t = max(1, min(32, (1 << 28) // p.n_fft))
-        x = torch.randn((2 * nb_t, p.n_fft), dtype=torch.complex64, device="cuda")
-        for _ in range(3):
-            y = torch.fft.fft(x)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record()
-        for _ in range(10):
-            y = torch.fft.fft(x)
-        e1.record()
-        torch.cuda.synchronize()
-        us = 1e3 * e0.elapsed_time(e1) / 10 / nb_t
-        cufft = {"us_per_template_two_ffts": us, "ours_us_per_template_whole_path": 1e3 * ms_per_step / n_t,
-                 "note": "torch.fft.fft (cuFFT) on [2 x %d, %d] complex64, out of place; comparison baseline only, "
-                         "not on the product path" % (nb_t, p.n_fft)}
-        del x, y
+    if not args.no_cufft_compare and rank == 0:
+        fft_ms = sum(prof[c][0] for c in ("fft_pass1", "fft_pass2", "fused_sky_pass1", "fft_single"))
+        cufft = cufft_variant(plan, p, 1e3 * fft_ms / args.steps / n_t)
+    plan.close()
 
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(p, args.cpu_templates)
+    c3 = None
+    if rank == 0 and world == 1 and not args.no_config3 and args.workload == "config2":
+        del p.series
+        torch.cuda.empty_cache()
+        c3 = config3_block(args, flush, traffic_tab, peak)
 
     if rank == 0:
+        from paper_2201_00451_b200 import build as _b
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
@@ -375,9 +564,9 @@ def run_ours(args):
                            "l2": "256 MiB flush buffer written between timed steps; each step also writes "
                                  f"{n_t * nb * 4 / 1e9:.2f} GB of 2F (> L2)"},
                 "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
-                "cpu_baseline": cpu, "cufft_compare": cufft}
+                "config3": c3, "cpu_baseline": cpu, "cufft_compare": cufft, "nccl": nccl,
+                "library": {"path": os.path.relpath(_b.LIB_PATH, ROOT), "mtime": int(os.path.getmtime(_b.LIB_PATH))}}
         print(json.dumps(line))
-    plan.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -390,15 +579,21 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--paths", default="", help="fused_sky,single overrides for fstat_debug_set_paths (-1 auto, 0 off, 1 on)")
     ap.add_argument("--mode", default="full", choices=["full", "topk"])
     ap.add_argument("--k", type=int, default=8)
-    ap.add_argument("--cpu-templates", type=int, default=32)
+    ap.add_argument("--cpu-templates-per-core", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-kernel-events", action="store_true")
-    ap.add_argument("--cufft-compare", action="store_true")
+    ap.add_argument("--no-cufft-compare", action="store_true")
+    ap.add_argument("--no-config3", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started without torchrun: start the N ranks ourselves (one process per GPU, NCCL over NVLink for the one all_reduce)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -140,6 +140,32 @@ FSTAT_API int fstat_compute_topk(fstat_plan_t *plan, const fstat_template_t *tmp
 FSTAT_API int fstat_compute_threshold(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float threshold,
                             int32_t k, float *val_dev, int32_t *bin_dev, int32_t *count_dev);
 
+/* fstat_compute_accumulate -- the semi-coherent building block (section 6: "data ... partitioned into
+ * segments ..., each segment is searched using the F-statistic, and results from all segments are summed"): same path
+ * as fstat_compute, but 2F is ADDED to what twoF_dev holds, so that the plans of several data segments that share the
+ * bin grid (same f_min and df) sum into one array.
+ *  bin_offset_host  host int32[n_tmpl] or NULL (= all 0): this plan's bin q of template t is added to output bin
+ *                   q - bin_offset[t] (bins that fall outside the row add nothing).  A signal's frequency at this
+ *                   segment's reference time tau_ref = t_start differs from its frequency at the search's reference
+ *                   time by fdot * (t_start - t_ref) + ...; the caller rounds that to bins.  |offset| < n_bins.
+ *  twoF_dev         caller-owned DEVICE memory float32[n_tmpl][n_bins], read and written; the caller zeroes it before the
+ *                   first segment.  Calls on the same rows must be ordered on one stream. */
+FSTAT_API int fstat_compute_accumulate(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl,
+                             const int32_t *bin_offset_host, float *twoF_dev);
+
+/* fstat_compute_per_detector -- the single-detector statistics 2F_X next to the coherent one (the quantity the paper's
+ * accuracy tooling compares per detector; eq. 8 with the sums over detector X only):
+ *  twoF_dev   caller-owned DEVICE memory float32[n_det][n_tmpl][n_bins].
+ * A detector without valid data gives D_X <= 0: its rows are NaN and fstat_sync reports FSTAT_EDOM. */
+FSTAT_API int fstat_compute_per_detector(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_dev);
+
+/* fstat_select_topk / fstat_select_threshold -- the selection of fstat_compute_topk / fstat_compute_threshold applied to
+ * rows the caller already holds in DEVICE memory (float32[n_rows][n_bins] of this plan's bin layout), e.g. the summed 2F
+ * of a semi-coherent search (PAPER.md:325 with the retention of PAPER.md:307).  Same ordering, tie rule and outputs. */
+FSTAT_API int fstat_select_topk(fstat_plan_t *plan, const float *twoF_dev, int32_t n_rows, int32_t k, float *val_dev, int32_t *bin_dev);
+FSTAT_API int fstat_select_threshold(fstat_plan_t *plan, const float *twoF_dev, int32_t n_rows, float threshold, int32_t k,
+                           float *val_dev, int32_t *bin_dev, int32_t *count_dev);
+
 /* Host-buffer variants (the end-to-end entry points): outputs are HOST memory (pinned
  * memory makes the copies asynchronous and overlapped); they return after the data
  * has landed and report FSTAT_EDOM if a template had D <= 0. */
@@ -159,21 +185,8 @@ FSTAT_API int fstat_resample_sky(fstat_plan_t *plan, double alpha, double delta,
  * last sync had D <= 0 (its outputs are NaN), FSTAT_ECUDA on a device fault. */
 FSTAT_API int fstat_sync(fstat_plan_t *plan);
 
-/* Number of kernels this plan has launched since setup (for the bench's launch count). */
-FSTAT_API int fstat_launch_count(const fstat_plan_t *plan, int64_t *count);
-
-/* Tuning knob for experiments (0 = default): how many templates' FFT intermediates are
- * kept in flight; bounds the L2 / HBM footprint of the four-step FFT. */
-FSTAT_API int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight);
-
-/* Per-kernel-class device timing with CUDA events on the plan's stream (for the roofline
- * report).  While enabled, every group of launches of one class is bracketed by two events.
- * fstat_get_profile waits for the stream, writes the summed elapsed milliseconds and launch
- * counts since the last call into HOST ms[4], launches[4], and resets the record.
- * Classes: 0 = sky-dependent kernels (timing, resampling, antenna sums), 1 = FFT pass 1
- * (spin-down prologue + column FFTs), 2 = FFT pass 2 (row FFTs + 2F epilogue), 3 = top-k. */
-FSTAT_API int fstat_set_profile(fstat_plan_t *plan, int32_t enable);
-FSTAT_API int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launches);
+/* Measurement and experiment hooks (launch counter, per-kernel-class timing, launch-shape overrides) are declared in
+ * fstat_debug.h; nothing on the product path needs them. */
 
 FSTAT_API void fstat_destroy(fstat_plan_t *plan);
 

@@ -1,0 +1,54 @@
+/* fstat_debug.h -- measurement and experiment hooks of the B200 F-statistic library.
+ *
+ * Not part of the computation ABI (fstat.h): nothing here changes what is computed, only how the work is
+ * launched or what is recorded about it.  bench.py uses the launch counter and the per-class timing for its
+ * roofline report; the tests use the launch-shape overrides to reach every kernel variant
+ * and the multi-batch paths at small sizes.  Same conventions as fstat.h (FSTAT_OK or a negative FSTAT_E* code).
+ */
+#ifndef FSTAT_B200_DEBUG_H
+#define FSTAT_B200_DEBUG_H
+
+#include "fstat.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Number of kernels this plan has launched since setup (bench.py's `gpu_launches`). */
+FSTAT_API int fstat_launch_count(const fstat_plan_t *plan, int64_t *count);
+
+/* How many templates' four-step intermediates are kept in flight per launch (0 = default); bounds the
+ * L2 / HBM footprint of the FFT. */
+FSTAT_API int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight);
+
+/* Per-kernel-class device timing with CUDA events on the plan's stream (for the roofline report,
+ * SURVEY.md 8(d)).  While enabled, every group of launches of one class is bracketed by two events.
+ * fstat_get_profile waits for the stream, writes the summed elapsed milliseconds and launch counts since
+ * the last call into HOST ms[FSTAT_PROFILE_CLASSES], launches[FSTAT_PROFILE_CLASSES], and resets the record.
+ * Classes: 0 = sky-dependent kernels (timing, resampling), 1 = FFT pass 1 (spin-down prologue + column
+ * FFTs), 2 = FFT pass 2 (row FFTs + 2F epilogue), 3 = top-k, 4 = fused sky + pass 1 (sky-varying search),
+ * 5 = single-kernel FFT (small n_fft). */
+#define FSTAT_PROFILE_CLASSES 6
+FSTAT_API int fstat_set_profile(fstat_plan_t *plan, int32_t enable);
+FSTAT_API int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launches);
+
+/* Launch-shape override for experiments and tests: n_fft = 2^log_n1 x 2^log_n2 with pass 2 transforming
+ * 2^log_n2 points, tiles of 2^log_tile1 / 2^log_tile2 elements, p2_elems (16 or 32) register elements per
+ * pass-2 thread.  Any argument < 0 keeps the plan's default for that field.  FSTAT_ESIZE if no kernel is
+ * instantiated for the combination (the plan is left unchanged).  Results do not depend on the shape beyond
+ * fp32 rounding order. */
+FSTAT_API int fstat_debug_set_geometry(fstat_plan_t *plan, int32_t log_n2, int32_t log_tile1, int32_t log_tile2, int32_t p2_elems);
+
+/* Upper bound on the sky positions resampled per batch (default: 1 GB of resampled series); lets a test reach
+ * the multi-batch path with a handful of sky positions.  0 = default. */
+FSTAT_API int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slots);
+
+/* Which path serves sky-varying banks / small FFTs: -1 = automatic (default), 0 = off, 1 = forced where supported.
+ *   fused_sky : per-sky work (H1-H5) inside the FFT pass-1 prologue instead of the hoisted sky kernel + S buffer
+ *   single    : one kernel for both FFT passes with the intermediate kept on chip (n_fft <= 2^17) */
+FSTAT_API int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSTAT_B200_DEBUG_H */

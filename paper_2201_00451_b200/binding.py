@@ -19,8 +19,11 @@ FSTAT_OK, FSTAT_EINVAL, FSTAT_ESIZE, FSTAT_EDOM, FSTAT_ECUDA, FSTAT_ENOMEM = 0, 
 
 EXPORTS = [
     "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_threshold", "fstat_compute_host",
-    "fstat_compute_topk_host", "fstat_resample_sky", "fstat_sync", "fstat_launch_count",
-    "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile", "fstat_destroy", "fstat_strerror", "fstat_last_error",
+    "fstat_compute_topk_host", "fstat_compute_accumulate", "fstat_compute_per_detector", "fstat_select_topk",
+    "fstat_select_threshold", "fstat_resample_sky", "fstat_sync", "fstat_destroy", "fstat_strerror", "fstat_last_error",
+    # include/fstat_debug.h: measurement / experiment hooks
+    "fstat_launch_count", "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile",
+    "fstat_debug_set_geometry", "fstat_debug_set_max_sky_slots", "fstat_debug_set_paths",
 ]
 
 
@@ -50,11 +53,11 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         return _lib
     path = _build.LIB_PATH
     if build_if_missing and _build.is_stale():
-        try:
-            _build.build_library()
-        except Exception:
-            if not os.path.exists(path):
-                raise
+        if _build.have_nvcc():
+            _build.build_library()             # a compile error must surface, never run stale kernels silently
+        elif os.path.exists(path):
+            import warnings
+            warnings.warn(f"{path} is older than its sources and nvcc is not available: loading the stale binary")
     if not os.path.exists(path):
         raise FileNotFoundError(f"{path} not built: run `python -m paper_2201_00451_b200.build`")
     lib = C.CDLL(path)
@@ -75,6 +78,14 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_compute_host.argtypes = [vp, vp, i32, vp]
     lib.fstat_compute_topk_host.restype = C.c_int
     lib.fstat_compute_topk_host.argtypes = [vp, vp, i32, i32, vp, vp]
+    lib.fstat_compute_accumulate.restype = C.c_int
+    lib.fstat_compute_accumulate.argtypes = [vp, vp, i32, vp, vp]
+    lib.fstat_compute_per_detector.restype = C.c_int
+    lib.fstat_compute_per_detector.argtypes = [vp, vp, i32, vp]
+    lib.fstat_select_topk.restype = C.c_int
+    lib.fstat_select_topk.argtypes = [vp, vp, i32, i32, vp, vp]
+    lib.fstat_select_threshold.restype = C.c_int
+    lib.fstat_select_threshold.argtypes = [vp, vp, i32, C.c_float, i32, vp, vp, vp]
     lib.fstat_resample_sky.restype = C.c_int
     lib.fstat_resample_sky.argtypes = [vp, dbl, dbl, vp, C.POINTER(dbl)]
     lib.fstat_sync.restype = C.c_int
@@ -87,6 +98,12 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_set_profile.argtypes = [vp, i32]
     lib.fstat_get_profile.restype = C.c_int
     lib.fstat_get_profile.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+    lib.fstat_debug_set_geometry.restype = C.c_int
+    lib.fstat_debug_set_geometry.argtypes = [vp, i32, i32, i32, i32]
+    lib.fstat_debug_set_max_sky_slots.restype = C.c_int
+    lib.fstat_debug_set_max_sky_slots.argtypes = [vp, i32]
+    lib.fstat_debug_set_paths.restype = C.c_int
+    lib.fstat_debug_set_paths.argtypes = [vp, i32, i32]
     lib.fstat_destroy.restype = None
     lib.fstat_destroy.argtypes = [vp]
     lib.fstat_strerror.restype = C.c_char_p
@@ -199,6 +216,45 @@ class FstatPlan:
                                                      val.data_ptr(), idx.data_ptr(), cnt.data_ptr()))
         return val, idx, cnt
 
+    def compute_accumulate(self, templates, out, bin_offsets=None):
+        """fstat_compute_accumulate: out[t][q - off_t] += 2F_t[q] (semi-coherent sum over segment plans)."""
+        t = _templates_array(templates)
+        torch = self._torch
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.numel() == t.shape[0] * self.n_bins
+        off = None if bin_offsets is None else np.ascontiguousarray(bin_offsets, dtype=np.int32)
+        assert off is None or off.shape == (t.shape[0],)
+        self._check(self.lib.fstat_compute_accumulate(self.handle, t.ctypes.data, t.shape[0],
+                                                      None if off is None else off.ctypes.data, out.data_ptr()))
+        return out
+
+    def compute_per_detector(self, templates, out=None):
+        """fstat_compute_per_detector: 2F_X[n_det][n_tmpl][n_bins] device tensor."""
+        t = _templates_array(templates)
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.prob.n_det, t.shape[0], self.n_bins), dtype=torch.float32, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+        self._check(self.lib.fstat_compute_per_detector(self.handle, t.ctypes.data, t.shape[0], out.data_ptr()))
+        return out
+
+    def select_topk(self, rows, k: int):
+        torch = self._torch
+        assert rows.is_cuda and rows.dtype == torch.float32 and rows.is_contiguous() and rows.shape[1] == self.n_bins
+        val = torch.empty((rows.shape[0], k), dtype=torch.float32, device="cuda")
+        idx = torch.empty((rows.shape[0], k), dtype=torch.int32, device="cuda")
+        self._check(self.lib.fstat_select_topk(self.handle, rows.data_ptr(), rows.shape[0], k, val.data_ptr(), idx.data_ptr()))
+        return val, idx
+
+    def select_threshold(self, rows, threshold: float, k: int):
+        torch = self._torch
+        assert rows.is_cuda and rows.dtype == torch.float32 and rows.is_contiguous() and rows.shape[1] == self.n_bins
+        val = torch.empty((rows.shape[0], k), dtype=torch.float32, device="cuda")
+        idx = torch.empty((rows.shape[0], k), dtype=torch.int32, device="cuda")
+        cnt = torch.empty((rows.shape[0],), dtype=torch.int32, device="cuda")
+        self._check(self.lib.fstat_select_threshold(self.handle, rows.data_ptr(), rows.shape[0], float(threshold), k,
+                                                    val.data_ptr(), idx.data_ptr(), cnt.data_ptr()))
+        return val, idx, cnt
+
     def compute_host(self, templates, out=None):
         """fstat_compute_host: 2F rows land in HOST memory (pinned torch tensor by default)."""
         t = _templates_array(templates)
@@ -231,17 +287,26 @@ class FstatPlan:
         self._check(self.lib.fstat_launch_count(self.handle, C.byref(n)))
         return int(n.value)
 
-    PROFILE_CLASSES = ("sky", "fft_pass1", "fft_pass2", "topk")
+    PROFILE_CLASSES = ("sky", "fft_pass1", "fft_pass2", "topk", "fused_sky_pass1", "fft_single")
 
     def set_profile(self, enable: bool):
         self._check(self.lib.fstat_set_profile(self.handle, 1 if enable else 0))
 
     def get_profile(self):
         """{class: (milliseconds, launches)} since the last call."""
-        ms = (C.c_double * 4)()
-        n = (C.c_int64 * 4)()
+        ms = (C.c_double * len(self.PROFILE_CLASSES))()
+        n = (C.c_int64 * len(self.PROFILE_CLASSES))()
         self._check(self.lib.fstat_get_profile(self.handle, ms, n))
         return {c: (float(ms[i]), int(n[i])) for i, c in enumerate(self.PROFILE_CLASSES)}
 
     def set_inflight(self, n: int):
         self._check(self.lib.fstat_set_inflight(self.handle, n))
+
+    def debug_set_geometry(self, log_n2: int = -1, log_tile1: int = -1, log_tile2: int = -1, p2_elems: int = -1):
+        self._check(self.lib.fstat_debug_set_geometry(self.handle, log_n2, log_tile1, log_tile2, p2_elems))
+
+    def debug_set_max_sky_slots(self, n: int):
+        self._check(self.lib.fstat_debug_set_max_sky_slots(self.handle, n))
+
+    def debug_set_paths(self, fused_sky: int = -1, single: int = -1):
+        self._check(self.lib.fstat_debug_set_paths(self.handle, fused_sky, single))

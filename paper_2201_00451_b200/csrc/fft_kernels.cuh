@@ -15,6 +15,7 @@
 // twiddle / 2F epilogue and the global stores of the current tile execute.
 #pragma once
 #include "fstat_common.cuh"
+#include "fft_launch.cuh"
 
 // Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
 // a register pair holds (Re Fa, Re Fb) or (Im Fa, Im Fb) and every add / multiply / FMA is one
@@ -199,23 +200,6 @@ __device__ __forceinline__ void pass_load_smem(float2 (&a)[E], float2 (&b)[E], c
     }
 }
 
-
-struct FftArgs {
-    const float4 *S;          // [n_sky_slots][n_fft] resampled series, tile-blocked: [k2/W1][k1][k2%W1]
-    float4 *T;                // [templates of this launch][n_fft] intermediate, tile-blocked: [m1/W2][k2][m1%W2]
-    const TmplDesc *tmpl;     // descriptors of the templates of this launch
-    const SkyABCD *abcd;      // [n_sky_slots]
-    float *twoF;              // output rows of this launch
-    uint32_t *gmax;           // top-k mode: [tile][warp] maximum (as topk_key) of the 512 bins each warp of pass 2 writes; else null
-    int64_t twoF_stride;      // floats between rows
-    const float2 *tw;         // twiddle table of this sub-FFT length
-    int64_t n_fft, n_src, n_bins, k_margin;
-    double dt;
-    int log_other;            // log2 of the other factor (N2 for pass 1, N1 for pass 2)
-    int log_w_other;          // log2 W of the other pass (layout of T)
-    int log_tiles;            // log2(tiles per template) = log_other - LOGW
-    int n_tiles;              // tiles per template * templates in this launch
-};
 
 // exp(-2 pi i x) for a phase x in cycles held in fp64: reduce mod 1 in fp64, sincospif in fp32.
 __device__ __forceinline__ float2 expm2pi(double cyc) {
@@ -460,15 +444,16 @@ __global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, 
 fft_pass2_kernel(const __grid_constant__ FftArgs p) {
     FFT_KERNEL_PREAMBLE(E);
     const uint64_t pol_T = l2_policy_evict_first();
-    int sky_next = p.tmpl[tile >> p.log_tiles].sky_slot;
+    int2 tm_next = *reinterpret_cast<const int2 *>(&p.tmpl[tile >> p.log_tiles].sky_slot);      // (sky_slot, bin_off)
     tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_T);
     for (; tile < p.n_tiles; tile += gridDim.x) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const int m1_0 = x << LOGW;
         const int nxt = tile + gridDim.x;
-        const SkyABCD *abp = p.abcd + sky_next;
+        const SkyABCD *abp = p.abcd + tm_next.x;
+        const int boff = tm_next.y;
         const float b_over_d = abp->b_over_d, a_over_d = abp->a_over_d, two_c_over_d = abp->two_c_over_d;
-        if (nxt < p.n_tiles) sky_next = p.tmpl[nxt >> p.log_tiles].sky_slot;
+        if (nxt < p.n_tiles) tm_next = *reinterpret_cast<const int2 *>(&p.tmpl[nxt >> p.log_tiles].sky_slot);
         mbar_wait(bar, parity);
         parity ^= 1;
         tile_take_inputs<LOGN, LOGT>(a, b, sm);
@@ -480,9 +465,14 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
             constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
             using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
-            float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride;
+            // bin q of this template goes to output bin q - boff (boff != 0 only in accumulate mode: the track of one
+            // signal through segments with different reference times); q in [lo, lo + span) lands inside the row
+            float *__restrict__ out = p.twoF + (int64_t)t * p.twoF_stride - boff;
             float tmax = __int_as_float(0xff800000);
             const int nb = (int)p.n_bins;                       // bins fit 32 bits (n_fft <= 2^24)
+            const int lo = max(0, boff);
+            const unsigned span = (unsigned)max(0, min(nb, nb + boff) - lo);
+            const bool acc = p.accumulate != 0;
             const int q_step = PL << p.log_other;               // out_idx(i, r) is linear in r with slope P
 #pragma unroll
             for (int bb = 0; bb < PI::NB; ++bb) {
@@ -491,11 +481,12 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
                 int q = (PI::out_idx(i, 0) << p.log_other) + m1_0 + w;
 #pragma unroll
                 for (int r = 0; r < RL; ++r, q += q_step) {
-                    if (q < nb) {
+                    if ((unsigned)(q - lo) < span) {
                         const float2 fa = make_float2(a[bb * RL + r].x, b[bb * RL + r].x);    // unpack (re, im) of Fa, Fb
                         const float2 fb = make_float2(a[bb * RL + r].y, b[bb * RL + r].y);
-                        const float twoF = b_over_d * (fa.x * fa.x + fa.y * fa.y) + a_over_d * (fb.x * fb.x + fb.y * fb.y)
-                                         - two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
+                        float twoF = b_over_d * (fa.x * fa.x + fa.y * fa.y) + a_over_d * (fb.x * fb.x + fb.y * fb.y)
+                                   - two_c_over_d * (fa.x * fb.x + fa.y * fb.y);
+                        if (acc) twoF += __ldcs(out + q);
                         __stcs(out + q, twoF);
                         tmax = fmaxf(tmax, twoF);
                     }
@@ -507,4 +498,11 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
             }
         }
     }
+}
+
+// kernel pointer by (sub-FFT, tile, pass, elements, padding variant)
+template <int LOGN, int LOGT, bool P2, int E, bool SKIPZ>
+inline void (*fft_kernel_ptr())(const FftArgs) {
+    if constexpr (P2) return fft_pass2_kernel<LOGN, LOGT, E>;
+    else return fft_pass1_kernel<LOGN, LOGT, E, SKIPZ>;
 }

@@ -1,0 +1,63 @@
+// One translation unit of FFT pass kernel instantiations (compiled once per -DFFT_UNIT=0..5; see fft_launch.cuh).
+#include "fft_kernels.cuh"
+#include "fft_launch.cuh"
+
+#ifndef FFT_UNIT
+#error "compile with -DFFT_UNIT=<0..5>"
+#endif
+
+namespace {
+
+template <int LOGN, int LOGT, bool P2, int E, bool SKIPZ>
+cudaError_t launch_pass(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, int n_t) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    constexpr int SMEM = C::SMEM_BYTES;
+    static thread_local int configured_dev = -1;
+    static thread_local int resident = 0;
+    auto kern = fft_kernel_ptr<LOGN, LOGT, P2, E, SKIPZ>();
+    if (configured_dev != ctx.device) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (e != cudaSuccess) return e;
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, SMEM);
+        if (e != cudaSuccess) return e;
+        resident = (per_sm > 0 ? per_sm : 1) * ctx.n_sm;
+        configured_dev = ctx.device;
+    }
+    int lt = 0;
+    while ((1 << lt) < tiles_per_tmpl) ++lt;
+    a.log_tiles = lt;
+    a.n_tiles = tiles_per_tmpl * n_t;
+    const int grid = a.n_tiles < resident ? a.n_tiles : resident;
+    kern<<<grid, C::NT, SMEM, ctx.stream>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+#define FFT_CAT2(a, b) a##b
+#define FFT_CAT(a, b) FFT_CAT2(a, b)
+#define K(P, LN, LT, E, Z) if (pass == P && logn == LN && logt == LT && elems == E && skipz == Z) return launch_pass<LN, LT, (P == 2), E, (Z != 0)>;
+
+fft_launch_fn FFT_CAT(fft_find_kernel_unit, FFT_UNIT)(int pass, int logn, int logt, int elems, int skipz) {
+#if FFT_UNIT == 0      // pass 1, sub-FFT 2^6 .. 2^9
+    K(1, 6, 11, 16, 0) K(1, 7, 11, 16, 0) K(1, 8, 11, 16, 0) K(1, 9, 11, 16, 0)
+    K(1, 6, 12, 16, 0) K(1, 7, 12, 16, 0) K(1, 8, 12, 16, 0) K(1, 9, 12, 16, 0)
+#elif FFT_UNIT == 1    // pass 1, sub-FFT 2^10, 2^11
+    K(1, 10, 11, 16, 0) K(1, 10, 12, 16, 0) K(1, 10, 13, 16, 0) K(1, 10, 11, 16, 1)
+    K(1, 11, 11, 16, 0) K(1, 11, 12, 16, 0) K(1, 11, 13, 16, 0) K(1, 11, 11, 16, 1) K(1, 11, 12, 16, 1)
+#elif FFT_UNIT == 2    // pass 1, sub-FFT 2^12
+    K(1, 12, 12, 16, 0) K(1, 12, 13, 16, 0) K(1, 12, 12, 16, 1) K(1, 12, 13, 16, 1)
+#elif FFT_UNIT == 3    // pass 2, sub-FFT 2^6 .. 2^9
+    K(2, 6, 11, 16, 0) K(2, 7, 11, 16, 0) K(2, 8, 11, 16, 0) K(2, 9, 11, 16, 0)
+    K(2, 6, 12, 16, 0) K(2, 7, 12, 16, 0) K(2, 8, 12, 16, 0) K(2, 9, 12, 16, 0) K(2, 9, 12, 32, 0)
+#elif FFT_UNIT == 4    // pass 2, sub-FFT 2^10, 2^11
+    K(2, 10, 11, 16, 0) K(2, 10, 12, 16, 0) K(2, 10, 13, 16, 0) K(2, 10, 12, 32, 0) K(2, 10, 13, 32, 0)
+    K(2, 11, 11, 16, 0) K(2, 11, 12, 16, 0) K(2, 11, 13, 16, 0)
+#elif FFT_UNIT == 5    // pass 2, sub-FFT 2^12
+    K(2, 12, 12, 16, 0) K(2, 12, 13, 16, 0)
+#endif
+    return nullptr;
+}

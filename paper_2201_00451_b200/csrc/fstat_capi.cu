@@ -2,9 +2,10 @@
 // kernel orchestration.  All arithmetic of the path runs in the kernels of sky_kernels.cuh,
 // fft_kernels.cuh and topk_kernels.cuh; the host only derives O(n_det) per-sky constants.
 #include "../../include/fstat.h"
+#include "../../include/fstat_debug.h"
 #include "fstat_common.cuh"
 #include "sky_kernels.cuh"
-#include "fft_kernels.cuh"
+#include "fft_launch.cuh"
 #include "topk_kernels.cuh"
 
 #include <cmath>
@@ -53,9 +54,11 @@ struct fstat_plan {
     SkyABCD *d_abcd = nullptr; SkyABCD *h_abcd = nullptr;   // per sky group of the current call (capacity sky_cap)
     double mom[FSTAT_MAX_DET][MOM_TERMS];                   // antenna moment matrices M_X (sky_kernels.cuh)
     bool pending_edom = false;                              // a template since the last sync had D <= 0
+    int force_fused_sky = -1, force_single = -1;            // fstat_debug_set_paths
     TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
     float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
     uint32_t *d_gmax = nullptr;       // top-k: per-group maxima of the rows in flight [n_inflight][n_groups]
+    uint32_t *d_gmax_lin = nullptr;   // fstat_select_*: per-group maxima of caller rows (linear groups)
     HostRing ring;
     float *d_topk_v = nullptr; int *d_topk_i = nullptr; size_t topk_cap = 0;
     // pinned staging
@@ -197,10 +200,11 @@ void fill_sky_const(const fstat_plan *p, double alpha, double delta, SkyConst *s
 
 // A, B, C, D of one sky position from the moment matrices: A = sum_X alpha_X^T M_X alpha_X etc., with
 // alpha_X, beta_X the coefficients of a_X(t), b_X(t) in the basis (1, cos 2th, sin 2th, cos th, sin th).
-void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
+void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out, uint32_t det_mask = 0xffffffffu) {
     double A = 0, B = 0, C = 0;
     const double C1 = cos(alpha), S1 = sin(alpha), C2 = cos(2 * alpha), S2 = sin(2 * alpha);
     for (int X = 0; X < p->g.n_det; ++X) {
+        if (!((det_mask >> X) & 1u)) continue;
         const fstat_detector_t &d = p->det[X];
         const double lam = d.lat_rad, gam = d.xarm_azimuth_rad + 0.75 * M_PI;
         const double s2g = sin(2 * gam), c2g = cos(2 * gam);
@@ -236,55 +240,54 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out) {
     }
 }
 
-// Persistent launch: grid = min(n_tiles, resident CTAs on the whole GPU).
-template <int LOGN, int LOGT, bool P2, int E = 16, bool SKIPZ = false> int launch_pass(fstat_plan *p, FftArgs &a, int tiles_per_tmpl, int n_t) {
-    using C = FftCfg<LOGN, LOGT, E>;
-    constexpr int SMEM = C::SMEM_BYTES;
-    static thread_local int configured_dev = -1;
-    static thread_local int resident = 0;
-    auto kern = P2 ? fft_pass2_kernel<LOGN, LOGT, E> : fft_pass1_kernel<LOGN, LOGT, E, SKIPZ>;
-    if (configured_dev != p->device) {
-        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
-        CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        int per_sm = 0;
-        CUDA_TRY(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::NT, SMEM));
-        resident = (per_sm > 0 ? per_sm : 1) * p->n_sm;
-        configured_dev = p->device;
-    }
-    a.log_tiles = ilog2(tiles_per_tmpl);
-    a.n_tiles = tiles_per_tmpl * n_t;
-    const int grid = a.n_tiles < resident ? a.n_tiles : resident;
-    kern<<<grid, C::NT, SMEM, p->stream>>>(a);
-    ++p->launches;
+// n_fft = 2^log_n1 x 2^log_n2 and the tile sizes of the two FFT passes, per size as measured on B200
+// (DESIGN.md 5 "How n_fft is split").  Pass 2 gets the shorter transform: its tile then spans more rows, which is what
+// makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
+// 2^11-element tiles.
+void default_geometry(int L, PlanGeom &g) {
+    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10 : L == 22 ? 10 : L - 12;
+    g.log_n1 = L - g.log_n2;
+    // pass 2: 2^12-element tiles; 2^13 (8 rows of 2^10 points: 128-byte runs in pass 1's transposed store, 32-byte
+    // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2; likewise 4 rows
+    // of 2^11 points at 2^23, which lets pass 1 run one 2^12-point column per 2^12-element tile
+    g.log_tile2 = (g.log_n2 == 12 || (g.log_n2 == 10 && L >= 21) || (g.log_n2 == 11 && L == 23)) ? 13 : 12;
+    // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
+    // of a single column needs >= 4 rows per pass-2 tile
+    const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
+    g.log_tile1 = g.log_n1 <= 10 ? 11 : (w2_rows >= 4 ? g.log_n1 : g.log_n1 + 1);
+    // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
+    // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles
+    g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
+    g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
+}
+
+// columns that are at least half zero padding take the pass-1 variant that neither stages nor touches the padding
+// (where one is instantiated)
+int pass1_skipz(const PlanGeom &g) {
+    return (2 * g.n_src <= g.n_fft && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, 1)) ? 1 : 0;
+}
+bool geometry_supported(const PlanGeom &g) {
+    return fft_find_kernel(1, g.log_n1, g.log_tile1, 16, 0) && fft_find_kernel(2, g.log_n2, g.log_tile2, g.p2_elems, 0);
+}
+
+// (re)upload the Stockham twiddle tables of the plan's current geometry
+int upload_twiddles(fstat_plan *p) {
+    const std::vector<float2> tw1 = make_twiddles(p->g.log_n1), tw2 = make_twiddles(p->g.log_n2, p->g.p2_elems);
+    cudaFree(p->d_tw1); cudaFree(p->d_tw2); p->d_tw1 = p->d_tw2 = nullptr;
+    CUDA_TRY(p, cudaMalloc(&p->d_tw1, tw1.size() * sizeof(float2)));
+    CUDA_TRY(p, cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));      // the host vectors go out of scope
     return FSTAT_OK;
 }
-#define DISPATCH_TILE(logn, logt, P2, ...)                                                        \
-    switch ((logn) * 16 + (logt)) {                                                              \
-        case 6 * 16 + 11: rc = launch_pass<6, 11, P2>(__VA_ARGS__); break;                       \
-        case 7 * 16 + 11: rc = launch_pass<7, 11, P2>(__VA_ARGS__); break;                       \
-        case 8 * 16 + 11: rc = launch_pass<8, 11, P2>(__VA_ARGS__); break;                       \
-        case 9 * 16 + 11: rc = launch_pass<9, 11, P2>(__VA_ARGS__); break;                       \
-        case 10 * 16 + 11: rc = launch_pass<10, 11, P2>(__VA_ARGS__); break;                     \
-        case 11 * 16 + 11: rc = launch_pass<11, 11, P2>(__VA_ARGS__); break;                     \
-        case 6 * 16 + 12: rc = launch_pass<6, 12, P2>(__VA_ARGS__); break;                       \
-        case 7 * 16 + 12: rc = launch_pass<7, 12, P2>(__VA_ARGS__); break;                       \
-        case 8 * 16 + 12: rc = launch_pass<8, 12, P2>(__VA_ARGS__); break;                       \
-        case 9 * 16 + 12: rc = launch_pass<9, 12, P2>(__VA_ARGS__); break;                       \
-        case 10 * 16 + 12: rc = launch_pass<10, 12, P2>(__VA_ARGS__); break;                     \
-        case 11 * 16 + 12: rc = launch_pass<11, 12, P2>(__VA_ARGS__); break;                     \
-        case 12 * 16 + 13: rc = launch_pass<12, 13, P2>(__VA_ARGS__); break;                     \
-        case 12 * 16 + 12: rc = launch_pass<12, 12, P2>(__VA_ARGS__); break;                     \
-        case 11 * 16 + 13: rc = launch_pass<11, 13, P2>(__VA_ARGS__); break;                     \
-        case 10 * 16 + 13: rc = launch_pass<10, 13, P2>(__VA_ARGS__); break;                     \
-        default: rc = fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination"); break;    \
-    }
 
 // log2 of the tile size used for a sub-FFT of length 2^logn under the plan's tile setting
 int tile_log1(const fstat_plan *p) { return p->g.log_tile1; }
 int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
-int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr) {
+int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr, bool accumulate = false) {
     if (nt > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         cudaFree(p->d_T); p->d_T = nullptr; p->t_cap = 0;
@@ -293,45 +296,39 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     }
     FftArgs a{};
     a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd + g0;
-    a.twoF = rows; a.twoF_stride = row_stride; a.gmax = gmax;
+    a.twoF = rows; a.twoF_stride = row_stride; a.gmax = gmax; a.accumulate = accumulate ? 1 : 0;
     a.n_fft = p->g.n_fft; a.n_src = p->g.n_src; a.n_bins = p->g.n_bins; a.k_margin = p->g.k_margin;
     a.dt = p->g.dt;
-    int rc = FSTAT_OK;
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
+    const LaunchCtx ctx{p->stream, p->device, p->n_sm};
     a.tw = p->d_tw1; a.log_other = l2; a.log_w_other = p->g.log_w2;
     {
         ProfScope ps(p, 1);
-        const int tiles1 = 1 << (l2 - p->g.log_w1), lt1 = tile_log1(p);
-        // columns that are at least half zero padding: the variant that neither stages nor touches the padding
-        const bool skipz = 2 * p->g.n_src <= p->g.n_fft;
-        if (skipz && l1 == 12 && lt1 == 12) rc = launch_pass<12, 12, false, 16, true>(p, a, tiles1, nt);
-        else if (skipz && l1 == 12 && lt1 == 13) rc = launch_pass<12, 13, false, 16, true>(p, a, tiles1, nt);
-        else if (skipz && l1 == 11 && lt1 == 11) rc = launch_pass<11, 11, false, 16, true>(p, a, tiles1, nt);
-        else if (skipz && l1 == 11 && lt1 == 12) rc = launch_pass<11, 12, false, 16, true>(p, a, tiles1, nt);
-        else if (skipz && l1 == 10 && lt1 == 11) rc = launch_pass<10, 11, false, 16, true>(p, a, tiles1, nt);
-        else DISPATCH_TILE(l1, lt1, false, p, a, tiles1, nt);
+        const int tiles1 = 1 << (l2 - p->g.log_w1);
+        const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, 16, pass1_skipz(p->g));
+        if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
+        CUDA_TRY(p, f(ctx, a, tiles1, nt));
+        ++p->launches;
     }
-    if (rc) return rc;
     a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
     {
         ProfScope ps(p, 2);
         const int tiles2 = 1 << (l1 - p->g.log_w2);
-        if (p->g.p2_elems == 32 && l2 == 10 && tile_log2(p) == 13) rc = launch_pass<10, 13, true, 32>(p, a, tiles2, nt);
-        else if (p->g.p2_elems == 32 && l2 == 10) rc = launch_pass<10, 12, true, 32>(p, a, tiles2, nt);
-        else if (p->g.p2_elems == 32 && l2 == 9) rc = launch_pass<9, 12, true, 32>(p, a, tiles2, nt);
-        else DISPATCH_TILE(l2, tile_log2(p), true, p, a, tiles2, nt);
+        const fft_launch_fn f = fft_find_kernel(2, l2, p->g.log_tile2, p->g.p2_elems, 0);
+        if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 2");
+        CUDA_TRY(p, f(ctx, a, tiles2, nt));
+        ++p->launches;
     }
-    if (rc) return rc;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
 }
 
 // Sky-dependent kernel for sky groups [g0, g0+ng) -> S slots 0..ng-1.
-int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked) {
+int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked, uint32_t det_mask = 0xffffffffu) {
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
     dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
-    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_base, p->d_farrow, p->d_wslot, S_dst, blocked);
+    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_base, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -374,6 +371,9 @@ struct OutSpec {
     int32_t *bin = nullptr;
     float thr = 0.f;             // threshold mode (count != null): only bins with 2F > thr
     int32_t *count = nullptr;    // device [n_tmpl]
+    bool accumulate = false;     // OUT_DEV_ROWS: rows += 2F (semi-coherent sum)
+    const int32_t *bin_off = nullptr;   // accumulate: host [n_tmpl] bin offsets (null = 0)
+    uint32_t det_mask = 0xffffffffu;    // detectors that take part
 };
 
 // groups of 512 bins (one warp of a pass-2 tile each) per row, and how pass 2 maps them to bins
@@ -389,6 +389,7 @@ TopkGeom topk_geom(const fstat_plan *p) {
     for (size_t i = 0; i + 1 < rl.size(); ++i) tg.pl *= rl[i];
     tg.log_other = p->g.log_n1;
     tg.n_groups = (int)(p->g.n_fft >> lt) * (tg.nt / 32);
+    tg.linear = 0;
     return tg;
 }
 
@@ -398,7 +399,9 @@ int ensure_topk_scratch(fstat_plan *p) {
     if (!p->d_gmax) {
         const TopkGeom tg = topk_geom(p);
         CUDA_TRY(p, cudaMalloc(&p->d_gmax, (size_t)p->n_inflight * tg.n_groups * sizeof(uint32_t)));
-        CUDA_TRY(p, cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tg.n_groups * (int)sizeof(uint32_t)));
+        // the attribute is per function and device, not per plan: always the maximum any plan can need
+        // (n_fft = 2^24 -> 2^24 / 512 groups = 128 KB, + 19 KB static)
+        CUDA_TRY(p, cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TOPK_MAX_GROUPS * (int)sizeof(uint32_t)));
     }
     return FSTAT_OK;
 }
@@ -451,13 +454,13 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     TmplDesc *h_tmpl = p->h_tmpl + (size_t)slot * p->tmpl_cap;
     for (size_t gi = 0; gi < groups.size(); ++gi) {
         fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &h_sky[gi]);
-        sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi]);
+        sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi], out.det_mask);
         if (h_abcd[gi].bad) p->pending_edom = true;
         for (int t = groups[gi].first; t < groups[gi].first + groups[gi].count; ++t) {
             h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
             h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
             h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
-            h_tmpl[t].pad = 0;
+            h_tmpl[t].bin_off = out.bin_off ? out.bin_off[t] : 0;
         }
     }
     CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
@@ -486,14 +489,14 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
 
     for (size_t gb = 0; gb < groups.size(); gb += p->n_sky_slots) {
         const int ng = (int)std::min<size_t>(p->n_sky_slots, groups.size() - gb);
-        rc = launch_sky_batch(p, (int)gb, ng, p->d_S, 1);
+        rc = launch_sky_batch(p, (int)gb, ng, p->d_S, 1, out.det_mask);
         if (rc) return rc;
         const int t_begin = groups[gb].first;
         const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
         for (int t0 = t_begin; t0 < t_end; t0 += TB) {
             const int nt = std::min(TB, t_end - t0);
             if (out.mode == OUT_DEV_ROWS) {
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb, nullptr, out.accumulate);
                 if (rc) return rc;
             } else if (out.mode == OUT_HOST_ROWS) {
                 if (ring_fill + nt > p->ring.rows) { rc = flush_ring(); if (rc) return rc; }
@@ -528,7 +531,7 @@ void destroy_impl(fstat_plan *p) {
     cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_base);
     for (void *t : p->d_tmp) cudaFree(t); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
-    cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax);
+    cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax); cudaFree(p->d_gmax_lin);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
     for (int i = 0; i < 2; ++i) { cudaFree(p->ring.buf[i]); if (p->ring.done[i]) cudaEventDestroy(p->ring.done[i]); }
     if (p->h_sky) cudaFreeHost(p->h_sky);
@@ -654,39 +657,13 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     g.n_fft = n_fft; g.n_bins = n_bins; g.series_stride = n_samples + 2 * SERIES_PAD; g.n_slots = n_slots;
     g.dt = dt; g.inv_dt = 1.0 / dt; g.t_sft = t_sft; g.inv_t_sft = 1.0 / t_sft; g.span = (double)n_samples * dt;
     g.f_het = f_het; g.omega_orb = eph->omega_orb; g.phi_orb0 = eph->phi_orb0; g.omega_rot = eph->omega_rot; g.gmst0 = eph->gmst0_rad;
-    const long long shift = llround((f_min - f_het) * (double)n_fft * dt);
+    // band placement (S13): bin q sits exactly at f_min + q df.  (f_min - f_het)/df = whole FFT bins (an index
+    // rotation, exact) + a fraction in [-1/2, 1/2] applied as a phase ramp over the grid index
+    const double shift_bins = (f_min - f_het) * (double)n_fft * dt;
+    const long long shift = llround(shift_bins);
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
-    const int L = ilog2(n_fft);
-    // n_fft = 2^log_n1 x 2^log_n2.  Pass 2 gets the shorter transform: its tile then spans more rows, which is what
-    // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
-    // 2^11-element tiles.  Split per size as measured on B200 (profiles/r01_v3_experiments.md, section 4).
-    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10
-             : L == 22 ? 10 : L - 12;
-    { const char *e = getenv("FSTAT_LOGN2"); if (e && atoi(e) >= 6 && atoi(e) <= 12 && L - atoi(e) >= 6 && L - atoi(e) <= 12) g.log_n2 = atoi(e); }
-    g.log_n1 = L - g.log_n2;        // pass 2 gets the shorter transform (wider tiles, longer 2F runs)
-    {   // tile sizes of the two FFT passes (profiles/r01_v3_experiments.md): 2^11-element tiles (128 threads, 4 CTAs per
-        // SM) help pass 1, whose prologue/epilogue phases need more independent CTAs to hide, as long as a
-        // tile still holds two columns (32-byte runs in the transposed store); pass 2 is indifferent and
-        // keeps 2^12 (longer 2F runs).  FSTAT_TILE_LOG1 / FSTAT_TILE_LOG2 override, for experiments.
-        // pass 2: 2^12-element tiles; 2^13 (8 rows of 2^10 points: 128-byte runs in pass 1's transposed store, 32-byte
-        // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2; likewise 4 rows
-        // of 2^11 points at 2^23, which lets pass 1 run one 2^12-point column per 2^12-element tile
-        g.log_tile2 = (g.log_n2 == 12 || (g.log_n2 == 10 && L >= 21) || (g.log_n2 == 11 && L == 23)) ? 13 : 12;
-        // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
-        // of a single column needs >= 4 rows per pass-2 tile
-        const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
-        g.log_tile1 = g.log_n1 <= 10 ? 11 : (w2_rows >= 4 ? g.log_n1 : g.log_n1 + 1);
-        const char *e1 = getenv("FSTAT_TILE_LOG1"), *e2 = getenv("FSTAT_TILE_LOG2");
-        if (e1 && (atoi(e1) >= 11 && atoi(e1) <= 13) && atoi(e1) >= g.log_n1) g.log_tile1 = atoi(e1);
-        if (e2 && (atoi(e2) >= 11 && atoi(e2) <= 13) && atoi(e2) >= g.log_n2) g.log_tile2 = atoi(e2);
-    }
-    {   // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
-        // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles; FSTAT_P2_ELEMS=16 switches it off (experiments)
-        g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
-        const char *e = getenv("FSTAT_P2_ELEMS");
-        if (e && atoi(e) == 16) g.p2_elems = 16;
-    }
-    g.log_w1 = tile_log1(p) - g.log_n1; g.log_w2 = tile_log2(p) - g.log_n2;
+    g.shift_frac_per_k = (float)((shift_bins - (double)shift) / (double)n_fft);
+    default_geometry(ilog2(n_fft), g);
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
         const double wa = fabs(eph->omega_orb * eph->au_over_c_s) + fabs(eph->omega_rot * eph->re_over_c_s);
         const double c2 = eph->omega_orb * eph->omega_orb * fabs(eph->au_over_c_s) + eph->omega_rot * eph->omega_rot * fabs(eph->re_over_c_s);
@@ -707,11 +684,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
                                   cudaMemcpyDefault, p->stream));
     SETUP_TRY(cudaMalloc(&p->d_wslot, wslot.size() * sizeof(float)));
     SETUP_TRY(cudaMemcpyAsync(p->d_wslot, wslot.data(), wslot.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-    const std::vector<float2> tw1 = make_twiddles(g.log_n1), tw2 = make_twiddles(g.log_n2, g.p2_elems);
-    SETUP_TRY(cudaMalloc(&p->d_tw1, tw1.size() * sizeof(float2)));
-    SETUP_TRY(cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
-    SETUP_TRY(cudaMemcpyAsync(p->d_tw1, tw1.data(), tw1.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
-    SETUP_TRY(cudaMemcpyAsync(p->d_tw2, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    if (upload_twiddles(p) != FSTAT_OK) return bail(FSTAT_ECUDA);
     p->n_inflight = default_inflight(n_fft, g.log_tile2);
     p->max_sky_slots = max_sky_slots_for(n_fft);
     if (ensure_sky_slots(p, 1) != FSTAT_OK) return bail(FSTAT_ENOMEM);
@@ -785,6 +758,66 @@ int fstat_compute_threshold(fstat_plan_t *plan, const fstat_template_t *tmpl_hos
     if (n_tmpl > 0 && !count_dev) return fail(plan, FSTAT_EINVAL, "null count output");
     OutSpec o; o.mode = OUT_TOPK; o.k = k; o.val = val_dev; o.bin = bin_dev; o.thr = threshold; o.count = count_dev;
     return compute_impl(plan, tmpl_host, n_tmpl, o);
+}
+
+int fstat_compute_accumulate(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, const int32_t *bin_offset_host,
+                             float *twoF_dev) {
+    OutSpec o; o.mode = OUT_DEV_ROWS; o.rows = twoF_dev; o.accumulate = true; o.bin_off = bin_offset_host;
+    if (plan && bin_offset_host)
+        for (int t = 0; t < n_tmpl; ++t)
+            if (bin_offset_host[t] <= -plan->g.n_bins || bin_offset_host[t] >= plan->g.n_bins) return fail(plan, FSTAT_EINVAL, "bin offset outside (-n_bins, n_bins)");
+    return compute_impl(plan, tmpl_host, n_tmpl, o);
+}
+
+int fstat_compute_per_detector(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_dev) {
+    if (!plan) return FSTAT_EINVAL;
+    for (int X = 0; X < plan->g.n_det; ++X) {
+        OutSpec o; o.mode = OUT_DEV_ROWS; o.det_mask = 1u << X;
+        o.rows = twoF_dev ? twoF_dev + (int64_t)X * n_tmpl * plan->g.n_bins : nullptr;
+        const int rc = compute_impl(plan, tmpl_host, n_tmpl, o);
+        if (rc) return rc;
+    }
+    return FSTAT_OK;
+}
+
+// top-k / threshold selection over caller-owned rows (e.g. the summed 2F of a semi-coherent search)
+static int select_rows(fstat_plan *p, const float *rows, int32_t n_rows, int32_t k, float *val, int32_t *bin, float thr, int32_t *count) {
+    if (!p) return FSTAT_EINVAL;
+    if (n_rows < 0 || (n_rows > 0 && (!rows || !val || !bin))) return fail(p, FSTAT_EINVAL, "null argument");
+    if (k < 1 || k > FSTAT_MAX_TOPK || k > p->g.n_bins) return fail(p, FSTAT_EINVAL, "k outside [1, min(64, n_bins)]");
+    if (n_rows == 0) return FSTAT_OK;
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    const int64_t nb = p->g.n_bins;
+    TopkGeom tg{};
+    tg.elems = 16; tg.linear = 1; tg.n_groups = (int)((nb + 511) / 512);
+    const int chunk = 1024;
+    if (!p->d_gmax_lin) {
+        CUDA_TRY(p, cudaMalloc(&p->d_gmax_lin, (size_t)chunk * tg.n_groups * sizeof(uint32_t)));
+        CUDA_TRY(p, cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TOPK_MAX_GROUPS * (int)sizeof(uint32_t)));
+    }
+    ProfScope ps(p, 3);
+    for (int r0 = 0; r0 < n_rows; r0 += chunk) {
+        const int nr = std::min(chunk, n_rows - r0);
+        const float *rp = rows + (int64_t)r0 * nb;
+        group_max_kernel<<<dim3((tg.n_groups + TOPK_THREADS / 32 - 1) / (TOPK_THREADS / 32), nr), TOPK_THREADS, 0, p->stream>>>(rp, nb, nb, tg.n_groups, p->d_gmax_lin);
+        topk_select_kernel<<<nr, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), p->stream>>>(
+            rp, nb, nb, k, p->d_gmax_lin, tg, val + (int64_t)r0 * k, bin + (int64_t)r0 * k, thr, count ? count + r0 : nullptr);
+        p->launches += 2;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    return FSTAT_OK;
+}
+
+int fstat_select_topk(fstat_plan_t *plan, const float *twoF_dev, int32_t n_rows, int32_t k, float *val_dev, int32_t *bin_dev) {
+    return select_rows(plan, twoF_dev, n_rows, k, val_dev, bin_dev, 0.f, nullptr);
+}
+
+int fstat_select_threshold(fstat_plan_t *plan, const float *twoF_dev, int32_t n_rows, float threshold, int32_t k,
+                           float *val_dev, int32_t *bin_dev, int32_t *count_dev) {
+    if (!plan) return FSTAT_EINVAL;
+    if (!std::isfinite(threshold)) return fail(plan, FSTAT_EINVAL, "non-finite threshold");
+    if (n_rows > 0 && !count_dev) return fail(plan, FSTAT_EINVAL, "null count output");
+    return select_rows(plan, twoF_dev, n_rows, k, val_dev, bin_dev, threshold, count_dev);
 }
 
 int fstat_compute_host(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_host) {
@@ -878,13 +911,54 @@ int fstat_set_profile(fstat_plan_t *plan, int32_t enable) {
 int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launches) {
     if (!plan || !ms || !launches) return FSTAT_EINVAL;
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
-    for (int c = 0; c < 4; ++c) { ms[c] = 0.0; launches[c] = 0; }
+    for (int c = 0; c < FSTAT_PROFILE_CLASSES; ++c) { ms[c] = 0.0; launches[c] = 0; }
     for (const fstat_plan::Seg &sg : plan->segs) {
         float t = 0.f;
         CUDA_TRY(plan, cudaEventElapsedTime(&t, plan->ev_pool[sg.e0], plan->ev_pool[sg.e1]));
         ms[sg.cls] += t; launches[sg.cls] += sg.launches;
     }
     plan->segs.clear(); plan->ev_used = 0;
+    return FSTAT_OK;
+}
+
+int fstat_debug_set_geometry(fstat_plan_t *plan, int32_t log_n2, int32_t log_tile1, int32_t log_tile2, int32_t p2_elems) {
+    if (!plan) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaSetDevice(plan->device));
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    PlanGeom g = plan->g;
+    const int L = ilog2(g.n_fft);
+    default_geometry(L, g);
+    if (log_n2 >= 0) { g.log_n2 = log_n2; g.log_n1 = L - log_n2; }
+    if (log_tile1 >= 0) g.log_tile1 = log_tile1;
+    if (log_tile2 >= 0) g.log_tile2 = log_tile2;
+    if (log_n2 >= 0 && log_tile1 < 0) g.log_tile1 = g.log_n1 <= 10 ? 11 : g.log_n1;
+    if (log_n2 >= 0 && log_tile2 < 0) g.log_tile2 = g.log_n2 <= 11 ? 12 : 13;
+    g.p2_elems = p2_elems >= 0 ? p2_elems : ((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 >= 12 && !(g.log_n2 == 9 && g.log_tile2 == 13)) ? 32 : 16;
+    g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
+    if (!geometry_supported(g)) return fail(plan, FSTAT_ESIZE, "no kernel instantiated for this (sub-FFT, tile, elements) combination");
+    plan->g = g;
+    cudaFree(plan->d_gmax); plan->d_gmax = nullptr;           // group count depends on the pass-2 tile shape
+    // the blocked layout of S moved: what is zero padding (k >= n_src, never written by the kernels) is now elsewhere
+    if (plan->d_S) CUDA_TRY(plan, cudaMemsetAsync(plan->d_S, 0, (size_t)plan->n_sky_slots * plan->g.n_fft * sizeof(float4), plan->stream));
+    return upload_twiddles(plan);
+}
+
+int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slots) {
+    if (!plan || max_slots < 0) return FSTAT_EINVAL;
+    CUDA_TRY(plan, cudaSetDevice(plan->device));
+    CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
+    plan->max_sky_slots = max_slots == 0 ? max_sky_slots_for(plan->g.n_fft) : max_slots;
+    if (plan->n_sky_slots > plan->max_sky_slots) {            // shrink: reallocate on the next call
+        cudaFree(plan->d_S); plan->d_S = nullptr; plan->n_sky_slots = 0;
+        return ensure_sky_slots(plan, 1);
+    }
+    return FSTAT_OK;
+}
+
+int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single) {
+    if (!plan || fused_sky < -1 || fused_sky > 1 || single < -1 || single > 1) return FSTAT_EINVAL;
+    plan->force_fused_sky = fused_sky;
+    plan->force_single = single;
     return FSTAT_OK;
 }
 

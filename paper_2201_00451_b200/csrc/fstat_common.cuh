@@ -42,7 +42,7 @@ struct TmplDesc {
     double half_fdot;     // fdot / 2
     double sixth_fddot;   // fddot / 6
     int32_t sky_slot;     // which S buffer / SkyABCD entry
-    int32_t pad;
+    int32_t bin_off;      // accumulate mode: 2F of this template's bin q is added to output bin q - bin_off (else 0)
 };
 
 // Geometry of the plan, passed by value to kernels.
@@ -60,6 +60,7 @@ struct PlanGeom {
     double f_het;
     double omega_orb, phi_orb0, omega_rot, gmst0;
     uint32_t shift_mod;     // (round((f_min - f_het)/df)) mod n_fft
+    float shift_frac_per_k; // ((f_min - f_het)/df - round(..)) / n_fft: residual band shift in cycles per grid index
     int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2 (log_n1 >= log_n2)
     int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
     int log_tile1, log_tile2;   // log2 of the tile size of FFT pass 1 / 2 (11 or 12; sub-FFTs of length 2^12 use 13)

@@ -119,6 +119,7 @@ ssb_base_kernel(PlanGeom g, double4 *__restrict__ base) {
 //   base   : [n_src] double4 from ssb_base_kernel
 //   Y      : [n_det][FARROW_NC/2][N+1] float4, the Farrow-filtered series (above)
 //   wslot  : [n_det][n_slots] float, 0 in gaps
+//   det_mask : bit X set = detector X contributes
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
 //            S[k2 / W1][k1][k2 % W1]
@@ -127,7 +128,8 @@ ssb_base_kernel(PlanGeom g, double4 *__restrict__ base) {
 // the two Horner recurrences, phase factors and antenna weights.
 __global__ void __launch_bounds__(SKY_THREADS)
 sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ base_tab,
-                    const float2 *__restrict__ Y, const float *__restrict__ wslot, float4 *__restrict__ S, int blocked) {
+                    const float2 *__restrict__ Y, const float *__restrict__ wslot, float4 *__restrict__ S, int blocked,
+                    uint32_t det_mask) {
     const int k = blockIdx.x * SKY_THREADS + threadIdx.x;          // n_src <= n_fft <= 2^24
     if (k >= g.n_src) return;
     const SkyConst &sc = skies[blockIdx.y];
@@ -143,7 +145,8 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft);
     // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32)
     const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
-    const float shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
+    // + the residual fraction of a bin when f_het is off the bin grid: |value| <= 1/2, k < 2^24 exact in fp32 (error 6e-8 cycles)
+    const float shift_cyc = fmaf((float)k, g.shift_frac_per_k, (float)tshift * (1.0f / (float)g.n_fft));
     const int n_rows = (int)g.n_samples + 1;
 
     for (int X0 = 0; X0 < g.n_det; X0 += 2) {
@@ -156,7 +159,9 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
             const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
             const double T = tau - delta;                       // detector epoch - t_start
             w[u] = 0.f;
-            if (X0 + u < g.n_det && T >= 0.0 && T < g.span) {  // step 3: inside the data and not in a gap
+            // step 3: inside the data and not in a gap (det_mask: the detectors that take part -- all of them, or one
+            // for the single-detector statistic)
+            if (X0 + u < g.n_det && ((det_mask >> X) & 1u) && T >= 0.0 && T < g.span) {
                 const int slot = min((int)(T * g.inv_t_sft), g.n_slots - 1);
                 w[u] = wslot[X * g.n_slots + slot];
             }

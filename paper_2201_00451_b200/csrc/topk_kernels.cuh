@@ -4,6 +4,7 @@
 #include "fstat_common.cuh"
 
 #define TOPK_THREADS 256
+#define TOPK_MAX_GROUPS ((1 << 24) / 512)     // groups of 512 bins per row at the largest n_fft
 
 // "a is better than b"
 __device__ __forceinline__ bool topk_better(float va, int ia, float vb, int ib) {
@@ -38,8 +39,10 @@ struct TopkGeom {
     int pl;          // product of the earlier radices
     int log_other;   // log2(N1)
     int n_groups;    // groups per row = tiles per template * warps per CTA
+    int linear;      // != 0: rows not written by pass 2 (fstat_select_*): group g is bins [512 g, 512 g + 512), maxima from group_max_kernel
 };
 __device__ __forceinline__ int64_t topk_group_bin(const TopkGeom &tg, int group, int lane, int e) {
+    if (tg.linear) return (int64_t)group * 512 + e * 32 + lane;
     const int warps = tg.nt >> 5;
     const int x = group / warps, wp = group - x * warps;
     const int rl = 1 << tg.log_rl;
@@ -198,4 +201,23 @@ topk_select_kernel(const float *__restrict__ twoF, int64_t row_stride, int64_t n
         }
         pv = v; pi = i;
     }
+}
+
+
+// Per-group maxima (as topk_key) of rows that did not come out of FFT pass 2 in this call -- e.g. the sum of 2F over the
+// segments of a semi-coherent search -- in the linear group layout: one warp per group of 512 bins.
+// grid = (ceil(n_groups / 8), n_rows), 256 threads.
+__global__ void __launch_bounds__(TOPK_THREADS)
+group_max_kernel(const float *__restrict__ rows, int64_t row_stride, int64_t n_bins, int n_groups, uint32_t *__restrict__ gmax) {
+    const int g = blockIdx.x * (TOPK_THREADS / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (g >= n_groups) return;
+    const float *row = rows + (int64_t)blockIdx.y * row_stride;
+    uint32_t key = 0u;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int64_t q = (int64_t)g * 512 + e * 32 + lane;
+        if (q < n_bins) key = max(key, topk_key(row[q]));
+    }
+    key = __reduce_max_sync(0xffffffffu, key);
+    if (lane == 0) gmax[(int64_t)blockIdx.y * n_groups + g] = key;
 }

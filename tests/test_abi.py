@@ -13,9 +13,12 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "fstat.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(fstat_[a-z_]+)\s*\(", text)))
+    syms = set()
+    for h in ("fstat.h", "fstat_debug.h"):
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        syms |= set(re.findall(r"\b(fstat_[a-z_]+)\s*\(", text))
+    return sorted(syms)
 
 
 def test_library_builds_loads_and_exports_header_symbols():

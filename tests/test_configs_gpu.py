@@ -8,8 +8,9 @@ import pytest
 from oracle import fstat_oracle as O
 from paper_2201_00451_b200 import synth
 
+from _parity_util import TOL, compare_rows
+
 pytestmark = pytest.mark.gpu
-TOL = 1e-3      # BASELINE.json north_star: |2F_gpu - 2F_cpu| <= 1e-3 * max(2F_cpu, 4)
 
 
 def _plan(prob):
@@ -56,9 +57,16 @@ def test_config2_full_size_sampled_templates_and_loudest():
     assert sample[int(np.argmax(cpu.max(axis=1)))] == p.injection_template
 
 
-@pytest.mark.parametrize("days,band", [(1, 0.1), (2, 1.0), (5, 0.5), (20, 2.0)])
-def test_config3_noise_statistics_and_sampled_parity(days, band):
-    p = synth.config3(days, band, n_templates=64 if days < 20 else 8)
+CELLS = [(d, b) for d in synth.CONFIG3_DAYS for b in synth.CONFIG3_BANDS]
+
+
+@pytest.mark.parametrize("days,band", CELLS)
+def test_config3_every_cell_noise_statistics_and_sampled_parity(days, band):
+    # all 20 cells of the timing sweep (PAPER.md:188-206 shape): 50 % gaps, pure noise.  The bank is cut to what
+    # gives >= 1e5 central bins where the cell is small and to 2-8 templates where one row is 2^21-2^22 bins.
+    p = synth.config3(days, band, n_templates=256)
+    n_t = int(min(256, max(2, (1 << 22) // p.n_bins)))
+    p.templates = p.templates[np.linspace(0, 255, n_t).astype(int)]
     with _plan(p) as plan:
         gpu = plan.compute(p.templates)
         plan.sync()
@@ -66,30 +74,73 @@ def test_config3_noise_statistics_and_sampled_parity(days, band):
     # pure noise: 2F ~ chi^2 with 4 dof over the central half of the band (pin P1 at full size)
     nb = gpu.shape[1]
     central = gpu[:, nb // 4: 3 * nb // 4].astype(np.float64)
-    assert abs(central.mean() - 4.0) < 0.1, central.mean()
-    assert abs(central.var() - 8.0) < 0.8, central.var()
-    sample = [0, len(p.templates) - 1]
-    cpu = O.fstat_2F_bank(p, sample)
-    assert _rel_err(gpu[sample], cpu).max() <= TOL
+    n_eff = central.size / 4.0          # zero padding correlates neighbouring bins
+    assert abs(central.mean() - 4.0) < max(0.1, 6.0 * np.sqrt(8.0 / n_eff)), central.mean()
+    assert abs(central.var() - 8.0) < max(0.8, 6.0 * 8.0 * np.sqrt(8.0 / n_eff)), central.var()
+    sample = [0, n_t - 1]
+    res = compare_rows(p, sample, gpu[sample], label=f"config3 T={days}d B={band}Hz n_fft=2^{int(np.log2(p.n_fft))}")
+    assert all(o["finite"] for o in res)
+    assert max(o["err"] for o in res) <= TOL
+    assert max(o["r2"] for o in res) <= 1e-4 and max(o["theta"] for o in res) <= 1e-3   # paper's own GPU-vs-CPU level: ~1e-5
 
 
-def test_config4_shape_topk_only_with_fddot():
-    # config 4 geometry (2 Hz band = sample rate, FFT 2^22, fdot x fddot bank), reduced bank; top-k output only
-    p = synth.config4(0, n_fdot=16, n_fddot=4)
+@pytest.mark.parametrize("target", [0, 1, 2, 3])
+def test_config4_full_bank_all_targets_subset_rule(target):
+    # config 4 at full geometry (10 d, 2 Hz band = sample rate, FFT 2^22, 4096 fdot x 4 fddot = 16384 templates) for
+    # all four targets 320 / 480 / 550 / 680 Hz: whole bank through fstat_compute_topk, then SURVEY.md 8(d)'s subset --
+    # every injection template, the GPU's 64 loudest, 16 seeded random ones -- as full rows against the oracle, bin by
+    # bin; "loudest template identical" = oracle argmax over the subset equals GPU argmax over the whole bank.
+    p = synth.config4(target)
     k = 8
+    n_t = len(p.templates)
+    assert n_t == 16384 and p.n_fft == 1 << 22 and p.n_bins == 1 << 22
     with _plan(p) as plan:
         val, idx = plan.compute_topk(p.templates, k)
         plan.sync()
         val, idx = val.cpu().numpy(), idx.cpu().numpy()
-    sample = [0, p.injection_template, len(p.templates) - 1]
-    cpu = O.fstat_2F_bank(p, sample)
-    for r, t in enumerate(sample):
-        cv, ci = O.topk(cpu[r], k)
-        assert idx[t, 0] == ci[0]
-        assert abs(val[t, 0] - cv[0]) <= TOL * max(cv[0], 4.0)
-        assert np.all(_rel_err(val[t], cpu[r][idx[t]]) <= TOL)       # every kept bin agrees with the oracle's 2F there
-        assert np.all(np.diff(val[t]) <= 0)
-    assert int(np.argmax(val[:, 0])) == p.injection_template
+        loud = np.lexsort((np.arange(n_t), -val[:, 0]))          # descending 2F, ties -> lower template index (S15)
+        gpu_best = int(loud[0])
+        rng = np.random.default_rng(4000 + target)
+        subset = list(loud[:64])
+        if p.injection_template is not None:
+            subset.append(p.injection_template)
+        subset += [int(t) for t in rng.choice(n_t, 16, replace=False)]
+        subset = sorted(set(int(t) for t in subset))
+        res, rows_top = [], {}
+        sky = O.per_sky(p, float(p.templates[0, 0]), float(p.templates[0, 1]))
+        for c0 in range(0, len(subset), 16):                     # 16 rows of 2^22 floats at a time
+            chunk = subset[c0:c0 + 16]
+            rows = plan.compute(p.templates[chunk])
+            plan.sync()
+            rows = rows.cpu().numpy()
+            for r, t in enumerate(chunk):                        # full rows agree with the whole-bank top-k run
+                ev, ei = O.topk(rows[r], k)
+                np.testing.assert_array_equal(idx[t], ei)
+                np.testing.assert_array_equal(val[t], ev)
+            res += compare_rows(p, chunk, rows, sky=sky, label=f"config4 target {target} ({synth.CONFIG4_TARGETS[target]:.0f} Hz) rows {c0}-{c0 + len(chunk) - 1}")
+    assert all(o["finite"] for o in res)
+    worst = max(o["err"] for o in res)
+    print(f"[parity] config4 target {target}: {len(subset)} full rows, worst {worst:.2e}")
+    assert worst <= TOL
+    # loudest template: oracle argmax over the subset == GPU argmax over all 16384
+    cpu_max = np.array([o["cpu_max"] for o in res])
+    order = np.lexsort((np.array(subset), -cpu_max))
+    cpu_best = subset[int(order[0])]
+    if cpu_best != gpu_best:        # S15: the oracle's two loudest may differ by less than twice the tolerance
+        top2 = cpu_max[order[:2]]
+        assert top2[0] - top2[1] <= 2 * TOL * max(top2[0], 4.0), (cpu_best, gpu_best, top2)
+        assert gpu_best == subset[int(order[1])]
+    for o, t in zip(res, subset):
+        assert o["cpu_argmax"] == idx[t, 0] or abs(o["cpu_max"] - val[t, 0]) <= TOL * max(o["cpu_max"], 4.0)
+    if p.injection_template is not None:
+        # the injected template peaks at the injected frequency with 2F ~ 4 + rho^2 (sd 2 sqrt(1 + rho^2 / 2)... here +- 5 sd);
+        # rho = 12 stands above the loudest noise bin of 6.9e10 trials (~57), rho = 8 (2F ~ 68 +- 16) need not
+        it, rho = p.injection_template, p.injection.rho
+        inj_bin = int(round((p.injection.f - p.f_min) / p.df))
+        assert idx[it, 0] == inj_bin
+        assert abs(val[it, 0] - (4.0 + rho * rho)) < 5.0 * np.sqrt(2.0 * (4.0 + 2.0 * rho * rho))
+        if rho >= 12.0:
+            assert gpu_best == it
 
 
 def test_config5_shape_sky_grid_dterms16():

@@ -1,0 +1,153 @@
+"""GPU parity of the entry points beyond fstat_compute / top-k: the semi-coherent accumulation over segment plans
+(PAPER.md:325), the single-detector statistic, selection over caller rows, exact band placement
+with an off-grid heterodyne frequency, and the launch-shape / multi-batch paths reached through fstat_debug.h."""
+import numpy as np
+import pytest
+
+from oracle import fstat_oracle as O
+from paper_2201_00451_b200 import synth
+from _parity_util import TOL, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _plan(prob, **kw):
+    from paper_2201_00451_b200.binding import FstatPlan
+    return FstatPlan(prob, **kw)
+
+
+@pytest.mark.parametrize("off", [0.45, -0.3])
+def test_off_grid_heterodyne_bins_are_labelled_exactly(off):
+    # DESIGN.md S13: bin q is f_min + q df whatever f_het; the injection sits exactly on a labelled bin
+    q = synth.small_problem(seed=60, rho=12.0, n_templates=3, n_samples=20000, n_fft=1 << 15)
+    p = synth.small_problem(seed=60, rho=12.0, n_templates=3, n_samples=20000, n_fft=1 << 15, f_het=q.f_het + off * q.df)
+    cpu = O.fstat_2F_bank(p)
+    with _plan(p) as plan:
+        gpu = plan.compute(p.templates)
+        plan.sync()
+        gpu = gpu.cpu().numpy()
+    assert rel_err(gpu, cpu).max() <= TOL
+    inj_bin = int(round((p.injection.f - p.f_min) / p.df))
+    assert gpu[p.injection_template].argmax() == inj_bin == cpu[p.injection_template].argmax()
+
+
+def test_semicoherent_accumulate_three_segments():
+    # three segments of a config-2-like problem (two detectors, gaps, weights), each with its own plan; the sum of 2F
+    # over segments with per-segment bin offsets, then top-k / threshold on the sum
+    import torch
+    n_seg = 3
+    probs = [synth.small_problem(seed=90 + s, rho=(7.0, 9.0, 8.0)[s], n_samples=60000, dt=0.5, n_fft=1 << 17, n_templates=4, gap_frac=0.3)
+             for s in range(n_seg)]
+    n_t, nb = len(probs[0].templates), probs[0].n_bins
+    offs = np.array([[0, 0, 0, 0], [3, -2, 0, 11], [-5, 0, 7, -1]], dtype=np.int32)      # [segment][template]
+    cpu = np.stack([O.fstat_2F_semicoherent(probs, [q.templates[t] for q in probs], offs[:, t]) for t in range(n_t)])
+    plans = [_plan(q) for q in probs]
+    try:
+        tot = torch.zeros((n_t, nb), dtype=torch.float32, device="cuda")
+        for s, plan in enumerate(plans):
+            plan.compute_accumulate(probs[s].templates, tot, offs[s])
+            plan.sync()
+        val, idx = plans[0].select_topk(tot, 6)
+        tv, ti, tc = plans[0].select_threshold(tot, 40.0, 6)
+        plans[0].sync()
+        g = tot.cpu().numpy()
+        err = np.abs(g - cpu) / np.maximum(cpu, 4.0 * n_seg)
+        assert err.max() <= TOL, err.max()
+        for t in range(n_t):
+            ev, ei = O.topk(g[t], 6)
+            np.testing.assert_array_equal(idx.cpu().numpy()[t], ei)
+            np.testing.assert_array_equal(val.cpu().numpy()[t], ev)
+            cv, ci, cc = O.threshold_candidates(g[t], np.float32(40.0), 6)
+            assert tc.cpu().numpy()[t] == cc
+            np.testing.assert_array_equal(ti.cpu().numpy()[t, :len(ci)], ci)
+            assert idx.cpu().numpy()[t, 0] == cpu[t].argmax()
+        # without offsets and on a fresh array == plain sum of fstat_compute rows (bit for bit: same adds in the same order)
+        tot2 = torch.zeros((n_t, nb), dtype=torch.float32, device="cuda")
+        ref = torch.zeros((n_t, nb), dtype=torch.float32, device="cuda")
+        for s, plan in enumerate(plans):
+            plan.compute_accumulate(probs[s].templates, tot2)
+            ref += plan.compute(probs[s].templates)
+            plan.sync()
+        assert torch.equal(tot2, ref)
+    finally:
+        for plan in plans:
+            plan.close()
+
+
+def test_per_detector_statistic_matches_oracle():
+    p = synth.small_problem(seed=95, n_det=3, rho=14.0, n_samples=30000, n_fft=1 << 16, n_templates=2, gap_frac=0.3)
+    cpu = np.stack([O.fstat_2F_per_detector(p, t) for t in p.templates], axis=1)       # [n_det][n_tmpl][n_bins]
+    with _plan(p) as plan:
+        gpu = plan.compute_per_detector(p.templates)
+        coh = plan.compute(p.templates)
+        plan.sync()
+        gpu, coh = gpu.cpu().numpy(), coh.cpu().numpy()
+    assert gpu.shape == cpu.shape
+    assert rel_err(gpu, cpu).max() <= TOL
+    assert rel_err(coh, O.fstat_2F_bank(p)).max() <= TOL          # the coherent path is untouched by the masked runs
+
+
+def test_two_live_topk_plans_of_different_size():
+    # the dynamic shared memory attribute of the selection kernel is per function, not per plan
+    big = synth.small_problem(seed=96, n_samples=int(0.7 * (1 << 20)), dt=0.5, n_fft=1 << 20, n_templates=2, rho=10.0)
+    small = synth.small_problem(seed=97, n_samples=9000, n_fft=1 << 14, n_templates=2, rho=10.0)
+    with _plan(big) as a, _plan(small) as b:
+        for _ in range(2):
+            for plan, prob in ((a, big), (b, small), (a, big)):
+                val, idx = plan.compute_topk(prob.templates, 16)
+                full = plan.compute(prob.templates)
+                plan.sync()
+                for t in range(2):
+                    ev, ei = O.topk(full.cpu().numpy()[t], 16)
+                    np.testing.assert_array_equal(idx.cpu().numpy()[t], ei)
+                    np.testing.assert_array_equal(val.cpu().numpy()[t], ev)
+
+
+def test_sky_major_bank_spanning_several_sky_batches():
+    # more sky groups than resampled-series slots: slots are reused batch after batch (fstat_debug_set_max_sky_slots)
+    p = synth.small_problem(seed=98, n_samples=20000, n_fft=1 << 15, n_templates=2, rho=None)
+    sky = synth.disc_sky_points(11, seed=3)
+    p.templates = np.array([(a, d, p.f_min, fd, 0.0) for (a, d) in sky for fd in (-3e-9, 0.0, -1e-9)])
+    cpu = O.fstat_2F_bank(p)
+    with _plan(p) as plan:
+        ref = plan.compute(p.templates)
+        plan.sync()
+        ref = ref.cpu().numpy()
+        assert rel_err(ref, cpu).max() <= TOL
+        for slots in (1, 3, 4):
+            plan.debug_set_max_sky_slots(slots)
+            got = plan.compute(p.templates)
+            val, idx = plan.compute_topk(p.templates, 3)
+            plan.sync()
+            np.testing.assert_array_equal(got.cpu().numpy(), ref)
+            np.testing.assert_array_equal(idx.cpu().numpy()[:, 0], ref.argmax(axis=1))
+
+
+@pytest.mark.parametrize("log_nfft,shapes", [
+    (16, [(8, 11, 11, 16), (8, 12, 12, 16), (7, 11, 12, 16), (9, 11, 12, 16), (9, 11, 12, 32), (9, 12, 11, 16), (6, 11, 11, 16), (10, 11, 12, 32)]),
+    (19, [(9, 11, 12, 32), (9, 12, 12, 16), (10, 11, 12, 32), (10, 11, 13, 32), (10, 11, 12, 16), (8, 11, 12, 16), (8, 12, 11, 16), (7, 12, 12, 16)]),
+    (22, [(11, 11, 12, 16), (11, 12, 13, 16), (10, 12, 13, 32), (10, 13, 12, 16), (12, 11, 13, 16), (12, 11, 12, 16), (11, 13, 11, 16)]),
+])
+def test_every_instantiated_launch_shape_gives_the_same_answer(log_nfft, shapes):
+    # fstat_debug_set_geometry: (log_n2, tile1, tile2, pass-2 elements); each shape against the oracle
+    n = int(0.72 * (1 << log_nfft))
+    p = synth.small_problem(seed=300 + log_nfft, n_samples=n, dt=0.5, n_fft=1 << log_nfft, n_templates=2, gap_frac=0.3, rho=11.0)
+    sample = [p.injection_template]
+    cpu = O.fstat_2F_bank(p, sample)
+    from paper_2201_00451_b200.binding import FstatError
+    with _plan(p) as plan:
+        for (ln2, t1, t2, e) in shapes:
+            plan.debug_set_geometry(ln2, t1, t2, e)
+            gpu = plan.compute(p.templates[sample])
+            val, idx = plan.compute_topk(p.templates[sample], 5)
+            plan.sync()
+            gpu = gpu.cpu().numpy()
+            assert rel_err(gpu, cpu).max() <= TOL, (ln2, t1, t2, e)
+            ev, ei = O.topk(gpu[0], 5)
+            np.testing.assert_array_equal(idx.cpu().numpy()[0], ei)
+        with pytest.raises(FstatError):
+            plan.debug_set_geometry(5, 11, 11, 16)                # no 2^5-point kernel
+        plan.debug_set_geometry()                                 # back to the default
+        gpu = plan.compute(p.templates[sample])
+        plan.sync()
+        assert rel_err(gpu.cpu().numpy(), cpu).max() <= TOL

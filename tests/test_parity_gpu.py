@@ -99,7 +99,7 @@ def test_resampled_series_and_antenna_sums_match_oracle():
         rot = np.exp(-2j * np.pi * np.mod(p.f_het * s["Delta"], 1.0))
         ya += s["wk"] * s["a"] * s["z"] * rot
         yb += s["wk"] * s["b"] * s["z"] * rot
-    shift = np.exp(-2j * np.pi * np.mod(O.bin_shift(p) * k, p.n_fft) / p.n_fft)
+    shift = np.exp(-2j * np.pi * O.band_shift_cycles(p, k))
     ya *= shift
     yb *= shift
     with _plan(p) as plan:
