@@ -112,22 +112,22 @@ template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     static constexpr int OFF1 = 0;
     static constexpr int OFF2 = (RadixPlan<LOGN, E>::r1 - 1) * P1;
     static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN, E>::np > 2 ? (RadixPlan<LOGN, E>::r2 - 1) * P2 : 0);
-    static constexpr int SMEM_BYTES = N * W * 16 + TW_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
+    static constexpr int BUF_ELEMS = (N + N / RadixPlan<LOGN, E>::r0) * W;  // exchange buffer: one pad column of W elements per r0 indices
+    static constexpr int SMEM_BYTES = BUF_ELEMS * 16 + TW_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
 };
 
 // Shared-memory exchange layout: element idx of lane w lives at 16-byte chunk
-//   ((idx ^ hi) << LOGW) + (w ^ lo)
-// with lo, hi taken from other bits of idx so that every access pattern of the passes --
-// "consecutive lanes -> consecutive w then consecutive idx" (loads), "stride R0 in idx" (pass-0
-// stores) and "consecutive lanes -> consecutive idx, fixed w" (last pass of pass 1) -- touches 8
-// distinct chunks per quarter warp (checked exhaustively for every LOGN by a simulator).
+//   ((idx + (idx >> LOGR0)) << LOGW) + w
+// i.e. after every r0 = 2^LOGR0 indices one column of W elements is left empty.  The stride-r0 stores of the first
+// pass then advance by (r0 + 1) W chunks from lane to lane (conflict-free: 8 distinct chunks per quarter warp for
+// every r0 in {8, 16, 32} and W in {1, 2, 4, >= 8}), the index-consecutive loads and stores of the later passes stay
+// consecutive within an aligned group of 8 lanes, and -- unlike an XOR swizzle -- every address a thread touches in one
+// pass is its base plus a compile-time offset (immediate operands instead of three integer instructions per element).
 template <int LOGW, int LOGR0> __device__ __forceinline__ int sm_phys(int idx, int w) {
-    constexpr int W = 1 << LOGW;
-    if (LOGW >= 3) return (idx << LOGW) + (w ^ (idx & 7));
-    const int hi = (idx >> LOGR0) & ((1 << (3 - LOGW)) - 1);
-    const int lo = (idx >> (3 - LOGW)) & (W - 1);
-    return ((idx ^ hi) << LOGW) + (w ^ lo);
+    return ((idx + (idx >> LOGR0)) << LOGW) + w;
 }
+// chunk offset of index distance d from a base index: valid when d is a multiple of r0, or d < r0 on an r0-aligned base
+template <int LOGW, int LOGR0> __host__ __device__ constexpr int sm_off(int d) { return (d + (d >> LOGR0)) << LOGW; }
 
 // One radix-R Stockham pass on the E register elements: twiddle (if P > 1) and DFT.
 // Work item bb of this thread is butterfly i = item_i(bb); inputs sit in slots bb*R + r.
@@ -173,9 +173,12 @@ __device__ __forceinline__ void pass_store_smem(const float2 (&a)[E], const floa
     for (int bb = 0; bb < PI::NB; ++bb) {
         int i, w;
         PI::item(bb, i, w);
+        // out_idx(i, r) = out_idx(i, 0) + r P with P = 1 (first pass: base index r0-aligned) or a multiple of r0
+        static_assert(P == 1 || (P >> LOGR0) >= 1, "pass stride must be 1 or a multiple of r0");
+        float4 *base = sm + sm_phys<LOGW, LOGR0>(PI::out_idx(i, 0), w);
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            sm[sm_phys<LOGW, LOGR0>(PI::out_idx(i, r), w)] = make_float4(a[bb * R + r].x, a[bb * R + r].y, b[bb * R + r].x, b[bb * R + r].y);
+            base[sm_off<LOGW, LOGR0>(r * P)] = make_float4(a[bb * R + r].x, a[bb * R + r].y, b[bb * R + r].x, b[bb * R + r].y);
     }
 }
 
@@ -186,14 +189,12 @@ __device__ __forceinline__ void pass_load_smem(float2 (&a)[E], float2 (&b)[E], c
     for (int bb = 0; bb < PI::NB; ++bb) {
         int i, w;
         PI::item(bb, i, w);
-#pragma unroll
-        // in_idx = i + r*NI: when r*NI only touches idx bits the swizzle does not read, the
-        // address is base + r*NI*W (immediate offsets instead of per-element index math)
-        constexpr bool AFFINE = (LOGW >= 3) ? (PI::NI >= 8) : (PI::NI >= (1 << (LOGR0 + 3 - LOGW)));
-        const int base = sm_phys<LOGW, LOGR0>(i, w);
+        // in_idx = i + r*NI with NI a multiple of r0: base + compile-time offsets
+        static_assert((PI::NI >> LOGR0) >= 1, "NI must be a multiple of r0");
+        const float4 *base = sm + sm_phys<LOGW, LOGR0>(i, w);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float4 v = AFFINE ? sm[base + ((r * PI::NI) << LOGW)] : sm[sm_phys<LOGW, LOGR0>(PI::in_idx(i, r), w)];
+            const float4 v = base[sm_off<LOGW, LOGR0>(r * PI::NI)];
             a[bb * R + r] = make_float2(v.x, v.y);
             b[bb * R + r] = make_float2(v.z, v.w);
         }
@@ -317,7 +318,7 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], c
     using RP = RadixPlan<LOGN, E>;                                                                   \
     constexpr int LOGW = C::LOGW, NT = C::NT;                                                     \
     extern __shared__ float4 sm[];                                                                \
-    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::N * C::W);                                 \
+    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::BUF_ELEMS);                                 \
     uint64_t *bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_ENTRIES);                          \
     for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];                     \
     if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }                             \
@@ -329,14 +330,63 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], c
     const int tile_mask = (1 << p.log_tiles) - 1;                                                 \
     constexpr int TILE_ELEMS = C::N * C::W
 
+// Spin-down factor exp(-i Phi_s) on the pass-0 inputs of FFT pass 1.  The r0 inputs of one butterfly sit on an
+// arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic phi(tau) = tau^2 (c1 + c2 tau):
+// its forward differences D1, D2 and the constant D3 are evaluated once per butterfly in fp64 (mod 1), and
+// exp(-2 pi i phi(tau_r)) follows by the recurrence e_{r+1} = e_r d_r, d_{r+1} = d_r q_r, q_{r+1} = q_r c (fp32
+// complex products).  Without a second spin-down (CUBIC = false) D2 is the same for every butterfly of the
+// template: q comes with the template descriptor (computed on the host in fp64) and the q recurrence disappears.
+template <int LOGN, int LOGT, int E, bool SKIPZ, bool CUBIC>
+__device__ __forceinline__ void spin_down(float2 (&a)[E], float2 (&b)[E], const FftArgs &p, const TmplDesc &td, int k2_0, int r_nz) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
+    using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
+    const double h = (double)((int64_t)PI::NI << p.log_other) * p.dt;
+    const double c1 = td.half_fdot, c2 = td.sixth_fddot;
+    float2 cc = make_float2(1.f, 0.f);
+    if (CUBIC) cc = expm2pi(6.0 * c2 * h * h * h);
+#pragma unroll
+    for (int bb = 0; bb < PI::NB; ++bb) {
+        int i, w;
+        PI::item(bb, i, w);
+        const int64_t k = ((int64_t)i << p.log_other) + k2_0 + w;
+        const double tau = (double)(k - p.k_margin) * p.dt;
+        float2 e, d, q;
+        if (CUBIC) {
+            const double t3 = 3.0 * c2 * tau;
+            e = expm2pi(tau * tau * fma(c2, tau, c1));
+            d = expm2pi(h * (fma(2.0 * tau, c1, tau * t3) + h * (c1 + t3 + c2 * h)));
+            q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
+        } else {
+            e = expm2pi(tau * tau * c1);
+            d = expm2pi(h * c1 * (2.0 * tau + h));
+            q = make_float2(td.q_re, td.q_im);             // exp(-2 pi i 2 c1 h^2)
+        }
+#pragma unroll
+        for (int r = 0; r < RP::r0; ++r) {
+            if (SKIPZ && r >= r_nz) break;
+            pcmul(a[bb * RP::r0 + r], b[bb * RP::r0 + r], e);
+            if (r + 1 < RP::r0) {
+                e = cmul(e, d);
+                d = cmul(d, q);
+                if (CUBIC) q = cmul(q, cc);
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
 // Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
 // ---------------------------------------------------------------------------------------
-// SKIPZ: do not stage or touch the zero padding (pays when at least half of every column is padding, as in config 4).
-template <int LOGN, int LOGT, int E, bool SKIPZ>
+// VAR (FFT_VAR_* bits, fft_launch.cuh) selects straight-line variants of the tile loop:
+//   SKIPZ   do not stage or touch the zero padding (pays when at least half of every column is padding, as in config 4)
+//   CUBIC   the launch holds templates with a second spin-down (fddot != 0): third forward difference in the prologue
+//   GENERIC the pass-2 tile has more rows than the last radix pass has butterflies (tiny transforms): general store address
+template <int LOGN, int LOGT, int E, int VAR>
 __global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
+    constexpr bool SKIPZ = (VAR & FFT_VAR_SKIPZ) != 0, CUBIC = (VAR & FFT_VAR_CUBIC) != 0, AFFINE = (VAR & FFT_VAR_GENERIC) == 0;
     FFT_KERNEL_PREAMBLE(E);
     const uint64_t pol_S = l2_policy_evict_last(), pol_T = l2_policy_evict_first();
     TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
@@ -355,39 +405,8 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
         mbar_wait(bar, parity);
         parity ^= 1;
         tile_take_inputs<LOGN, LOGT>(a, b, sm, SKIPZ ? r_nz : 32);
-        {   // times exp(-i Phi_s) (S9).  The r0 inputs of one butterfly sit on an
-            // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic
-            // phi(tau) = tau^2 (c1 + c2 tau): its forward differences D1, D2 and the constant D3 are
-            // evaluated once per butterfly in fp64 (mod 1), and exp(-2 pi i phi(tau_r)) follows by the
-            // recurrence e_{r+1} = e_r d_r, d_{r+1} = d_r q_r, q_{r+1} = q_r c  (fp32 complex products).
-            using PI = PassIdx<RP::r0, 1, LOGN, LOGW, NT, false>;
-            const double h = (double)((int64_t)PI::NI << p.log_other) * p.dt;
-            const double c1 = td.half_fdot, c2 = td.sixth_fddot;
-            const bool cubic = (c2 != 0.0);
-            float2 cc = make_float2(1.f, 0.f);
-            if (cubic) cc = expm2pi(6.0 * c2 * h * h * h);
-#pragma unroll
-            for (int bb = 0; bb < PI::NB; ++bb) {
-                int i, w;
-                PI::item(bb, i, w);
-                const int64_t k = ((int64_t)i << p.log_other) + k2_0 + w;
-                const double tau = (double)(k - p.k_margin) * p.dt;
-                const double t3 = 3.0 * c2 * tau;
-                float2 e = expm2pi(tau * tau * fma(c2, tau, c1));
-                float2 d = expm2pi(h * (fma(2.0 * tau, c1, tau * t3) + h * (c1 + t3 + c2 * h)));
-                float2 q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
-#pragma unroll
-                for (int r = 0; r < RP::r0; ++r) {
-                    if (SKIPZ && r >= r_nz) break;
-                    pcmul(a[bb * RP::r0 + r], b[bb * RP::r0 + r], e);
-                    if (r + 1 < RP::r0) {
-                        e = cmul(e, d);
-                        d = cmul(d, q);
-                        if (cubic) q = cmul(q, cc);
-                    }
-                }
-            }
-        }
+        // times exp(-i Phi_s) (S9)
+        spin_down<LOGN, LOGT, E, SKIPZ, CUBIC>(a, b, p, td, k2_0, r_nz);
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < p.n_tiles)
             tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
@@ -403,30 +422,32 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
             const float inv_n = 1.0f / (float)p.n_fft;
             const uint32_t nmask = (uint32_t)(p.n_fft - 1);
             const int lw2 = p.log_w_other, ln2 = p.log_other;
+            // m1 = i + r NI: when NI is a multiple of W2 the output address is affine in r (one 64-bit multiply-add per
+            // element); tiny transforms (NI < W2) take the general form (kernel variant GENERIC).
+            const uint32_t rstride_b = ((uint32_t)PI::NI << ln2) * 16u;
+            {
 #pragma unroll
-            for (int bb = 0; bb < PI::NB; ++bb) {
-                int i, w;
-                PI::item(bb, i, w);
-                const uint32_t k2 = (uint32_t)(k2_0 + w);
-                float sp, cp;
-                sincospif(-2.0f * ((float)((k2 * (uint32_t)i) & nmask) * inv_n), &sp, &cp);
-                float2 tw = make_float2(cp, sp);
-                sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
-                const float2 step = make_float2(cp, sp);
-                float4 *colbase = T + ((int64_t)k2 << lw2);
-                float4 *dst = colbase + ((int64_t)(i >> lw2) << (ln2 + lw2)) + (i & ((1 << lw2) - 1));
-                const int64_t rstride = (int64_t)PI::NI << ln2;           // valid when NI is a multiple of W2
-                const bool affine = (PI::NI >> lw2) != 0;
-                float4 *orun = dst;
+                for (int bb = 0; bb < PI::NB; ++bb) {
+                    int i, w;
+                    PI::item(bb, i, w);
+                    const uint32_t k2 = (uint32_t)(k2_0 + w);
+                    float sp, cp;
+                    sincospif(-2.0f * ((float)((k2 * (uint32_t)i) & nmask) * inv_n), &sp, &cp);
+                    float2 tw = make_float2(cp, sp);
+                    sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
+                    const float2 step = make_float2(cp, sp);
+                    float4 *colbase = T + ((uint32_t)k2 << lw2);
+                    const char *dst = reinterpret_cast<const char *>(colbase + (((uint32_t)(i >> lw2) << (ln2 + lw2)) + (uint32_t)(i & ((1 << lw2) - 1))));
 #pragma unroll
-                for (int r = 0; r < RL; ++r, orun += rstride) {
-                    float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
-                    pcmul(xx, yy, tw);
-                    const int m1 = i + r * PI::NI;
-                    float4 *o = affine ? orun
-                                       : colbase + ((int64_t)(m1 >> lw2) << (ln2 + lw2)) + (m1 & ((1 << lw2) - 1));
-                    st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
-                    if (r + 1 < RL) tw = cmul(tw, step);
+                    for (int r = 0; r < RL; ++r) {
+                        float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
+                        pcmul(xx, yy, tw);
+                        const int m1 = i + r * PI::NI;
+                        float4 *o = AFFINE ? reinterpret_cast<float4 *>(const_cast<char *>(dst) + (uint64_t)rstride_b * (uint32_t)r)
+                                           : colbase + (((uint32_t)(m1 >> lw2) << (ln2 + lw2)) + (uint32_t)(m1 & ((1 << lw2) - 1)));
+                        st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
+                        if (r + 1 < RL) tw = cmul(tw, step);
+                    }
                 }
             }
         }
@@ -501,8 +522,8 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
 }
 
 // kernel pointer by (sub-FFT, tile, pass, elements, padding variant)
-template <int LOGN, int LOGT, bool P2, int E, bool SKIPZ>
+template <int LOGN, int LOGT, bool P2, int E, int VAR>
 inline void (*fft_kernel_ptr())(const FftArgs) {
     if constexpr (P2) return fft_pass2_kernel<LOGN, LOGT, E>;
-    else return fft_pass1_kernel<LOGN, LOGT, E, SKIPZ>;
+    else return fft_pass1_kernel<LOGN, LOGT, E, VAR>;
 }

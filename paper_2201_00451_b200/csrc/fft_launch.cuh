@@ -33,20 +33,23 @@ struct LaunchCtx {
 typedef cudaError_t (*fft_launch_fn)(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, int n_t);
 
 // pass: 1 or 2; logn: log2 of the sub-FFT length; logt: log2 of the tile size; elems: register elements per thread (16
-// or 32); skipz: pass-1 variant that neither stages nor touches the zero padding.  Null when the unit has no such kernel.
+// or 32); var: FFT_VAR_* bits of the pass-1 variant (0 for pass 2).  Null when the unit has no such kernel.
+#define FFT_VAR_SKIPZ 1      // neither stage nor touch the zero padding
+#define FFT_VAR_CUBIC 2      // templates with fddot != 0 in the launch
+#define FFT_VAR_GENERIC 4    // general (non-affine) address of the transposed store
 #define FFT_N_UNITS 6
-fft_launch_fn fft_find_kernel_unit0(int pass, int logn, int logt, int elems, int skipz);
-fft_launch_fn fft_find_kernel_unit1(int pass, int logn, int logt, int elems, int skipz);
-fft_launch_fn fft_find_kernel_unit2(int pass, int logn, int logt, int elems, int skipz);
-fft_launch_fn fft_find_kernel_unit3(int pass, int logn, int logt, int elems, int skipz);
-fft_launch_fn fft_find_kernel_unit4(int pass, int logn, int logt, int elems, int skipz);
-fft_launch_fn fft_find_kernel_unit5(int pass, int logn, int logt, int elems, int skipz);
+fft_launch_fn fft_find_kernel_unit0(int pass, int logn, int logt, int elems, int var);
+fft_launch_fn fft_find_kernel_unit1(int pass, int logn, int logt, int elems, int var);
+fft_launch_fn fft_find_kernel_unit2(int pass, int logn, int logt, int elems, int var);
+fft_launch_fn fft_find_kernel_unit3(int pass, int logn, int logt, int elems, int var);
+fft_launch_fn fft_find_kernel_unit4(int pass, int logn, int logt, int elems, int var);
+fft_launch_fn fft_find_kernel_unit5(int pass, int logn, int logt, int elems, int var);
 
-inline fft_launch_fn fft_find_kernel(int pass, int logn, int logt, int elems, int skipz) {
+inline fft_launch_fn fft_find_kernel(int pass, int logn, int logt, int elems, int var) {
     fft_launch_fn (*const units[FFT_N_UNITS])(int, int, int, int, int) = {
         fft_find_kernel_unit0, fft_find_kernel_unit1, fft_find_kernel_unit2,
         fft_find_kernel_unit3, fft_find_kernel_unit4, fft_find_kernel_unit5};
     for (int u = 0; u < FFT_N_UNITS; ++u)
-        if (fft_launch_fn f = units[u](pass, logn, logt, elems, skipz)) return f;
+        if (fft_launch_fn f = units[u](pass, logn, logt, elems, var)) return f;
     return nullptr;
 }

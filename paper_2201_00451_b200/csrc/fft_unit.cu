@@ -8,13 +8,13 @@
 
 namespace {
 
-template <int LOGN, int LOGT, bool P2, int E, bool SKIPZ>
+template <int LOGN, int LOGT, bool P2, int E, int VAR>
 cudaError_t launch_pass(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN, LOGT, E>;
     constexpr int SMEM = C::SMEM_BYTES;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
-    auto kern = fft_kernel_ptr<LOGN, LOGT, P2, E, SKIPZ>();
+    auto kern = fft_kernel_ptr<LOGN, LOGT, P2, E, VAR>();
     if (configured_dev != ctx.device) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
@@ -39,17 +39,20 @@ cudaError_t launch_pass(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, in
 
 #define FFT_CAT2(a, b) a##b
 #define FFT_CAT(a, b) FFT_CAT2(a, b)
-#define K(P, LN, LT, E, Z) if (pass == P && logn == LN && logt == LT && elems == E && skipz == Z) return launch_pass<LN, LT, (P == 2), E, (Z != 0)>;
+#define K(P, LN, LT, E, V) if (pass == P && logn == LN && logt == LT && elems == E && var == V) return launch_pass<LN, LT, (P == 2), E, V>;
+#define K1(LN, LT) K(1, LN, LT, 16, 0) K(1, LN, LT, 16, FFT_VAR_CUBIC)                                             // pass 1, plain + cubic
+#define K1Z(LN, LT) K(1, LN, LT, 16, FFT_VAR_SKIPZ) K(1, LN, LT, 16, FFT_VAR_SKIPZ | FFT_VAR_CUBIC)                 // + padding-skipping variants
+#define K1G(LN, LT) K(1, LN, LT, 16, FFT_VAR_GENERIC) K(1, LN, LT, 16, FFT_VAR_GENERIC | FFT_VAR_CUBIC)             // + general store address
 
-fft_launch_fn FFT_CAT(fft_find_kernel_unit, FFT_UNIT)(int pass, int logn, int logt, int elems, int skipz) {
+fft_launch_fn FFT_CAT(fft_find_kernel_unit, FFT_UNIT)(int pass, int logn, int logt, int elems, int var) {
 #if FFT_UNIT == 0      // pass 1, sub-FFT 2^6 .. 2^9
-    K(1, 6, 11, 16, 0) K(1, 7, 11, 16, 0) K(1, 8, 11, 16, 0) K(1, 9, 11, 16, 0)
-    K(1, 6, 12, 16, 0) K(1, 7, 12, 16, 0) K(1, 8, 12, 16, 0) K(1, 9, 12, 16, 0)
+    K1(6, 11) K1(7, 11) K1(8, 11) K1(9, 11) K1(6, 12) K1(7, 12) K1(8, 12) K1(9, 12)
+    K1G(6, 11) K1G(7, 11) K1G(8, 11) K1G(6, 12) K1G(7, 12) K1G(8, 12)
 #elif FFT_UNIT == 1    // pass 1, sub-FFT 2^10, 2^11
-    K(1, 10, 11, 16, 0) K(1, 10, 12, 16, 0) K(1, 10, 13, 16, 0) K(1, 10, 11, 16, 1)
-    K(1, 11, 11, 16, 0) K(1, 11, 12, 16, 0) K(1, 11, 13, 16, 0) K(1, 11, 11, 16, 1) K(1, 11, 12, 16, 1)
+    K1(10, 11) K1(10, 12) K1(10, 13) K1Z(10, 11)
+    K1(11, 11) K1(11, 12) K1(11, 13) K1Z(11, 11) K1Z(11, 12)
 #elif FFT_UNIT == 2    // pass 1, sub-FFT 2^12
-    K(1, 12, 12, 16, 0) K(1, 12, 13, 16, 0) K(1, 12, 12, 16, 1) K(1, 12, 13, 16, 1)
+    K1(12, 12) K1(12, 13) K1Z(12, 12) K1Z(12, 13)
 #elif FFT_UNIT == 3    // pass 2, sub-FFT 2^6 .. 2^9
     K(2, 6, 11, 16, 0) K(2, 7, 11, 16, 0) K(2, 8, 11, 16, 0) K(2, 9, 11, 16, 0)
     K(2, 6, 12, 16, 0) K(2, 7, 12, 16, 0) K(2, 8, 12, 16, 0) K(2, 9, 12, 16, 0) K(2, 9, 12, 32, 0)

@@ -43,7 +43,8 @@ struct fstat_plan {
     // device memory
     float2 *d_series = nullptr;
     void *d_tmp[3] = {nullptr, nullptr, nullptr};   // setup-time scratch (freed by destroy_impl if setup fails half-way)
-    double4 *d_base = nullptr;        // [n_src] trigonometric base of the timing model per SSB grid point
+    float2 *d_rot = nullptr;          // [n_src] cos, sin of the Greenwich sidereal angle per SSB grid point
+    double4 *d_nodes = nullptr; size_t nodes_cap = 0;   // timing nodes of the sky positions of one batch [nodes_cap][n_det][n_nodes]
     float2 *d_farrow = nullptr;       // [n_det][FARROW_NC/2][N+1] float4: Farrow-filtered series (sky_kernels.cuh)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
@@ -261,13 +262,19 @@ void default_geometry(int L, PlanGeom &g) {
     g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
 }
 
-// columns that are at least half zero padding take the pass-1 variant that neither stages nor touches the padding
-// (where one is instantiated)
-int pass1_skipz(const PlanGeom &g) {
-    return (2 * g.n_src <= g.n_fft && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, 1)) ? 1 : 0;
+// pass-1 kernel variant for the plan's geometry: columns that are at least half zero padding take the variant that
+// neither stages nor touches the padding (where one is instantiated); a pass-2 tile with more rows than the last radix
+// pass of pass 1 has butterflies needs the general store address; cubic = the launch holds templates with fddot != 0
+int pass1_variant(const PlanGeom &g, bool cubic) {
+    const std::vector<int> rl = radix_list(g.log_n1);
+    const int ni_last = (1 << g.log_n1) / rl.back();
+    int var = (cubic ? FFT_VAR_CUBIC : 0) | ((ni_last >> g.log_w2) == 0 ? FFT_VAR_GENERIC : 0);
+    if (2 * g.n_src <= g.n_fft && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, var | FFT_VAR_SKIPZ)) var |= FFT_VAR_SKIPZ;
+    return var;
 }
 bool geometry_supported(const PlanGeom &g) {
-    return fft_find_kernel(1, g.log_n1, g.log_tile1, 16, 0) && fft_find_kernel(2, g.log_n2, g.log_tile2, g.p2_elems, 0);
+    return fft_find_kernel(1, g.log_n1, g.log_tile1, 16, pass1_variant(g, false)) && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, pass1_variant(g, true))
+        && fft_find_kernel(2, g.log_n2, g.log_tile2, g.p2_elems, 0);
 }
 
 // (re)upload the Stockham twiddle tables of the plan's current geometry
@@ -287,7 +294,7 @@ int tile_log1(const fstat_plan *p) { return p->g.log_tile1; }
 int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
-int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, uint32_t *gmax = nullptr, bool accumulate = false) {
+int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, bool cubic, uint32_t *gmax = nullptr, bool accumulate = false) {
     if (nt > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         cudaFree(p->d_T); p->d_T = nullptr; p->t_cap = 0;
@@ -305,7 +312,7 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     {
         ProfScope ps(p, 1);
         const int tiles1 = 1 << (l2 - p->g.log_w1);
-        const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, 16, pass1_skipz(p->g));
+        const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, 16, pass1_variant(p->g, cubic));
         if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
         CUDA_TRY(p, f(ctx, a, tiles1, nt));
         ++p->launches;
@@ -324,11 +331,34 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
 }
 
 // Sky-dependent kernel for sky groups [g0, g0+ng) -> S slots 0..ng-1.
+// room for the timing nodes of n sky positions
+int ensure_nodes(fstat_plan *p, size_t n) {
+    if (n <= p->nodes_cap) return FSTAT_OK;
+    CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    cudaFree(p->d_nodes); p->d_nodes = nullptr; p->nodes_cap = 0;
+    if (cudaMalloc(&p->d_nodes, n * p->g.n_det * p->g.n_nodes * sizeof(double4)) != cudaSuccess) { cudaGetLastError(); return fail(p, FSTAT_ENOMEM, "device allocation of the timing nodes failed"); }
+    p->nodes_cap = n;
+    return FSTAT_OK;
+}
+
+// H1 at the timing nodes of sky groups [g0, g0+ng) -> d_nodes[0..ng)
+int launch_timing_nodes(fstat_plan *p, int g0, int ng) {
+    const PlanGeom &g = p->g;
+    int rc = ensure_nodes(p, ng);
+    if (rc) return rc;
+    timing_nodes_kernel<<<dim3((unsigned)((g.n_nodes + NODE_THREADS - 1) / NODE_THREADS), g.n_det, ng), NODE_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes);
+    p->launches += 1;
+    CUDA_TRY(p, cudaGetLastError());
+    return FSTAT_OK;
+}
+
 int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked, uint32_t det_mask = 0xffffffffu) {
     const PlanGeom &g = p->g;
     ProfScope ps(p, 0);
+    int rc = launch_timing_nodes(p, g0, ng);
+    if (rc) return rc;
     dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
-    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_base, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask);
+    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;
@@ -452,6 +482,8 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     SkyConst *h_sky = p->h_sky + (size_t)slot * p->sky_cap;
     SkyABCD *h_abcd = p->h_abcd + (size_t)slot * p->sky_cap;
     TmplDesc *h_tmpl = p->h_tmpl + (size_t)slot * p->tmpl_cap;
+    // spacing in time of the first-pass inputs of one FFT pass-1 butterfly: (N1 / r0) rows of N2 samples
+    const double h_p1 = (double)(((int64_t)1 << p->g.log_n1) / radix_list(p->g.log_n1)[0]) * (double)((int64_t)1 << p->g.log_n2) * p->g.dt;
     for (size_t gi = 0; gi < groups.size(); ++gi) {
         fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &h_sky[gi]);
         sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi], out.det_mask);
@@ -461,6 +493,13 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
             h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
             h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
             h_tmpl[t].bin_off = out.bin_off ? out.bin_off[t] : 0;
+            {   // second forward difference of the spin-down phase over the first-pass input spacing of FFT pass 1
+                // (fft_kernels.cuh spin_down): 2 (fdot / 2) h^2 cycles, reduced mod 1 in fp64
+                const double cyc = tm[t].fdot * h_p1 * h_p1;
+                const double fr = cyc - std::rint(cyc);
+                h_tmpl[t].q_re = (float)cos(2.0 * M_PI * fr);
+                h_tmpl[t].q_im = (float)(-sin(2.0 * M_PI * fr));
+            }
         }
     }
     CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
@@ -495,16 +534,18 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
         for (int t0 = t_begin; t0 < t_end; t0 += TB) {
             const int nt = std::min(TB, t_end - t0);
+            bool cubic = false;                      // second spin-down anywhere in this launch?
+            for (int t = t0; t < t0 + nt && !cubic; ++t) cubic = (tm[t].fddot != 0.0);
             if (out.mode == OUT_DEV_ROWS) {
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb, nullptr, out.accumulate);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb, cubic, nullptr, out.accumulate);
                 if (rc) return rc;
             } else if (out.mode == OUT_HOST_ROWS) {
                 if (ring_fill + nt > p->ring.rows) { rc = flush_ring(); if (rc) return rc; }
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb, cubic);
                 if (rc) return rc;
                 ring_fill += nt;
             } else {
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->d_rows, nb, p->d_gmax);
+                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->d_rows, nb, cubic, p->d_gmax);
                 if (rc) return rc;
                 ProfScope ps(p, 3);
                 const TopkGeom tg = topk_geom(p);
@@ -528,7 +569,7 @@ void destroy_impl(fstat_plan *p) {
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_base);
+    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_rot); cudaFree(p->d_nodes);
     for (void *t : p->d_tmp) cudaFree(t); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
     cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
     cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax); cudaFree(p->d_gmax_lin);
@@ -664,6 +705,11 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     g.shift_mod = (uint32_t)(((shift % n_fft) + n_fft) % n_fft);
     g.shift_frac_per_k = (float)((shift_bins - (double)shift) / (double)n_fft);
     default_geometry(ilog2(n_fft), g);
+    // timing nodes (sky_kernels.cuh): the largest power of two of grid points that spans at most 256 s
+    g.log_node = 0;
+    while (g.log_node < 16 && (double)(2 << g.log_node) * dt <= 256.0) ++g.log_node;
+    g.n_nodes = (int)((g.n_src - 1) >> g.log_node) + 1;
+    g.inv_node = 1.0 / (double)(1 << g.log_node);
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
         const double wa = fabs(eph->omega_orb * eph->au_over_c_s) + fabs(eph->omega_rot * eph->re_over_c_s);
         const double c2 = eph->omega_orb * eph->omega_orb * fabs(eph->au_over_c_s) + eph->omega_rot * eph->omega_rot * fabs(eph->re_over_c_s);
@@ -698,8 +744,8 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         farrow_filter_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_series, d_fc, p->d_farrow);
         ++p->launches;
         SETUP_TRY(cudaGetLastError());
-        SETUP_TRY(cudaMalloc(&p->d_base, (size_t)g.n_src * sizeof(double4)));
-        ssb_base_kernel<<<(unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), SKY_THREADS, 0, p->stream>>>(g, p->d_base);
+        SETUP_TRY(cudaMalloc(&p->d_rot, (size_t)g.n_src * sizeof(float2)));
+        sidereal_table_kernel<<<(unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), SKY_THREADS, 0, p->stream>>>(g, p->d_rot);
         ++p->launches;
         SETUP_TRY(cudaGetLastError());
         SETUP_TRY(cudaStreamSynchronize(p->stream));

@@ -43,6 +43,7 @@ struct TmplDesc {
     double sixth_fddot;   // fddot / 6
     int32_t sky_slot;     // which S buffer / SkyABCD entry
     int32_t bin_off;      // accumulate mode: 2F of this template's bin q is added to output bin q - bin_off (else 0)
+    float q_re, q_im;     // exp(-2 pi i fdot h^2), h = time step between the first-pass inputs of FFT pass 1 (fddot = 0 path)
 };
 
 // Geometry of the plan, passed by value to kernels.
@@ -66,4 +67,6 @@ struct PlanGeom {
     int log_tile1, log_tile2;   // log2 of the tile size of FFT pass 1 / 2 (11 or 12; sub-FFTs of length 2^12 use 13)
     int p2_elems;           // register elements per thread of FFT pass 2 (16 or 32)
     int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
+    int log_node, n_nodes;  // timing nodes: every 2^log_node grid points (<= 256 s apart), n_nodes = ((n_src - 1) >> log_node) + 1
+    double inv_node;        // 2^-log_node
 };

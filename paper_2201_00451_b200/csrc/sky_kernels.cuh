@@ -105,47 +105,76 @@ farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float 
         out[(int64_t)p * (g.n_samples + 1)] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
 }
 
-// Trigonometric base of the timing model at every SSB grid point: (cos, sin) of the orbital phase and of the
-// Greenwich sidereal angle at tau_k.  Sky-independent: computed once per plan in fp64 (32 bytes per grid point).
-__global__ void __launch_bounds__(SKY_THREADS)
-ssb_base_kernel(PlanGeom g, double4 *__restrict__ base) {
-    const int64_t k = (int64_t)blockIdx.x * SKY_THREADS + threadIdx.x;
-    if (k >= g.n_src) return;
-    const SsbBase b = ssb_base(g, (double)(k - g.k_margin) * g.dt);
-    base[k] = make_double4(b.co, b.so, b.cr, b.sr);
+// ---- H1 on a coarse node grid --------------------------------------------------------------------------------
+// The delay Delta(tau) = tau - T(tau) is smooth (sidereal rotation: 21 ms amplitude, one-day period; orbit: 499 s, one
+// year), so the exact Newton inversion runs only at nodes M = 2^log_node grid points apart (M dt <= 256 s) and every
+// grid point evaluates the cubic Hermite interpolant through the node values and slopes
+//     Delta(tau_n + theta M dt) = d0 + theta (m + theta (c2 + theta c3)),   theta in [0, 1),
+// in fp64.  Interpolation error (4th derivative) h^4 / 384 < 1e-10 s (measured 6e-11 s at h = 256 s; needed: <~ 3e-8 s,
+// SURVEY 7).
+//   nodes : [n_sky][n_det][n_nodes] double4 = (d0, m, c2, c3) in seconds
+// grid = (ceil(n_nodes / 128), n_det, n_sky), 128 threads.
+#define NODE_THREADS 128
+__device__ __forceinline__ void timing_node(const PlanGeom &g, const SkyConst &sc, int X, double tau, double &delta, double &slope) {
+    const SsbBase b = ssb_base(g, tau);
+    double cth, sth;
+    delta = ssb_invert_newton(g, sc, X, b, cth, sth);
+    // d Delta / d tau = Delta_X'(T) / (1 + Delta_X'(T)) at the converged epoch T = tau - delta
+    double se, ce, sr, cr;
+    tiny_sincos(g.omega_orb * delta, se, ce);
+    small_sincos(g.omega_rot * delta, sr, cr);
+    const double co = b.co * ce + b.so * se, so = b.so * ce - b.co * se;
+    cth = b.cr * cr + b.sr * sr; sth = b.sr * cr - b.cr * sr;
+    const double dp = g.omega_orb * (sc.Ps * co - sc.Pc * so) + g.omega_rot * (sc.Qs[X] * cth - sc.Qc[X] * sth);
+    slope = dp / (1.0 + dp);
+}
+__global__ void __launch_bounds__(NODE_THREADS)
+timing_nodes_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, double4 *__restrict__ nodes) {
+    const int n = blockIdx.x * NODE_THREADS + threadIdx.x, X = blockIdx.y;
+    if (n >= g.n_nodes) return;
+    const SkyConst &sc = skies[blockIdx.z];
+    const double hstep = (double)(1 << g.log_node) * g.dt;
+    const double tau0 = (double)(((int64_t)n << g.log_node) - g.k_margin) * g.dt;
+    double d0, s0, d1, s1;
+    timing_node(g, sc, X, tau0, d0, s0);
+    timing_node(g, sc, X, tau0 + hstep, d1, s1);
+    const double m0 = s0 * hstep, m1 = s1 * hstep;
+    nodes[((int64_t)blockIdx.z * g.n_det + X) * g.n_nodes + n] =
+        make_double4(d0, m0, 3.0 * (d1 - d0) - 2.0 * m0 - m1, 2.0 * (d0 - d1) + m0 + m1);
 }
 
-// H1-H5 for one SSB grid point per thread.  grid = (ceil(n_src/256), n_sky).
-//   base   : [n_src] double4 from ssb_base_kernel
-//   Y      : [n_det][FARROW_NC/2][N+1] float4, the Farrow-filtered series (above)
+// cos, sin of the Greenwich sidereal angle at every SSB grid point (sky-independent, once per plan; fp64 -> fp32):
+// the antenna patterns need it at the detector epoch T = tau - Delta, a rotation by the small angle omega_rot Delta.
+__global__ void __launch_bounds__(SKY_THREADS)
+sidereal_table_kernel(PlanGeom g, float2 *__restrict__ rot) {
+    const int64_t k = (int64_t)blockIdx.x * SKY_THREADS + threadIdx.x;
+    if (k >= g.n_src) return;
+    double s, c;
+    sincos(g.gmst0 + g.omega_rot * ((double)(k - g.k_margin) * g.dt), &s, &c);
+    rot[k] = make_float2((float)c, (float)s);
+}
+
+// H1-H5 for SSB grid point k: adds the detectors' contributions to (ya, yb) = (Fa(t), Fb(t)) before the spin-down factor.
+//   nodes  : [n_det][n_nodes] double4 of this sky position (timing_nodes_kernel)
+//   rot    : [n_src] float2 from sidereal_table_kernel
+//   Y      : [n_det][FARROW_NC/2][N+1] float4, the Farrow-filtered series
 //   wslot  : [n_det][n_slots] float, 0 in gaps
 //   det_mask : bit X set = detector X contributes
-//   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
-//            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
-//            S[k2 / W1][k1][k2 % W1]
-// Detectors are taken two at a time: both timing inversions first, then the 2 x 80 bytes of Farrow
-// coefficients are requested together (the kernel is bound by the latency of these L2 reads), then
-// the two Horner recurrences, phase factors and antenna weights.
-__global__ void __launch_bounds__(SKY_THREADS)
-sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ base_tab,
-                    const float2 *__restrict__ Y, const float *__restrict__ wslot, float4 *__restrict__ S, int blocked,
-                    uint32_t det_mask) {
-    const int k = blockIdx.x * SKY_THREADS + threadIdx.x;          // n_src <= n_fft <= 2^24
-    if (k >= g.n_src) return;
-    const SkyConst &sc = skies[blockIdx.y];
+// Detectors are taken two at a time: the timing of both first, then the 2 x 80 bytes of Farrow coefficients are requested
+// together (these L2 reads are what the thread waits for), then the two Horner recurrences, phase factors and
+// antenna weights.  fp64 only for Delta, the fractional sample index and the heterodyne phase.
+__device__ __forceinline__ void sky_point(const PlanGeom &g, const SkyConst &sc, const double4 *__restrict__ nodes,
+                                          const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
+                                          int k, uint32_t det_mask, float2 &ya, float2 &yb) {
     const int krel = k - (int)g.k_margin;
     const double tau = (double)krel * g.dt;
-    SsbBase base;
-    {
-        const double2 *bp = reinterpret_cast<const double2 *>(base_tab + k);
-        const double2 b0 = __ldg(bp), b1 = __ldg(bp + 1);
-        base.co = b0.x; base.so = b0.y; base.cr = b1.x; base.sr = b1.y;
-    }
-    float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
+    const int nn = k >> g.log_node;
+    const double theta = (double)(k & ((1 << g.log_node) - 1)) * g.inv_node;
+    const float2 cs = __ldg(rot + k);
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft);
-    // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32)
-    const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
+    // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32);
     // + the residual fraction of a bin when f_het is off the bin grid: |value| <= 1/2, k < 2^24 exact in fp32 (error 6e-8 cycles)
+    const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
     const float shift_cyc = fmaf((float)k, g.shift_frac_per_k, (float)tshift * (1.0f / (float)g.n_fft));
     const int n_rows = (int)g.n_samples + 1;
 
@@ -155,8 +184,9 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             const int X = min(X0 + u, g.n_det - 1);
-            double cth, sth;
-            const double delta = ssb_invert_newton(g, sc, X, base, cth, sth);
+            const double2 *np = reinterpret_cast<const double2 *>(nodes + (int64_t)X * g.n_nodes + nn);
+            const double2 n0 = __ldg(np), n1 = __ldg(np + 1);
+            const double delta = fma(theta, fma(theta, fma(theta, n1.y, n1.x), n0.y), n0.x);
             const double T = tau - delta;                       // detector epoch - t_start
             w[u] = 0.f;
             // step 3: inside the data and not in a gap (det_mask: the detectors that take part -- all of them, or one
@@ -175,7 +205,11 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
             // (phase reduced mod 1 in fp64, then fp32)
             const double cyc = g.f_het * delta;
             fc[u] = (float)(cyc - floor(cyc)) + shift_cyc;
-            antenna_ab(sc, X, (float)cth, (float)sth, ca[u], cb[u]);
+            // sidereal angle at T: rotate the table value by e = omega_rot Delta (|e| < 0.05: Taylor to 1e-9)
+            const float e = (float)(g.omega_rot * delta), e2 = e * e;
+            const float se = e * fmaf(e2, fmaf(e2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+            const float ce = fmaf(e2, fmaf(e2, 1.0f / 24.0f, -0.5f), 1.0f);
+            antenna_ab(sc, X, cs.x * ce + cs.y * se, cs.y * ce - cs.x * se, ca[u], cb[u]);
         }
         float4 c[2][FARROW_NC / 2];
 #pragma unroll
@@ -200,6 +234,21 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
             yb.x = fmaf(wb, er, yb.x); yb.y = fmaf(wb, ei, yb.y);
         }
     }
+}
+
+// The hoisted form of the sky-dependent half: one SSB grid point per thread, S written once per sky position and
+// re-read by every spin-down template (long fdot banks).  grid = (ceil(n_src/256), n_sky).
+//   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
+//            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
+//            S[k2 / W1][k1][k2 % W1]
+__global__ void __launch_bounds__(SKY_THREADS)
+sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ nodes,
+                    const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
+                    float4 *__restrict__ S, int blocked, uint32_t det_mask) {
+    const int k = blockIdx.x * SKY_THREADS + threadIdx.x;          // n_src <= n_fft <= 2^24
+    if (k >= g.n_src) return;
+    float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
+    sky_point(g, skies[blockIdx.y], nodes + (int64_t)blockIdx.y * g.n_det * g.n_nodes, rot, Y, wslot, k, det_mask, ya, yb);
     int off = k;
     if (blocked) {
         const int k1 = k >> g.log_n2, k2 = k & ((1 << g.log_n2) - 1);
