@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(HERE, "..", "include")
 OBJ_DIR = os.path.join(HERE, "build")
 LIB_PATH = os.path.join(HERE, "libfstat_b200.so")
-N_FFT_UNITS = 6
+N_FFT_UNITS = 8        # 0-5: FFT pass kernels, 6: fused sky + pass 1, 7: single cooperative kernel
 # (object name, source, extra flags)
 UNITS = [("fstat_capi", "fstat_capi.cu", [])] + [(f"fft_unit{u}", "fft_unit.cu", [f"-DFFT_UNIT={u}"]) for u in range(N_FFT_UNITS)]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -16,6 +16,7 @@
 #pragma once
 #include "fstat_common.cuh"
 #include "fft_launch.cuh"
+#include "sky_math.cuh"
 
 // Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
 // a register pair holds (Re Fa, Re Fb) or (Im Fa, Im Fb) and every add / multiply / FMA is one
@@ -312,24 +313,6 @@ __device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], c
     else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
 }
 
-// Common kernel preamble: shared-memory carve-up, twiddles to shared memory, mbarrier init.
-#define FFT_KERNEL_PREAMBLE(E)                                                                   \
-    using C = FftCfg<LOGN, LOGT, E>;                                                                       \
-    using RP = RadixPlan<LOGN, E>;                                                                   \
-    constexpr int LOGW = C::LOGW, NT = C::NT;                                                     \
-    extern __shared__ float4 sm[];                                                                \
-    float2 *sm_tw = reinterpret_cast<float2 *>(sm + C::BUF_ELEMS);                                 \
-    uint64_t *bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_ENTRIES);                          \
-    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];                     \
-    if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }                             \
-    __syncthreads();                                                                              \
-    float2 a[E], b[E];                                                                              \
-    unsigned parity = 0;                                                                          \
-    int tile = blockIdx.x;                                                                        \
-    if (tile >= p.n_tiles) return;                                                                \
-    const int tile_mask = (1 << p.log_tiles) - 1;                                                 \
-    constexpr int TILE_ELEMS = C::N * C::W
-
 // Spin-down factor exp(-i Phi_s) on the pass-0 inputs of FFT pass 1.  The r0 inputs of one butterfly sit on an
 // arithmetic progression tau_r = tau_0 + r*h, and the phase (cycles) is the cubic phi(tau) = tau^2 (c1 + c2 tau):
 // its forward differences D1, D2 and the constant D3 are evaluated once per butterfly in fp64 (mod 1), and
@@ -375,6 +358,48 @@ __device__ __forceinline__ void spin_down(float2 (&a)[E], float2 (&b)[E], const 
     }
 }
 
+// Epilogue of FFT pass 1: outputs m1 = i + r*NI of column k2 = k2_0 + w, times the four-step twiddle
+// W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r (two exact sincospif per butterfly, powers by products), stored
+// tile-blocked for pass 2: T[m1 / W2][k2][m1 % W2] -- consecutive lanes (w, then i) fill whole 128-byte lines.
+// m1 = i + r NI: when NI is a multiple of W2 the output address is affine in r (one 64-bit multiply-add per element);
+// tiny transforms (NI < W2) take the general form (kernel variant GENERIC, AFFINE = false).
+template <int LOGN, int LOGT, int E, bool AFFINE>
+__device__ __forceinline__ void store_columns(const float2 (&a)[E], const float2 (&b)[E], const FftArgs &p, float4 *__restrict__ T,
+                                              int k2_0, uint64_t pol_T) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
+    constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
+    constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
+    using PI = PassIdx<RL, PL, LOGN, C::LOGW, C::NT, false>;
+    const float inv_n = 1.0f / (float)p.n_fft;
+    const uint32_t nmask = (uint32_t)(p.n_fft - 1);
+    const int lw2 = p.log_w_other, ln2 = p.log_other;
+    const uint32_t rstride_b = ((uint32_t)PI::NI << ln2) * 16u;
+#pragma unroll
+    for (int bb = 0; bb < PI::NB; ++bb) {
+        int i, w;
+        PI::item(bb, i, w);
+        const uint32_t k2 = (uint32_t)(k2_0 + w);
+        float sp, cp;
+        sincospif(-2.0f * ((float)((k2 * (uint32_t)i) & nmask) * inv_n), &sp, &cp);
+        float2 tw = make_float2(cp, sp);
+        sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
+        const float2 step = make_float2(cp, sp);
+        float4 *colbase = T + ((uint32_t)k2 << lw2);
+        const char *dst = reinterpret_cast<const char *>(colbase + (((uint32_t)(i >> lw2) << (ln2 + lw2)) + (uint32_t)(i & ((1 << lw2) - 1))));
+#pragma unroll
+        for (int r = 0; r < RL; ++r) {
+            float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
+            pcmul(xx, yy, tw);
+            const int m1 = i + r * PI::NI;
+            float4 *o = AFFINE ? reinterpret_cast<float4 *>(const_cast<char *>(dst) + (uint64_t)rstride_b * (uint32_t)r)
+                               : colbase + (((uint32_t)(m1 >> lw2) << (ln2 + lw2)) + (uint32_t)(m1 & ((1 << lw2) - 1)));
+            st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
+            if (r + 1 < RL) tw = cmul(tw, step);
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------
 // Pass 1: spin-down prologue + column FFTs of length N1 = 2^LOGN + four-step twiddle.
 // Persistent: grid = min(n_tiles, CTAs that fit the GPU); tile = (template, W adjacent columns).
@@ -383,12 +408,19 @@ __device__ __forceinline__ void spin_down(float2 (&a)[E], float2 (&b)[E], const 
 //   SKIPZ   do not stage or touch the zero padding (pays when at least half of every column is padding, as in config 4)
 //   CUBIC   the launch holds templates with a second spin-down (fddot != 0): third forward difference in the prologue
 //   GENERIC the pass-2 tile has more rows than the last radix pass has butterflies (tiny transforms): general store address
+// Tile loop over tiles tile0, tile0 + stride, ... < tile_end (tile = template * tiles_per_template + column block); the
+// intermediate of template t goes to p.T[t - t_off] (t_off != 0 only in the single-kernel form, which cycles two
+// groups of templates through an L2-resident buffer).
 template <int LOGN, int LOGT, int E, int VAR>
-__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
-fft_pass1_kernel(const __grid_constant__ FftArgs p) {
+__device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, const float2 *sm_tw, uint64_t *bar, unsigned &parity,
+                                                int tile, int tile_end, int stride, int t_off, uint64_t pol_S, uint64_t pol_T) {
     constexpr bool SKIPZ = (VAR & FFT_VAR_SKIPZ) != 0, CUBIC = (VAR & FFT_VAR_CUBIC) != 0, AFFINE = (VAR & FFT_VAR_GENERIC) == 0;
-    FFT_KERNEL_PREAMBLE(E);
-    const uint64_t pol_S = l2_policy_evict_last(), pol_T = l2_policy_evict_first();
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
+    constexpr int LOGW = C::LOGW, TILE_ELEMS = C::N * C::W;
+    if (tile >= tile_end) return;
+    float2 a[E], b[E];
+    const int tile_mask = (1 << p.log_tiles) - 1;
     TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
     // zero padding: rows k1 >= ceil(n_src / N2) of every column are zero, i.e. the inputs r >= r_nz of every first-pass
     // butterfly (k1 = i + r*NI): they are neither staged nor multiplied by the spin-down factor
@@ -396,60 +428,104 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
         : min((int)RP::r0, (int)((((p.n_src + ((int64_t)1 << p.log_other) - 1) >> p.log_other) + (C::N / RP::r0) - 1) / (C::N / RP::r0)));
     const unsigned stage_bytes = (unsigned)min(r_nz * (C::N / RP::r0), (int)C::N) * C::W * 16u;
     tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
-    for (; tile < p.n_tiles; tile += gridDim.x) {
+    for (; tile < tile_end; tile += stride) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const TmplDesc td = td_next;
         const int k2_0 = x << LOGW;
-        const int nxt = tile + gridDim.x;               // fetch the next tile's descriptor early
-        if (nxt < p.n_tiles) td_next = p.tmpl[nxt >> p.log_tiles];
+        const int nxt = tile + stride;                  // fetch the next tile's descriptor early
+        if (nxt < tile_end) td_next = p.tmpl[nxt >> p.log_tiles];
         mbar_wait(bar, parity);
         parity ^= 1;
         tile_take_inputs<LOGN, LOGT>(a, b, sm, SKIPZ ? r_nz : 32);
         // times exp(-i Phi_s) (S9)
         spin_down<LOGN, LOGT, E, SKIPZ, CUBIC>(a, b, p, td, k2_0, r_nz);
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
-        if (nxt < p.n_tiles)
+        if (nxt < tile_end)
             tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
         tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
-        {   // outputs m1 = i + r*NI of column k2 = k2_0 + w, times the four-step twiddle
-            // W_N^{k2 m1} = W_N^{k2 i} (W_N^{k2 NI})^r (two exact sincospif per butterfly, powers by
-            // products), stored tile-blocked for pass 2: T[m1 / W2][k2][m1 % W2] -- consecutive lanes
-            // (w, then i) fill whole 128-byte lines.
-            constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
-            constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
-            using PI = PassIdx<RL, PL, LOGN, LOGW, NT, false>;
-            float4 *__restrict__ T = p.T + (int64_t)t * p.n_fft;
-            const float inv_n = 1.0f / (float)p.n_fft;
-            const uint32_t nmask = (uint32_t)(p.n_fft - 1);
-            const int lw2 = p.log_w_other, ln2 = p.log_other;
-            // m1 = i + r NI: when NI is a multiple of W2 the output address is affine in r (one 64-bit multiply-add per
-            // element); tiny transforms (NI < W2) take the general form (kernel variant GENERIC).
-            const uint32_t rstride_b = ((uint32_t)PI::NI << ln2) * 16u;
-            {
-#pragma unroll
-                for (int bb = 0; bb < PI::NB; ++bb) {
-                    int i, w;
-                    PI::item(bb, i, w);
-                    const uint32_t k2 = (uint32_t)(k2_0 + w);
-                    float sp, cp;
-                    sincospif(-2.0f * ((float)((k2 * (uint32_t)i) & nmask) * inv_n), &sp, &cp);
-                    float2 tw = make_float2(cp, sp);
-                    sincospif(-2.0f * ((float)((k2 * (uint32_t)PI::NI) & nmask) * inv_n), &sp, &cp);
-                    const float2 step = make_float2(cp, sp);
-                    float4 *colbase = T + ((uint32_t)k2 << lw2);
-                    const char *dst = reinterpret_cast<const char *>(colbase + (((uint32_t)(i >> lw2) << (ln2 + lw2)) + (uint32_t)(i & ((1 << lw2) - 1))));
-#pragma unroll
-                    for (int r = 0; r < RL; ++r) {
-                        float2 xx = a[bb * RL + r], yy = b[bb * RL + r];
-                        pcmul(xx, yy, tw);
-                        const int m1 = i + r * PI::NI;
-                        float4 *o = AFFINE ? reinterpret_cast<float4 *>(const_cast<char *>(dst) + (uint64_t)rstride_b * (uint32_t)r)
-                                           : colbase + (((uint32_t)(m1 >> lw2) << (ln2 + lw2)) + (uint32_t)(m1 & ((1 << lw2) - 1)));
-                        st_global_hint(o, make_float4(xx.x, xx.y, yy.x, yy.y), pol_T);
-                        if (r + 1 < RL) tw = cmul(tw, step);
-                    }
-                }
+        store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)(t - t_off) * p.n_fft, k2_0, pol_T);
+    }
+}
+
+// shared-memory carve-up of a pass kernel: exchange buffer | twiddle table | mbarrier
+template <int LOGN, int LOGT, int E>
+__device__ __forceinline__ void pass_smem_setup(const FftArgs &p, float4 *sm, float2 *&sm_tw, uint64_t *&bar) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    sm_tw = reinterpret_cast<float2 *>(sm + C::BUF_ELEMS);
+    bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_ENTRIES);
+    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += C::NT) sm_tw[e] = p.tw[e];
+    if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }
+    __syncthreads();
+}
+
+template <int LOGN, int LOGT, int E, int VAR>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
+fft_pass1_kernel(const __grid_constant__ FftArgs p) {
+    extern __shared__ float4 sm[];
+    float2 *sm_tw; uint64_t *bar;
+    pass_smem_setup<LOGN, LOGT, E>(p, sm, sm_tw, bar);
+    unsigned parity = 0;
+    pass1_tile_loop<LOGN, LOGT, E, VAR>(p, sm, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_last(), l2_policy_evict_first());
+}
+
+// ---------------------------------------------------------------------------------------
+// Sky-varying search (PAPER.md:188 "100 sky locations", :293 2.7e5 sky pointings x 11 spin-downs): FFT pass 1 with
+// the sky-dependent half of the path (H1-H5: timing, resampling, heterodyne correction, antenna weights, detector
+// sum) in its tile prologue.  Tile = (sky position, W adjacent columns): phase A computes the tile's N1 x W values of
+// (Fa(t), Fb(t)) before the spin-down factor from the timing nodes and the Farrow-filtered series (sky_point) into
+// shared memory; phase B runs, for every spin-down template of that sky position, spin-down factor -> column FFTs ->
+// four-step twiddle -> T.  The resampled series never exists in global memory.  Phase A of one CTA (L2-latency
+// bound) overlaps with the FFT phases of the other CTAs on the SM.
+// ---------------------------------------------------------------------------------------
+template <int LOGN, int LOGT> struct FusedCfg {
+    using C = FftCfg<LOGN, LOGT, 16>;
+    static constexpr int S_ELEMS = C::N * C::W;                                   // phase-A output, linear layout
+    static constexpr int SMEM_BYTES = (S_ELEMS + C::BUF_ELEMS) * 16 + C::TW_ENTRIES * 8;
+    static constexpr int MIN_CTAS = (228 * 1024 / (SMEM_BYTES + 1024)) < 1 ? 1 : ((228 * 1024 / (SMEM_BYTES + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES + 1024)));
+};
+
+template <int LOGN, int LOGT, int VAR>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, 16>::NT, FusedCfg<LOGN, LOGT>::MIN_CTAS)
+fft_sky_pass1_kernel(const __grid_constant__ FusedArgs q) {
+    constexpr int E = 16;
+    constexpr bool CUBIC = (VAR & FFT_VAR_CUBIC) != 0, AFFINE = (VAR & FFT_VAR_GENERIC) == 0;
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
+    constexpr int LOGW = C::LOGW, NT = C::NT;
+    const FftArgs &p = q.f;
+    extern __shared__ float4 sm[];
+    float4 *sS = sm, *sX = sm + FusedCfg<LOGN, LOGT>::S_ELEMS;
+    float2 *sm_tw = reinterpret_cast<float2 *>(sX + C::BUF_ELEMS);
+    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];
+    const uint64_t pol_T = l2_policy_evict_first();
+    const int tile_mask = (1 << p.log_tiles) - 1;
+    float2 a[E], b[E];
+    for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+        const int sg = tile >> p.log_tiles, x = tile & tile_mask;
+        const int k2_0 = x << LOGW;
+        const int2 grp = q.groups[sg];                  // (first template of this sky position within the launch, count)
+        __syncthreads();                                // the previous tile's last template has taken its inputs (and the twiddles are in place)
+        {   // phase A
+            const SkyConst &sc = q.skies[sg];
+            const double4 *nodes = q.nodes + (int64_t)sg * q.g.n_det * q.g.n_nodes;
+#pragma unroll 2
+            for (int bb = 0; bb < E; ++bb) {
+                const int gi = threadIdx.x + bb * NT;                       // = k1 * W + w
+                const int k = ((gi >> LOGW) << p.log_other) + k2_0 + (gi & (C::W - 1));
+                float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
+                if (k < (int)p.n_src) sky_point(q.g, sc, nodes, q.rot, q.Y, q.wslot, k, q.det_mask, ya, yb);
+                sS[gi] = make_float4(ya.x, yb.x, ya.y, yb.y);
             }
+        }
+        __syncthreads();
+        for (int tt = 0; tt < grp.y; ++tt) {            // phase B
+            const int t = grp.x + tt;
+            const TmplDesc td = p.tmpl[t];
+            tile_take_inputs<LOGN, LOGT>(a, b, sS);
+            spin_down<LOGN, LOGT, E, false, CUBIC>(a, b, p, td, k2_0, RP::r0);
+            tile_passes<LOGN, LOGT>(a, b, sX, sm_tw);
+            tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
+            store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)t * p.n_fft, k2_0, pol_T);
         }
     }
 }
@@ -461,26 +537,30 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
 // E = register elements per thread: 16, or 32 for the two-pass radix-32 plans (sub-FFT 2^9, 2^10: one trip through
 // shared memory instead of two).
 template <int LOGN, int LOGT, int E>
-__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
-fft_pass2_kernel(const __grid_constant__ FftArgs p) {
-    FFT_KERNEL_PREAMBLE(E);
-    const uint64_t pol_T = l2_policy_evict_first();
+__device__ __forceinline__ void pass2_tile_loop(const FftArgs &p, float4 *sm, const float2 *sm_tw, uint64_t *bar, unsigned &parity,
+                                                int tile, int tile_end, int stride, int t_off, uint64_t pol_T) {
+    using C = FftCfg<LOGN, LOGT, E>;
+    using RP = RadixPlan<LOGN, E>;
+    constexpr int LOGW = C::LOGW, NT = C::NT, TILE_ELEMS = C::N * C::W;
+    if (tile >= tile_end) return;
+    float2 a[E], b[E];
+    const int tile_mask = (1 << p.log_tiles) - 1;
     int2 tm_next = *reinterpret_cast<const int2 *>(&p.tmpl[tile >> p.log_tiles].sky_slot);      // (sky_slot, bin_off)
-    tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(tile >> p.log_tiles) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_T);
-    for (; tile < p.n_tiles; tile += gridDim.x) {
+    tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)((tile >> p.log_tiles) - t_off) * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_T);
+    for (; tile < tile_end; tile += stride) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const int m1_0 = x << LOGW;
-        const int nxt = tile + gridDim.x;
+        const int nxt = tile + stride;
         const SkyABCD *abp = p.abcd + tm_next.x;
         const int boff = tm_next.y;
         const float b_over_d = abp->b_over_d, a_over_d = abp->a_over_d, two_c_over_d = abp->two_c_over_d;
-        if (nxt < p.n_tiles) tm_next = *reinterpret_cast<const int2 *>(&p.tmpl[nxt >> p.log_tiles].sky_slot);
+        if (nxt < tile_end) tm_next = *reinterpret_cast<const int2 *>(&p.tmpl[nxt >> p.log_tiles].sky_slot);
         mbar_wait(bar, parity);
         parity ^= 1;
         tile_take_inputs<LOGN, LOGT>(a, b, sm);
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
-        if (nxt < p.n_tiles)
-            tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)(nxt >> p.log_tiles) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_T);
+        if (nxt < tile_end)
+            tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)((nxt >> p.log_tiles) - t_off) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_T);
         tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
         {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
@@ -518,6 +598,70 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
                 if ((threadIdx.x & 31) == 0) p.gmax[(int64_t)tile * (NT / 32) + (threadIdx.x >> 5)] = key;
             }
         }
+    }
+}
+
+template <int LOGN, int LOGT, int E>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
+fft_pass2_kernel(const __grid_constant__ FftArgs p) {
+    extern __shared__ float4 sm[];
+    float2 *sm_tw; uint64_t *bar;
+    pass_smem_setup<LOGN, LOGT, E>(p, sm, sm_tw, bar);
+    unsigned parity = 0;
+    pass2_tile_loop<LOGN, LOGT, E>(p, sm, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_first());
+}
+
+// ---------------------------------------------------------------------------------------
+// Both passes in ONE cooperative kernel for small transforms (n_fft <= 2^18 and a bank whose intermediates fit L2):
+// with two launches per batch the path is launch-bound there (~35 us of ramp-up, tail and launch gap per pair against
+// 50-100 us of work).  The CTAs (all resident: cooperative launch) run pass 1 over a group of G templates, meet at a
+// grid-wide barrier, run pass 2 over the group, and go on to the next group; the intermediates of two consecutive
+// groups alternate between the two halves of a 2 G-template buffer that stays L2-resident (L2 evict_last stores,
+// never re-fetched from HBM), so one barrier per group is enough: when a CTA writes half (g+1) % 2 in pass 1 of group
+// g+1, every CTA has passed barrier g, i.e. finished pass 2 of group g-1, the last reader of that half.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_barrier(unsigned *counter, unsigned &target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();                                  // this CTA's stores of T are visible device-wide before it arrives
+        atomicAdd(counter, 1u);
+        unsigned seen;
+        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(seen) : "l"(counter) : "memory"); } while ((int)(seen - target) < 0);
+        asm volatile("fence.proxy.async.global;\n" ::: "memory");   // the bulk-copy (async proxy) reads that follow see those stores
+    }
+    __syncthreads();
+}
+
+template <int LOGN1, int LOGN2, int LOGT, int VAR>
+struct SingleCfg {
+    using C1 = FftCfg<LOGN1, LOGT, 16>;
+    using C2 = FftCfg<LOGN2, LOGT, 16>;
+    static constexpr int BUF = C1::BUF_ELEMS > C2::BUF_ELEMS ? C1::BUF_ELEMS : C2::BUF_ELEMS;
+    static constexpr int SMEM_BYTES = BUF * 16 + (C1::TW_ENTRIES + C2::TW_ENTRIES) * 8 + 16;
+    static constexpr int MIN_CTAS = (228 * 1024 / (SMEM_BYTES + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES + 1024));
+};
+
+template <int LOGN1, int LOGN2, int LOGT, int VAR>
+__global__ void __launch_bounds__(FftCfg<LOGN1, LOGT, 16>::NT, SingleCfg<LOGN1, LOGN2, LOGT, VAR>::MIN_CTAS)
+fft_single_kernel(const __grid_constant__ SingleArgs q) {
+    using SC = SingleCfg<LOGN1, LOGN2, LOGT, VAR>;
+    extern __shared__ float4 sm[];
+    float2 *tw1 = reinterpret_cast<float2 *>(sm + SC::BUF), *tw2 = tw1 + SC::C1::TW_ENTRIES;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(tw2 + SC::C2::TW_ENTRIES);
+    for (int e = threadIdx.x; e < SC::C1::TW_ENTRIES; e += SC::C1::NT) tw1[e] = q.p1.tw[e];
+    for (int e = threadIdx.x; e < SC::C2::TW_ENTRIES; e += SC::C1::NT) tw2[e] = q.p2.tw[e];
+    if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }
+    __syncthreads();
+    unsigned parity = 0, target = 0;
+    const uint64_t pol_keep = l2_policy_evict_last();
+    const int tiles1 = 1 << q.p1.log_tiles, tiles2 = 1 << q.p2.log_tiles;
+    for (int g = 0, t0 = 0; t0 < q.n_tmpl; ++g, t0 += q.group) {
+        const int t1 = min(t0 + q.group, q.n_tmpl);
+        const int t_off = t0 - (g & 1) * q.group;            // template t of this group lives at T[t - t_off]
+        pass1_tile_loop<LOGN1, LOGT, 16, VAR>(q.p1, sm, tw1, bar, parity, t0 * tiles1 + (int)blockIdx.x, t1 * tiles1, (int)gridDim.x, t_off, pol_keep, pol_keep);
+        grid_barrier(q.counter, target);
+        pass2_tile_loop<LOGN2, LOGT, 16>(q.p2, sm, tw2, bar, parity, t0 * tiles2 + (int)blockIdx.x, t1 * tiles2, (int)gridDim.x, t_off, pol_keep);
     }
 }
 

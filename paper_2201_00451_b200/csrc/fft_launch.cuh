@@ -23,6 +23,29 @@ struct FftArgs {
     int accumulate;           // pass 2: add 2F to what the output row holds (semi-coherent sum over segments)
 };
 
+// Arguments of the fused sky + FFT pass-1 kernel (sky-varying search): the FFT arguments plus what the sky-dependent
+// half needs.  Tiles are (sky group of the launch, column block); f.tmpl / f.T are indexed by template within the launch.
+struct FusedArgs {
+    FftArgs f;
+    PlanGeom g;
+    const SkyConst *skies;    // [groups of this launch]
+    const double4 *nodes;     // [groups of this launch][n_det][n_nodes] timing nodes
+    const float2 *rot;        // [n_src] sidereal-angle table
+    const float2 *Y;          // Farrow-filtered series
+    const float *wslot;       // [n_det][n_slots]
+    const int2 *groups;       // [groups of this launch] (first template within the launch, count)
+    uint32_t det_mask;
+};
+
+// Arguments of the single-kernel form (both passes, small transforms): the two passes' arguments, the group size G
+// (templates whose intermediates share one half of the 2 G-template buffer p1.T = p2.T) and the grid barrier counter
+// (zeroed by the host before the launch).
+struct SingleArgs {
+    FftArgs p1, p2;
+    int n_tmpl, group;
+    unsigned *counter;
+};
+
 struct LaunchCtx {
     cudaStream_t stream;
     int device;
@@ -37,6 +60,13 @@ typedef cudaError_t (*fft_launch_fn)(const LaunchCtx &ctx, FftArgs &a, int tiles
 #define FFT_VAR_SKIPZ 1      // neither stage nor touch the zero padding
 #define FFT_VAR_CUBIC 2      // templates with fddot != 0 in the launch
 #define FFT_VAR_GENERIC 4    // general (non-affine) address of the transposed store
+typedef cudaError_t (*fused_launch_fn)(const LaunchCtx &ctx, FusedArgs &a, int tiles_per_tmpl, int n_groups);
+fused_launch_fn fft_find_fused_kernel(int logn, int logt, int var);      // unit 6
+
+// single cooperative kernel (unit 7): *resident = CTAs the launch runs with (all co-resident)
+typedef cudaError_t (*single_launch_fn)(const LaunchCtx &ctx, SingleArgs &a, int *resident);
+single_launch_fn fft_find_single_kernel(int logn1, int logn2, int var);
+
 #define FFT_N_UNITS 6
 fft_launch_fn fft_find_kernel_unit0(int pass, int logn, int logt, int elems, int var);
 fft_launch_fn fft_find_kernel_unit1(int pass, int logn, int logt, int elems, int var);

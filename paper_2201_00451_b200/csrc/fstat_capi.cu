@@ -53,9 +53,11 @@ struct fstat_plan {
     int t_cap = 0;                                 // templates d_T currently holds (grown on demand up to n_inflight)
     SkyConst *d_sky = nullptr; size_t sky_cap = 0;
     SkyABCD *d_abcd = nullptr; SkyABCD *h_abcd = nullptr;   // per sky group of the current call (capacity sky_cap)
+    int2 *d_grp = nullptr; int2 *h_grp = nullptr;           // fused path: (first template within its launch, count) per sky group
     double mom[FSTAT_MAX_DET][MOM_TERMS];                   // antenna moment matrices M_X (sky_kernels.cuh)
     bool pending_edom = false;                              // a template since the last sync had D <= 0
     int force_fused_sky = -1, force_single = -1;            // fstat_debug_set_paths
+    unsigned *d_counter = nullptr;                          // grid barrier of the single-kernel form
     TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
     float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
     uint32_t *d_gmax = nullptr;       // top-k: per-group maxima of the rows in flight [n_inflight][n_groups]
@@ -259,6 +261,9 @@ void default_geometry(int L, PlanGeom &g) {
     // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
     // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles
     g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
+    // small transforms: 2^11-element tiles in both passes (pass 2 is indifferent, experiments section 2), the shape of
+    // the single-kernel form (both passes in one cooperative launch, same block size)
+    if (L <= 18) g.log_tile2 = 11;
     g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
 }
 
@@ -294,12 +299,30 @@ int tile_log1(const fstat_plan *p) { return p->g.log_tile1; }
 int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).
-int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, bool cubic, uint32_t *gmax = nullptr, bool accumulate = false) {
-    if (nt > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
+// fused_ng > 0: the templates are those of sky groups [g0, g0 + fused_ng), whose timing nodes are in d_nodes; pass 1 runs as
+// the fused sky + pass-1 kernel (no resampled series in global memory).  Otherwise pass 1 reads the S slots of the batch.
+// How the single-kernel form would group nt templates: 0 = not applicable (no kernel for the geometry, or the bank is
+// so long that the two-launch form is faster: more than 4 groups).  A group's intermediates take at most 48 MB, so
+// that two groups stay L2-resident.
+int single_group_size(fstat_plan *p, int nt, bool cubic) {
+    if (p->force_single == 0 || p->g.log_tile1 != 11 || p->g.log_tile2 != 11 || p->g.p2_elems != 16) return 0;
+    if (!fft_find_single_kernel(p->g.log_n1, p->g.log_n2, pass1_variant(p->g, cubic) & ~FFT_VAR_SKIPZ)) return 0;
+    const int cap = (int)std::max<int64_t>(1, (48ll << 20) / (p->g.n_fft * 16));
+    if (nt <= cap) return nt;
+    if (p->force_single < 0 && nt > 4 * cap) return 0;
+    const int n_groups = (nt + cap - 1) / cap;
+    return (nt + n_groups - 1) / n_groups;                  // equal groups
+}
+
+int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, bool cubic, uint32_t *gmax = nullptr,
+                     bool accumulate = false, int fused_ng = 0, uint32_t det_mask = 0xffffffffu) {
+    const int single_group = fused_ng > 0 ? 0 : single_group_size(p, nt, cubic);
+    const int t_need = single_group > 0 ? std::min(nt, 2 * single_group) : nt;
+    if (t_need > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
         cudaFree(p->d_T); p->d_T = nullptr; p->t_cap = 0;
-        if (cudaMalloc(&p->d_T, (size_t)nt * p->g.n_fft * sizeof(float4)) != cudaSuccess) { cudaGetLastError(); return fail(p, FSTAT_ENOMEM, "device allocation of the FFT intermediates failed"); }
-        p->t_cap = nt;
+        if (cudaMalloc(&p->d_T, (size_t)t_need * p->g.n_fft * sizeof(float4)) != cudaSuccess) { cudaGetLastError(); return fail(p, FSTAT_ENOMEM, "device allocation of the FFT intermediates failed"); }
+        p->t_cap = t_need;
     }
     FftArgs a{};
     a.S = p->d_S; a.T = p->d_T; a.tmpl = p->d_tmpl + t0; a.abcd = p->d_abcd + g0;
@@ -309,9 +332,36 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     const int l1 = p->g.log_n1, l2 = p->g.log_n2;
     const LaunchCtx ctx{p->stream, p->device, p->n_sm};
     a.tw = p->d_tw1; a.log_other = l2; a.log_w_other = p->g.log_w2;
-    {
+    const int tiles1 = 1 << (l2 - p->g.log_w1);
+    if (single_group > 0) {
+        // both passes in one cooperative kernel, groups of single_group templates through an L2-resident buffer
+        ProfScope ps(p, 5);
+        const single_launch_fn f = fft_find_single_kernel(l1, l2, pass1_variant(p->g, cubic) & ~FFT_VAR_SKIPZ);
+        if (!f) return fail(p, FSTAT_ESIZE, "no single-kernel form for this geometry");
+        if (!p->d_counter) CUDA_TRY(p, cudaMalloc(&p->d_counter, sizeof(unsigned)));
+        CUDA_TRY(p, cudaMemsetAsync(p->d_counter, 0, sizeof(unsigned), p->stream));
+        SingleArgs sa{};
+        sa.p1 = a; sa.p1.log_tiles = ilog2(tiles1); sa.p1.n_tiles = tiles1 * nt;
+        sa.p2 = a; sa.p2.tw = p->d_tw2; sa.p2.log_other = l1; sa.p2.log_w_other = p->g.log_w1;
+        const int tiles2 = 1 << (l1 - p->g.log_w2);
+        sa.p2.log_tiles = ilog2(tiles2); sa.p2.n_tiles = tiles2 * nt;
+        sa.n_tmpl = nt; sa.group = single_group; sa.counter = p->d_counter;
+        CUDA_TRY(p, f(ctx, sa, nullptr));
+        ++p->launches;
+        CUDA_TRY(p, cudaGetLastError());
+        return FSTAT_OK;
+    }
+    if (fused_ng > 0) {
+        ProfScope ps(p, 4);
+        const fused_launch_fn f = fft_find_fused_kernel(l1, p->g.log_tile1, pass1_variant(p->g, cubic) & ~FFT_VAR_SKIPZ);
+        if (!f) return fail(p, FSTAT_ESIZE, "no fused sky + pass-1 kernel for this geometry");
+        FusedArgs fa{};
+        fa.f = a; fa.g = p->g; fa.skies = p->d_sky + g0; fa.nodes = p->d_nodes; fa.rot = p->d_rot; fa.Y = p->d_farrow;
+        fa.wslot = p->d_wslot; fa.groups = p->d_grp + g0; fa.det_mask = det_mask;
+        CUDA_TRY(p, f(ctx, fa, tiles1, fused_ng));
+        ++p->launches;
+    } else {
         ProfScope ps(p, 1);
-        const int tiles1 = 1 << (l2 - p->g.log_w1);
         const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, 16, pass1_variant(p->g, cubic));
         if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
         CUDA_TRY(p, f(ctx, a, tiles1, nt));
@@ -380,12 +430,16 @@ int ensure_tmpl_capacity(fstat_plan *p, size_t n_tmpl, size_t n_groups) {
         if (p->h_sky) cudaFreeHost(p->h_sky);
         if (p->d_abcd) cudaFree(p->d_abcd);
         if (p->h_abcd) cudaFreeHost(p->h_abcd);
-        p->d_sky = nullptr; p->h_sky = nullptr; p->d_abcd = nullptr; p->h_abcd = nullptr; p->sky_cap = 0;
+        if (p->d_grp) cudaFree(p->d_grp);
+        if (p->h_grp) cudaFreeHost(p->h_grp);
+        p->d_sky = nullptr; p->h_sky = nullptr; p->d_abcd = nullptr; p->h_abcd = nullptr; p->d_grp = nullptr; p->h_grp = nullptr; p->sky_cap = 0;
         const size_t cap = n_groups + n_groups / 2 + 16;
         CUDA_TRY(p, cudaMalloc(&p->d_sky, cap * sizeof(SkyConst)));
         CUDA_TRY(p, cudaMallocHost(&p->h_sky, STAGE_SLOTS * cap * sizeof(SkyConst)));
         CUDA_TRY(p, cudaMalloc(&p->d_abcd, cap * sizeof(SkyABCD)));
         CUDA_TRY(p, cudaMallocHost(&p->h_abcd, STAGE_SLOTS * cap * sizeof(SkyABCD)));
+        CUDA_TRY(p, cudaMalloc(&p->d_grp, cap * sizeof(int2)));
+        CUDA_TRY(p, cudaMallocHost(&p->h_grp, STAGE_SLOTS * cap * sizeof(int2)));
         p->sky_cap = cap;
     }
     return FSTAT_OK;
@@ -473,8 +527,30 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     }
     int rc = ensure_tmpl_capacity(p, n_tmpl, groups.size());
     if (rc) return rc;
-    rc = ensure_sky_slots(p, groups.size());
-    if (rc) return rc;
+    const int TB = p->n_inflight;
+    // Two forms of the sky-dependent half.  Hoisted (default): sky_resample_kernel writes the resampled series S once per
+    // sky position, every template of that position re-reads it (from L2).  Fused (fstat_debug_set_paths(fused_sky = 1)):
+    // the per-sky work runs in the FFT pass-1 prologue and S never goes to global memory.  Measured on B200 the fused
+    // form is slower at every size (a pass-1 tile gathers grid points N2 samples apart, so the reads of
+    // the Farrow-filtered series are uncoalesced and run at 12 warps per SM), so it is never chosen automatically.
+    int max_count = 0;
+    for (const SkyGroup &sg : groups) max_count = std::max(max_count, sg.count);
+    bool fused = fft_find_fused_kernel(p->g.log_n1, p->g.log_tile1, pass1_variant(p->g, false) & ~FFT_VAR_SKIPZ) != nullptr && max_count <= TB;
+    if (fused && p->force_fused_sky == 0) fused = false;
+    if (p->force_fused_sky < 0) fused = false;
+    // fused: launches cover whole sky groups, at most TB templates each
+    std::vector<int> chunk_of(fused ? groups.size() : 0), chunk_g0;
+    if (fused) {
+        int cur_t = 0;
+        for (size_t gi = 0; gi < groups.size(); ++gi) {
+            if (chunk_g0.empty() || cur_t + groups[gi].count > TB) { chunk_g0.push_back((int)gi); cur_t = 0; }
+            chunk_of[gi] = (int)chunk_g0.size() - 1;
+            cur_t += groups[gi].count;
+        }
+    } else {
+        rc = ensure_sky_slots(p, groups.size());
+        if (rc) return rc;
+    }
     // staging buffers are reused between calls: wait until the previous upload has been consumed
     const int slot = p->stage_slot;
     p->stage_slot = (slot + 1) % STAGE_SLOTS;
@@ -482,16 +558,19 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     SkyConst *h_sky = p->h_sky + (size_t)slot * p->sky_cap;
     SkyABCD *h_abcd = p->h_abcd + (size_t)slot * p->sky_cap;
     TmplDesc *h_tmpl = p->h_tmpl + (size_t)slot * p->tmpl_cap;
+    int2 *h_grp = p->h_grp + (size_t)slot * p->sky_cap;
     // spacing in time of the first-pass inputs of one FFT pass-1 butterfly: (N1 / r0) rows of N2 samples
     const double h_p1 = (double)(((int64_t)1 << p->g.log_n1) / radix_list(p->g.log_n1)[0]) * (double)((int64_t)1 << p->g.log_n2) * p->g.dt;
     for (size_t gi = 0; gi < groups.size(); ++gi) {
         fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &h_sky[gi]);
         sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi], out.det_mask);
         if (h_abcd[gi].bad) p->pending_edom = true;
+        if (fused) h_grp[gi] = make_int2(groups[gi].first - groups[chunk_g0[chunk_of[gi]]].first, groups[gi].count);
         for (int t = groups[gi].first; t < groups[gi].first + groups[gi].count; ++t) {
             h_tmpl[t].half_fdot = 0.5 * tm[t].fdot;
             h_tmpl[t].sixth_fddot = tm[t].fddot / 6.0;
-            h_tmpl[t].sky_slot = (int)(gi % p->n_sky_slots);
+            // which SkyABCD entry (and S slot) relative to the launch's first group
+            h_tmpl[t].sky_slot = fused ? (int)gi - chunk_g0[chunk_of[gi]] : (int)(gi % p->n_sky_slots);
             h_tmpl[t].bin_off = out.bin_off ? out.bin_off[t] : 0;
             {   // second forward difference of the spin-down phase over the first-pass input spacing of FFT pass 1
                 // (fft_kernels.cuh spin_down): 2 (fdot / 2) h^2 cycles, reduced mod 1 in fp64
@@ -505,13 +584,13 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     CUDA_TRY(p, cudaMemcpyAsync(p->d_sky, h_sky, groups.size() * sizeof(SkyConst), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaMemcpyAsync(p->d_abcd, h_abcd, groups.size() * sizeof(SkyABCD), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaMemcpyAsync(p->d_tmpl, h_tmpl, (size_t)n_tmpl * sizeof(TmplDesc), cudaMemcpyHostToDevice, p->stream));
+    if (fused) CUDA_TRY(p, cudaMemcpyAsync(p->d_grp, h_grp, groups.size() * sizeof(int2), cudaMemcpyHostToDevice, p->stream));
     CUDA_TRY(p, cudaEventRecord(p->staging_ev[slot], p->stream));
 
     if (out.mode == OUT_TOPK) { rc = ensure_topk_scratch(p); if (rc) return rc; }
     if (out.mode == OUT_HOST_ROWS) { rc = ensure_host_ring(p); if (rc) return rc; }
 
     const int64_t nb = p->g.n_bins;
-    const int TB = p->n_inflight;
     int ring_i = 0; int64_t ring_fill = 0; int64_t ring_row0 = 0;   // host-ring state
     auto flush_ring = [&](void) -> int {
         if (ring_fill == 0) return FSTAT_OK;
@@ -526,34 +605,54 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         return FSTAT_OK;
     };
 
-    for (size_t gb = 0; gb < groups.size(); gb += p->n_sky_slots) {
-        const int ng = (int)std::min<size_t>(p->n_sky_slots, groups.size() - gb);
-        rc = launch_sky_batch(p, (int)gb, ng, p->d_S, 1, out.det_mask);
-        if (rc) return rc;
-        const int t_begin = groups[gb].first;
-        const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
-        for (int t0 = t_begin; t0 < t_end; t0 += TB) {
-            const int nt = std::min(TB, t_end - t0);
-            bool cubic = false;                      // second spin-down anywhere in this launch?
-            for (int t = t0; t < t0 + nt && !cubic; ++t) cubic = (tm[t].fddot != 0.0);
-            if (out.mode == OUT_DEV_ROWS) {
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, out.rows + (int64_t)t0 * nb, nb, cubic, nullptr, out.accumulate);
+    // FFT + 2F (+ selection) of templates [t0, t0 + nt), whose sky groups start at g0
+    auto run_chunk = [&](int g0, int t0, int nt, int fused_ng) -> int {
+        bool cubic = false;                      // second spin-down anywhere in this launch?
+        for (int t = t0; t < t0 + nt && !cubic; ++t) cubic = (tm[t].fddot != 0.0);
+        int r;
+        if (out.mode == OUT_DEV_ROWS) {
+            r = launch_fft_chunk(p, g0, t0, nt, out.rows + (int64_t)t0 * nb, nb, cubic, nullptr, out.accumulate, fused_ng, out.det_mask);
+            if (r) return r;
+        } else if (out.mode == OUT_HOST_ROWS) {
+            if (ring_fill + nt > p->ring.rows) { r = flush_ring(); if (r) return r; }
+            r = launch_fft_chunk(p, g0, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb, cubic, nullptr, false, fused_ng, out.det_mask);
+            if (r) return r;
+            ring_fill += nt;
+        } else {
+            r = launch_fft_chunk(p, g0, t0, nt, p->d_rows, nb, cubic, p->d_gmax, false, fused_ng, out.det_mask);
+            if (r) return r;
+            ProfScope ps(p, 3);
+            const TopkGeom tg = topk_geom(p);
+            topk_select_kernel<<<nt, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), p->stream>>>(
+                p->d_rows, nb, nb, out.k, p->d_gmax, tg, out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k,
+                out.thr, out.count ? out.count + t0 : nullptr);
+            p->launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
+        }
+        return FSTAT_OK;
+    };
+    if (fused) {
+        for (size_t c = 0; c < chunk_g0.size(); ++c) {
+            const int gA = chunk_g0[c], gB = c + 1 < chunk_g0.size() ? chunk_g0[c + 1] : (int)groups.size();
+            const int tA = groups[gA].first, tB = groups[gB - 1].first + groups[gB - 1].count;
+            {
+                ProfScope ps(p, 0);
+                rc = launch_timing_nodes(p, gA, gB - gA);
                 if (rc) return rc;
-            } else if (out.mode == OUT_HOST_ROWS) {
-                if (ring_fill + nt > p->ring.rows) { rc = flush_ring(); if (rc) return rc; }
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->ring.buf[ring_i] + ring_fill * nb, nb, cubic);
+            }
+            rc = run_chunk(gA, tA, tB - tA, gB - gA);
+            if (rc) return rc;
+        }
+    } else {
+        for (size_t gb = 0; gb < groups.size(); gb += p->n_sky_slots) {
+            const int ng = (int)std::min<size_t>(p->n_sky_slots, groups.size() - gb);
+            rc = launch_sky_batch(p, (int)gb, ng, p->d_S, 1, out.det_mask);
+            if (rc) return rc;
+            const int t_begin = groups[gb].first;
+            const int t_end = groups[gb + ng - 1].first + groups[gb + ng - 1].count;
+            for (int t0 = t_begin; t0 < t_end; t0 += TB) {
+                rc = run_chunk((int)gb, t0, std::min(TB, t_end - t0), 0);
                 if (rc) return rc;
-                ring_fill += nt;
-            } else {
-                rc = launch_fft_chunk(p, (int)gb, t0, nt, p->d_rows, nb, cubic, p->d_gmax);
-                if (rc) return rc;
-                ProfScope ps(p, 3);
-                const TopkGeom tg = topk_geom(p);
-                topk_select_kernel<<<nt, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), p->stream>>>(
-                    p->d_rows, nb, nb, out.k, p->d_gmax, tg, out.val + (int64_t)t0 * out.k, out.bin + (int64_t)t0 * out.k,
-                    out.thr, out.count ? out.count + t0 : nullptr);
-                p->launches += 1;
-                CUDA_TRY(p, cudaGetLastError());
             }
         }
     }
@@ -569,15 +668,16 @@ void destroy_impl(fstat_plan *p) {
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_rot); cudaFree(p->d_nodes);
+    cudaFree(p->d_series); cudaFree(p->d_farrow); cudaFree(p->d_rot); cudaFree(p->d_nodes); cudaFree(p->d_counter);
     for (void *t : p->d_tmp) cudaFree(t); cudaFree(p->d_wslot); cudaFree(p->d_tw1); cudaFree(p->d_tw2);
-    cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd);
+    cudaFree(p->d_S); cudaFree(p->d_T); cudaFree(p->d_sky); cudaFree(p->d_abcd); cudaFree(p->d_grp);
     cudaFree(p->d_tmpl); cudaFree(p->d_rows); cudaFree(p->d_gmax); cudaFree(p->d_gmax_lin);
     cudaFree(p->d_topk_v); cudaFree(p->d_topk_i);
     for (int i = 0; i < 2; ++i) { cudaFree(p->ring.buf[i]); if (p->ring.done[i]) cudaEventDestroy(p->ring.done[i]); }
     if (p->h_sky) cudaFreeHost(p->h_sky);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
     if (p->h_abcd) cudaFreeHost(p->h_abcd);
+    if (p->h_grp) cudaFreeHost(p->h_grp);
     for (int i = 0; i < STAGE_SLOTS; ++i) if (p->staging_ev[i]) cudaEventDestroy(p->staging_ev[i]);
     if (p->chunk_ev) cudaEventDestroy(p->chunk_ev);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);

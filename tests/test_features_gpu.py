@@ -151,3 +151,87 @@ def test_every_instantiated_launch_shape_gives_the_same_answer(log_nfft, shapes)
         gpu = plan.compute(p.templates[sample])
         plan.sync()
         assert rel_err(gpu.cpu().numpy(), cpu).max() <= TOL
+
+
+def _sky_bank(p, n_sky, fdots, seed, fddot=0.0):
+    sky = synth.disc_sky_points(n_sky, seed=seed)
+    rows = []
+    for s, (a, d) in enumerate(sky):
+        for fd in fdots[: 1 + (s % len(fdots))] if isinstance(fdots, tuple) else fdots:
+            rows.append((a, d, p.f_min, fd, fddot))
+    return np.array(rows)
+
+
+@pytest.mark.parametrize("log_nfft,n_samples,dt,fddot", [(15, 20000, 1.0, 0.0), (17, 100003, 1.0, 2e-15), (18, 250000, 0.5, 0.0), (12, 1500, 1.0, 0.0)])
+def test_fused_sky_pass1_matches_oracle_and_hoisted_path(log_nfft, n_samples, dt, fddot):
+    # sky-varying bank: the per-sky work runs inside the FFT pass-1 prologue (no resampled series in
+    # global memory).  Ragged bank: 1..3 spin-down templates per sky position; several launches (small in-flight count).
+    p = synth.small_problem(seed=400 + log_nfft, n_samples=n_samples, dt=dt, n_fft=1 << log_nfft, n_templates=2, gap_frac=0.3, rho=None)
+    p.templates = _sky_bank(p, 9, (-3e-9, 0.0, -1e-9), seed=5, fddot=fddot)
+    cpu = O.fstat_2F_bank(p)
+    with _plan(p) as plan:
+        plan.debug_set_paths(fused_sky=0)
+        hoisted = plan.compute(p.templates)
+        plan.sync()
+        hoisted = hoisted.cpu().numpy()
+        plan.debug_set_paths(fused_sky=1)
+        l0 = plan.launch_count()
+        plan.set_profile(True)
+        fused = plan.compute(p.templates)
+        plan.sync()
+        prof = plan.get_profile()
+        plan.set_profile(False)
+        assert prof["fused_sky_pass1"][1] >= 1 and prof["fft_pass1"][1] == 0       # the fused kernel ran, the plain pass 1 did not
+        fused = fused.cpu().numpy()
+        assert rel_err(hoisted, cpu).max() <= TOL
+        assert rel_err(fused, cpu).max() <= TOL
+        np.testing.assert_allclose(fused, hoisted, rtol=0, atol=2e-5 * max(4.0, float(cpu.max())))
+        plan.set_inflight(4)                                   # several launches, sky groups never split
+        again = plan.compute(p.templates)
+        val, idx = plan.compute_topk(p.templates, 4)
+        per = plan.compute_per_detector(p.templates[:5])
+        plan.sync()
+        np.testing.assert_array_equal(again.cpu().numpy(), fused)
+        np.testing.assert_array_equal(idx.cpu().numpy()[:, 0], fused.argmax(axis=1))
+        cpu_per = np.stack([O.fstat_2F_per_detector(p, t) for t in p.templates[:5]], axis=1)
+        assert rel_err(per.cpu().numpy(), cpu_per).max() <= TOL
+        plan.debug_set_paths()                                 # automatic: the hoisted form (measured faster)
+        plan.set_inflight(0)
+        plan.set_profile(True)
+        auto = plan.compute(p.templates)
+        plan.sync()
+        assert plan.get_profile()["fused_sky_pass1"][1] == 0
+        np.testing.assert_array_equal(auto.cpu().numpy(), hoisted)
+
+
+@pytest.mark.parametrize("log_nfft,n_samples,dt,n_t", [(12, 1500, 1.0, 5), (13, 5000, 1.0, 3), (14, 11000, 1.0, 3), (15, 20000, 1.0, 200),
+                                                       (16, 50001, 1.0, 7), (17, 100003, 1.0, 40), (18, 250000, 0.5, 30)])
+def test_single_kernel_form_matches_two_launch_form_and_oracle(log_nfft, n_samples, dt, n_t):
+    # small transforms: both FFT passes in one cooperative kernel, groups of templates through an L2-resident buffer with a
+    # grid-wide barrier per group (n_t is chosen so that 2^15, 2^17 and 2^18 need 2-3 groups)
+    p = synth.small_problem(seed=500 + log_nfft, n_samples=n_samples, dt=dt, n_fft=1 << log_nfft, n_templates=n_t, gap_frac=0.3,
+                            rho=11.0, fddot=3e-16 if log_nfft % 2 else 0.0)
+    sample = sorted({0, p.injection_template, n_t - 1})
+    cpu = O.fstat_2F_bank(p, sample)
+    with _plan(p) as plan:
+        plan.debug_set_paths(single=0)
+        plan.set_profile(True)
+        two = plan.compute(p.templates)
+        plan.sync()
+        prof = plan.get_profile()
+        assert prof["fft_single"][1] == 0 and prof["fft_pass1"][1] >= 1
+        plan.debug_set_paths(single=1)
+        one = plan.compute(p.templates)
+        val, idx = plan.compute_topk(p.templates, 5)
+        plan.sync()
+        prof = plan.get_profile()
+        plan.set_profile(False)
+        assert prof["fft_single"][1] == 2 and prof["fft_pass1"][1] == 0 and prof["fft_pass2"][1] == 0
+        two, one = two.cpu().numpy(), one.cpu().numpy()
+        np.testing.assert_array_equal(one, two)                   # same tiles, same arithmetic, same order
+        assert rel_err(one[sample], cpu).max() <= TOL
+        for t in sample:
+            ev, ei = O.topk(one[t], 5)
+            np.testing.assert_array_equal(idx.cpu().numpy()[t], ei)
+            np.testing.assert_array_equal(val.cpu().numpy()[t], ev)
+        assert int(np.argmax(one.max(axis=1))) == p.injection_template or n_samples * dt < 50000
