@@ -114,7 +114,12 @@ template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     static constexpr int OFF2 = (RadixPlan<LOGN, E>::r1 - 1) * P1;
     static constexpr int TW_ENTRIES = OFF2 + (RadixPlan<LOGN, E>::np > 2 ? (RadixPlan<LOGN, E>::r2 - 1) * P2 : 0);
     static constexpr int BUF_ELEMS = (N + N / RadixPlan<LOGN, E>::r0) * W;  // exchange buffer: one pad column of W elements per r0 indices
-    static constexpr int SMEM_BYTES = BUF_ELEMS * 16 + TW_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
+    // twiddles of the last radix pass of the 2^11-point plan (14 KB) are read from global memory through L1 instead of
+    // shared memory: one more CTA per SM with 2^11-element tiles (measured +1 %; at 2^12 points a third CTA per SM costs
+    // more in registers than it gains)
+    static constexpr bool TW_LAST_GLOBAL = (RadixPlan<LOGN, E>::np > 2) && (LOGN == 11);
+    static constexpr int TW_SMEM_ENTRIES = TW_LAST_GLOBAL ? OFF2 : TW_ENTRIES;
+    static constexpr int SMEM_BYTES = BUF_ELEMS * 16 + TW_SMEM_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
 };
 
 // Shared-memory exchange layout: element idx of lane w lives at 16-byte chunk
@@ -149,7 +154,7 @@ struct PassIdx {
     }
 };
 
-template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int E>
+template <int R, int P, int LOGN, int LOGW, int NT, bool IFAST, int E, bool TW_LDG = false>
 __device__ __forceinline__ void pass_compute(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw) {
     using PI = PassIdx<R, P, LOGN, LOGW, NT, IFAST>;
 #pragma unroll
@@ -160,7 +165,7 @@ __device__ __forceinline__ void pass_compute(float2 (&a)[E], float2 (&b)[E], con
             const int k = i & (P - 1);
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                pcmul(a[bb * R + r], b[bb * R + r], tw[(r - 1) * P + k]);
+                pcmul(a[bb * R + r], b[bb * R + r], TW_LDG ? __ldg(tw + (r - 1) * P + k) : tw[(r - 1) * P + k]);
             }
         }
         dft<R>(&a[bb * R], &b[bb * R]);
@@ -305,11 +310,13 @@ __device__ __forceinline__ void tile_passes(float2 (&a)[E], float2 (&b)[E], floa
     __syncthreads();                                   // buffer free: the next tile may be prefetched
 }
 
+// tw: the shared-memory table; tw_g: the same table in global memory (used for the last pass when it is not in shared memory)
 template <int LOGN, int LOGT, int E>
-__device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw) {
+__device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw, const float2 *__restrict__ tw_g) {
     using C = FftCfg<LOGN, LOGT, E>;
     using RP = RadixPlan<LOGN, E>;
     if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
+    else if (C::TW_LAST_GLOBAL) pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false, E, true>(a, b, tw_g + C::OFF2);
     else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
 }
 
@@ -442,7 +449,7 @@ __device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, co
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < tile_end)
             tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
-        tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
+        tile_last_pass<LOGN, LOGT>(a, b, sm_tw, p.tw);
         store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)(t - t_off) * p.n_fft, k2_0, pol_T);
     }
 }
@@ -452,8 +459,8 @@ template <int LOGN, int LOGT, int E>
 __device__ __forceinline__ void pass_smem_setup(const FftArgs &p, float4 *sm, float2 *&sm_tw, uint64_t *&bar) {
     using C = FftCfg<LOGN, LOGT, E>;
     sm_tw = reinterpret_cast<float2 *>(sm + C::BUF_ELEMS);
-    bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_ENTRIES);
-    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += C::NT) sm_tw[e] = p.tw[e];
+    bar = reinterpret_cast<uint64_t *>(sm_tw + C::TW_SMEM_ENTRIES);
+    for (int e = threadIdx.x; e < C::TW_SMEM_ENTRIES; e += C::NT) sm_tw[e] = p.tw[e];
     if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }
     __syncthreads();
 }
@@ -480,7 +487,7 @@ fft_pass1_kernel(const __grid_constant__ FftArgs p) {
 template <int LOGN, int LOGT> struct FusedCfg {
     using C = FftCfg<LOGN, LOGT, 16>;
     static constexpr int S_ELEMS = C::N * C::W;                                   // phase-A output, linear layout
-    static constexpr int SMEM_BYTES = (S_ELEMS + C::BUF_ELEMS) * 16 + C::TW_ENTRIES * 8;
+    static constexpr int SMEM_BYTES = (S_ELEMS + C::BUF_ELEMS) * 16 + C::TW_SMEM_ENTRIES * 8;
     static constexpr int MIN_CTAS = (228 * 1024 / (SMEM_BYTES + 1024)) < 1 ? 1 : ((228 * 1024 / (SMEM_BYTES + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES + 1024)));
 };
 
@@ -496,7 +503,7 @@ fft_sky_pass1_kernel(const __grid_constant__ FusedArgs q) {
     extern __shared__ float4 sm[];
     float4 *sS = sm, *sX = sm + FusedCfg<LOGN, LOGT>::S_ELEMS;
     float2 *sm_tw = reinterpret_cast<float2 *>(sX + C::BUF_ELEMS);
-    for (int e = threadIdx.x; e < C::TW_ENTRIES; e += NT) sm_tw[e] = p.tw[e];
+    for (int e = threadIdx.x; e < C::TW_SMEM_ENTRIES; e += NT) sm_tw[e] = p.tw[e];
     const uint64_t pol_T = l2_policy_evict_first();
     const int tile_mask = (1 << p.log_tiles) - 1;
     float2 a[E], b[E];
@@ -524,7 +531,7 @@ fft_sky_pass1_kernel(const __grid_constant__ FusedArgs q) {
             tile_take_inputs<LOGN, LOGT>(a, b, sS);
             spin_down<LOGN, LOGT, E, false, CUBIC>(a, b, p, td, k2_0, RP::r0);
             tile_passes<LOGN, LOGT>(a, b, sX, sm_tw);
-            tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
+            tile_last_pass<LOGN, LOGT>(a, b, sm_tw, p.tw);
             store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)t * p.n_fft, k2_0, pol_T);
         }
     }
@@ -561,7 +568,7 @@ __device__ __forceinline__ void pass2_tile_loop(const FftArgs &p, float4 *sm, co
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (nxt < tile_end)
             tile_prefetch<LOGN, LOGT>(sm, p.T + (int64_t)((nxt >> p.log_tiles) - t_off) * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_T);
-        tile_last_pass<LOGN, LOGT>(a, b, sm_tw);
+        tile_last_pass<LOGN, LOGT>(a, b, sm_tw, p.tw);
         {   // epilogue: 2F[q], q = m1 + N1*m2 (consecutive lanes -> consecutive m1)
             constexpr int RL = (RP::np == 2) ? RP::r1 : RP::r2;
             constexpr int PL = (RP::np == 2) ? C::P1 : C::P2;
@@ -638,7 +645,7 @@ struct SingleCfg {
     using C1 = FftCfg<LOGN1, LOGT, 16>;
     using C2 = FftCfg<LOGN2, LOGT, 16>;
     static constexpr int BUF = C1::BUF_ELEMS > C2::BUF_ELEMS ? C1::BUF_ELEMS : C2::BUF_ELEMS;
-    static constexpr int SMEM_BYTES = BUF * 16 + (C1::TW_ENTRIES + C2::TW_ENTRIES) * 8 + 16;
+    static constexpr int SMEM_BYTES = BUF * 16 + (C1::TW_SMEM_ENTRIES + C2::TW_SMEM_ENTRIES) * 8 + 16;
     static constexpr int MIN_CTAS = (228 * 1024 / (SMEM_BYTES + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES + 1024));
 };
 
@@ -647,10 +654,10 @@ __global__ void __launch_bounds__(FftCfg<LOGN1, LOGT, 16>::NT, SingleCfg<LOGN1, 
 fft_single_kernel(const __grid_constant__ SingleArgs q) {
     using SC = SingleCfg<LOGN1, LOGN2, LOGT, VAR>;
     extern __shared__ float4 sm[];
-    float2 *tw1 = reinterpret_cast<float2 *>(sm + SC::BUF), *tw2 = tw1 + SC::C1::TW_ENTRIES;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(tw2 + SC::C2::TW_ENTRIES);
-    for (int e = threadIdx.x; e < SC::C1::TW_ENTRIES; e += SC::C1::NT) tw1[e] = q.p1.tw[e];
-    for (int e = threadIdx.x; e < SC::C2::TW_ENTRIES; e += SC::C1::NT) tw2[e] = q.p2.tw[e];
+    float2 *tw1 = reinterpret_cast<float2 *>(sm + SC::BUF), *tw2 = tw1 + SC::C1::TW_SMEM_ENTRIES;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(tw2 + SC::C2::TW_SMEM_ENTRIES);
+    for (int e = threadIdx.x; e < SC::C1::TW_SMEM_ENTRIES; e += SC::C1::NT) tw1[e] = q.p1.tw[e];
+    for (int e = threadIdx.x; e < SC::C2::TW_SMEM_ENTRIES; e += SC::C1::NT) tw2[e] = q.p2.tw[e];
     if (threadIdx.x == 0) { mbar_init(bar, 1); fence_proxy_async(); }
     __syncthreads();
     unsigned parity = 0, target = 0;

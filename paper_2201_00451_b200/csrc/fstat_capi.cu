@@ -261,9 +261,6 @@ void default_geometry(int L, PlanGeom &g) {
     // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
     // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles
     g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
-    // small transforms: 2^11-element tiles in both passes (pass 2 is indifferent, experiments section 2), the shape of
-    // the single-kernel form (both passes in one cooperative launch, same block size)
-    if (L <= 18) g.log_tile2 = 11;
     g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
 }
 
@@ -305,11 +302,13 @@ int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 // so long that the two-launch form is faster: more than 4 groups).  A group's intermediates take at most 48 MB, so
 // that two groups stay L2-resident.
 int single_group_size(fstat_plan *p, int nt, bool cubic) {
-    if (p->force_single == 0 || p->g.log_tile1 != 11 || p->g.log_tile2 != 11 || p->g.p2_elems != 16) return 0;
+    // opt-in only (fstat_debug_set_paths(single = 1) on a plan whose passes both use 2^11-element tiles): measured on B200
+    // the single-kernel form is never faster than two launches (the passes are bound on the SM side, so
+    // L2 residency of the intermediate buys nothing and every grid barrier adds a tail)
+    if (p->force_single <= 0 || p->g.log_tile1 != 11 || p->g.log_tile2 != 11 || p->g.p2_elems != 16) return 0;
     if (!fft_find_single_kernel(p->g.log_n1, p->g.log_n2, pass1_variant(p->g, cubic) & ~FFT_VAR_SKIPZ)) return 0;
     const int cap = (int)std::max<int64_t>(1, (48ll << 20) / (p->g.n_fft * 16));
     if (nt <= cap) return nt;
-    if (p->force_single < 0 && nt > 4 * cap) return 0;
     const int n_groups = (nt + cap - 1) / cap;
     return (nt + n_groups - 1) / n_groups;                  // equal groups
 }
