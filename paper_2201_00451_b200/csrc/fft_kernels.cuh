@@ -16,6 +16,11 @@
 #pragma once
 #include "fstat_common.cuh"
 #include "fft_launch.cuh"
+// Experiment switch (profiles/r02_experiments.md): FFT pass 1 with a staging buffer of its own, so that the next tile's
+// bulk copy starts as soon as the current tile's inputs are in registers.  Measured slower (3 instead of 5 CTAs per SM).
+#ifndef FFT_P1_DB
+#define FFT_P1_DB 0
+#endif
 #include "sky_math.cuh"
 
 // Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
@@ -120,6 +125,11 @@ template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     static constexpr bool TW_LAST_GLOBAL = (RadixPlan<LOGN, E>::np > 2) && (LOGN == 11);
     static constexpr int TW_SMEM_ENTRIES = TW_LAST_GLOBAL ? OFF2 : TW_ENTRIES;
     static constexpr int SMEM_BYTES = BUF_ELEMS * 16 + TW_SMEM_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
+    // pass 1 with a staging buffer of its own (FFT_P1_DB): the next tile's bulk copy starts as soon as the current tile's
+    // inputs are in registers instead of after its last exchange
+    static constexpr int P1_STAGE_ELEMS = FFT_P1_DB ? N * W : 0;
+    static constexpr int SMEM_BYTES_P1 = SMEM_BYTES + P1_STAGE_ELEMS * 16;
+    static constexpr int MIN_CTAS_P1 = FFT_P1_DB ? ((228 * 1024 / (SMEM_BYTES_P1 + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES_P1 + 1024))) : MIN_CTAS;
 };
 
 // Shared-memory exchange layout: element idx of lane w lives at 16-byte chunk
@@ -332,7 +342,9 @@ __device__ __forceinline__ void spin_down(float2 (&a)[E], float2 (&b)[E], const 
     using RP = RadixPlan<LOGN, E>;
     using PI = PassIdx<RP::r0, 1, LOGN, C::LOGW, C::NT, false>;
     const double h = (double)((int64_t)PI::NI << p.log_other) * p.dt;
-    const double c1 = td.half_fdot, c2 = td.sixth_fddot;
+    // one set of formulas for both variants (c2 = 0 folds the cubic terms away at compile time), and a template
+    // without second spin-down takes q from its descriptor in both: its 2F bits do not depend on what else is in the launch
+    const double c1 = td.half_fdot, c2 = CUBIC ? td.sixth_fddot : 0.0;
     float2 cc = make_float2(1.f, 0.f);
     if (CUBIC) cc = expm2pi(6.0 * c2 * h * h * h);
 #pragma unroll
@@ -341,17 +353,11 @@ __device__ __forceinline__ void spin_down(float2 (&a)[E], float2 (&b)[E], const 
         PI::item(bb, i, w);
         const int64_t k = ((int64_t)i << p.log_other) + k2_0 + w;
         const double tau = (double)(k - p.k_margin) * p.dt;
-        float2 e, d, q;
-        if (CUBIC) {
-            const double t3 = 3.0 * c2 * tau;
-            e = expm2pi(tau * tau * fma(c2, tau, c1));
-            d = expm2pi(h * (fma(2.0 * tau, c1, tau * t3) + h * (c1 + t3 + c2 * h)));
-            q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
-        } else {
-            e = expm2pi(tau * tau * c1);
-            d = expm2pi(h * c1 * (2.0 * tau + h));
-            q = make_float2(td.q_re, td.q_im);             // exp(-2 pi i 2 c1 h^2)
-        }
+        const double t3 = 3.0 * c2 * tau;
+        float2 e = expm2pi(tau * tau * fma(c2, tau, c1));
+        float2 d = expm2pi(h * (fma(2.0 * tau, c1, tau * t3) + h * (c1 + t3 + c2 * h)));
+        float2 q = make_float2(td.q_re, td.q_im);             // exp(-2 pi i 2 c1 h^2)
+        if (CUBIC && c2 != 0.0) q = expm2pi(h * h * (2.0 * c1 + 2.0 * t3 + 6.0 * c2 * h));
 #pragma unroll
         for (int r = 0; r < RP::r0; ++r) {
             if (SKIPZ && r >= r_nz) break;
@@ -419,7 +425,7 @@ __device__ __forceinline__ void store_columns(const float2 (&a)[E], const float2
 // intermediate of template t goes to p.T[t - t_off] (t_off != 0 only in the single-kernel form, which cycles two
 // groups of templates through an L2-resident buffer).
 template <int LOGN, int LOGT, int E, int VAR>
-__device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, const float2 *sm_tw, uint64_t *bar, unsigned &parity,
+__device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, float4 *stage, const float2 *sm_tw, uint64_t *bar, unsigned &parity,
                                                 int tile, int tile_end, int stride, int t_off, uint64_t pol_S, uint64_t pol_T) {
     constexpr bool SKIPZ = (VAR & FFT_VAR_SKIPZ) != 0, CUBIC = (VAR & FFT_VAR_CUBIC) != 0, AFFINE = (VAR & FFT_VAR_GENERIC) == 0;
     using C = FftCfg<LOGN, LOGT, E>;
@@ -434,7 +440,7 @@ __device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, co
     const int r_nz = !SKIPZ ? (int)RP::r0
         : min((int)RP::r0, (int)((((p.n_src + ((int64_t)1 << p.log_other) - 1) >> p.log_other) + (C::N / RP::r0) - 1) / (C::N / RP::r0)));
     const unsigned stage_bytes = (unsigned)min(r_nz * (C::N / RP::r0), (int)C::N) * C::W * 16u;
-    tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
+    tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
     for (; tile < tile_end; tile += stride) {
         const int t = tile >> p.log_tiles, x = tile & tile_mask;
         const TmplDesc td = td_next;
@@ -443,11 +449,16 @@ __device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, co
         if (nxt < tile_end) td_next = p.tmpl[nxt >> p.log_tiles];
         mbar_wait(bar, parity);
         parity ^= 1;
-        tile_take_inputs<LOGN, LOGT>(a, b, sm, SKIPZ ? r_nz : 32);
+        tile_take_inputs<LOGN, LOGT>(a, b, stage, SKIPZ ? r_nz : 32);
+        if (FFT_P1_DB) {
+            __syncthreads();                            // every thread has taken its inputs: the staging buffer is free
+            if (nxt < tile_end)
+                tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
+        }
         // times exp(-i Phi_s) (S9)
         spin_down<LOGN, LOGT, E, SKIPZ, CUBIC>(a, b, p, td, k2_0, r_nz);
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
-        if (nxt < tile_end)
+        if (!FFT_P1_DB && nxt < tile_end)
             tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
         tile_last_pass<LOGN, LOGT>(a, b, sm_tw, p.tw);
         store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)(t - t_off) * p.n_fft, k2_0, pol_T);
@@ -466,13 +477,14 @@ __device__ __forceinline__ void pass_smem_setup(const FftArgs &p, float4 *sm, fl
 }
 
 template <int LOGN, int LOGT, int E, int VAR>
-__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS_P1)
 fft_pass1_kernel(const __grid_constant__ FftArgs p) {
     extern __shared__ float4 sm[];
     float2 *sm_tw; uint64_t *bar;
     pass_smem_setup<LOGN, LOGT, E>(p, sm, sm_tw, bar);
     unsigned parity = 0;
-    pass1_tile_loop<LOGN, LOGT, E, VAR>(p, sm, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_last(), l2_policy_evict_first());
+    float4 *stage = FFT_P1_DB ? reinterpret_cast<float4 *>(reinterpret_cast<char *>(sm) + FftCfg<LOGN, LOGT, E>::SMEM_BYTES) : sm;
+    pass1_tile_loop<LOGN, LOGT, E, VAR>(p, sm, stage, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_last(), l2_policy_evict_first());
 }
 
 // ---------------------------------------------------------------------------------------
@@ -645,7 +657,8 @@ struct SingleCfg {
     using C1 = FftCfg<LOGN1, LOGT, 16>;
     using C2 = FftCfg<LOGN2, LOGT, 16>;
     static constexpr int BUF = C1::BUF_ELEMS > C2::BUF_ELEMS ? C1::BUF_ELEMS : C2::BUF_ELEMS;
-    static constexpr int SMEM_BYTES = BUF * 16 + (C1::TW_SMEM_ENTRIES + C2::TW_SMEM_ENTRIES) * 8 + 16;
+    static constexpr int SMEM_CORE = BUF * 16 + (C1::TW_SMEM_ENTRIES + C2::TW_SMEM_ENTRIES) * 8 + 16;
+    static constexpr int SMEM_BYTES = SMEM_CORE + C1::P1_STAGE_ELEMS * 16;
     static constexpr int MIN_CTAS = (228 * 1024 / (SMEM_BYTES + 1024)) > 5 ? 5 : (228 * 1024 / (SMEM_BYTES + 1024));
 };
 
@@ -666,7 +679,7 @@ fft_single_kernel(const __grid_constant__ SingleArgs q) {
     for (int g = 0, t0 = 0; t0 < q.n_tmpl; ++g, t0 += q.group) {
         const int t1 = min(t0 + q.group, q.n_tmpl);
         const int t_off = t0 - (g & 1) * q.group;            // template t of this group lives at T[t - t_off]
-        pass1_tile_loop<LOGN1, LOGT, 16, VAR>(q.p1, sm, tw1, bar, parity, t0 * tiles1 + (int)blockIdx.x, t1 * tiles1, (int)gridDim.x, t_off, pol_keep, pol_keep);
+        pass1_tile_loop<LOGN1, LOGT, 16, VAR>(q.p1, sm, FFT_P1_DB ? reinterpret_cast<float4 *>(reinterpret_cast<char *>(sm) + SC::SMEM_CORE) : sm, tw1, bar, parity, t0 * tiles1 + (int)blockIdx.x, t1 * tiles1, (int)gridDim.x, t_off, pol_keep, pol_keep);
         grid_barrier(q.counter, target);
         pass2_tile_loop<LOGN2, LOGT, 16>(q.p2, sm, tw2, bar, parity, t0 * tiles2 + (int)blockIdx.x, t1 * tiles2, (int)gridDim.x, t_off, pol_keep);
     }

@@ -11,7 +11,7 @@ namespace {
 template <int LOGN, int LOGT, bool P2, int E, int VAR>
 cudaError_t launch_pass(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, int n_t) {
     using C = FftCfg<LOGN, LOGT, E>;
-    constexpr int SMEM = C::SMEM_BYTES;
+    constexpr int SMEM = P2 ? C::SMEM_BYTES : C::SMEM_BYTES_P1;
     static thread_local int configured_dev = -1;
     static thread_local int resident = 0;
     auto kern = fft_kernel_ptr<LOGN, LOGT, P2, E, VAR>();
