@@ -22,6 +22,9 @@
 #define FFT_P1_DB 0
 #endif
 #include "sky_math.cuh"
+#ifndef FFT_CTAS11
+#define FFT_CTAS11 5
+#endif
 
 // Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
 // a register pair holds (Re Fa, Re Fb) or (Im Fa, Im Fb) and every add / multiply / FMA is one
@@ -109,7 +112,7 @@ template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     static_assert(LOGT >= LOGN && LOGT >= 11 && LOGT <= 13, "tile must hold at least one sub-FFT");
     static constexpr int LOGW = LOGT - LOGN;
     static constexpr int W = 1 << LOGW;
-    static constexpr int MIN_CTAS = (E == 32) ? (LOGT == 13 ? 1 : 3) : (LOGT == 11) ? 5 : (LOGT == 12) ? 2 : 1;
+    static constexpr int MIN_CTAS = (E == 32) ? (LOGT == 13 ? 1 : 3) : (LOGT == 11) ? FFT_CTAS11 : (LOGT == 12) ? 2 : 1;
     static constexpr int N = 1 << LOGN;
     static constexpr int NT = (N * W) / E;
     // twiddle table offsets (float2 entries): pass s >= 1 holds (R_s - 1) * P_s entries, [r-1][k]

@@ -406,8 +406,10 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked, 
     ProfScope ps(p, 0);
     int rc = launch_timing_nodes(p, g0, ng);
     if (rc) return rc;
-    dim3 grid((unsigned)((g.n_src + SKY_THREADS - 1) / SKY_THREADS), ng);
-    sky_resample_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask);
+    const int n_kblocks = (int)((g.n_src + SKY_THREADS * SKY_PTS - 1) / (SKY_THREADS * SKY_PTS));
+    // sky position fastest when the Farrow-filtered series would not stay in L2 between sky positions
+    const int sky_major = ng > 1 && (size_t)g.n_det * (FARROW_NC / 2) * (size_t)(g.n_samples + 1) * sizeof(float4) > ((size_t)48 << 20);
+    sky_resample_kernel<<<(unsigned)n_kblocks * (unsigned)ng, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask, ng, n_kblocks, sky_major);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;

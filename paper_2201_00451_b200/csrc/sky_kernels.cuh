@@ -64,26 +64,68 @@ sidereal_table_kernel(PlanGeom g, float2 *__restrict__ rot) {
     rot[k] = make_float2((float)c, (float)s);
 }
 
-// The hoisted form of the sky-dependent half: one SSB grid point per thread, S written once per sky position and
-// re-read by every spin-down template (long fdot banks).  grid = (ceil(n_src/256), n_sky).
+// The hoisted form of the sky-dependent half: S written once per sky position and re-read by every spin-down template
+// (long fdot banks).  A block works on SKY_PTS * 256 consecutive SSB grid points of one sky position, a thread on
+// SKY_PTS of them 256 apart (coalesced): what depends on (sky position, detector) only -- antenna coefficients, table
+// bases -- is loaded once per thread for the first detector pair instead of once per grid point.
+// Block order: sky_major != 0 lets the sky position vary fastest, so that the blocks running at the same time cover
+// the same stretch of the SSB grid for all sky positions of the batch and read the same stretch (+- the spread of the
+// delays) of the Farrow-filtered series, which then comes from HBM once per batch instead of once per sky position
+// (used when that table exceeds what the L2 holds: 276 MB at config-2 size); otherwise the grid index varies fastest.
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
 //            S[k2 / W1][k1][k2 % W1]
-__global__ void __launch_bounds__(SKY_THREADS)
+#ifndef SKY_PTS
+#define SKY_PTS 4
+#endif
+#ifndef SKY_MIN_BLOCKS
+#define SKY_MIN_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(SKY_THREADS, SKY_MIN_BLOCKS)
 sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ nodes,
                     const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
-                    float4 *__restrict__ S, int blocked, uint32_t det_mask) {
-    const int k = blockIdx.x * SKY_THREADS + threadIdx.x;          // n_src <= n_fft <= 2^24
-    if (k >= g.n_src) return;
-    float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
-    sky_point(g, skies[blockIdx.y], nodes + (int64_t)blockIdx.y * g.n_det * g.n_nodes, rot, Y, wslot, k, det_mask, ya, yb);
-    int off = k;
-    if (blocked) {
-        const int k1 = k >> g.log_n2, k2 = k & ((1 << g.log_n2) - 1);
-        off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
+                    float4 *__restrict__ S, int blocked, uint32_t det_mask, int n_sky, int n_kblocks, int sky_major) {
+    const int sky = sky_major ? (int)(blockIdx.x % (unsigned)n_sky) : (int)(blockIdx.x / (unsigned)n_kblocks);
+    const int kb = sky_major ? (int)(blockIdx.x / (unsigned)n_sky) : (int)(blockIdx.x % (unsigned)n_kblocks);
+    const int k0 = kb * (SKY_THREADS * SKY_PTS) + threadIdx.x;          // n_src <= n_fft <= 2^24
+    const SkyConst &sc = skies[sky];
+    const double4 *nd = nodes + (int64_t)sky * g.n_det * g.n_nodes;
+    const int n_rows = (int)g.n_samples + 1;
+    float4 *Ss = S + (int64_t)sky * g.n_fft;
+    // the first detector pair (all there is in the two-detector configurations) hoisted out of the loop over grid points
+    const SkyDetConst d0 = sky_det_const(g, sc, nd, Y, wslot, 0, det_mask);
+    const SkyDetConst d1 = sky_det_const(g, sc, nd, Y, wslot, 1, det_mask);
+#pragma unroll 1
+    for (int i = 0; i < SKY_PTS; ++i) {
+        const int k = k0 + i * SKY_THREADS;
+        if (k >= g.n_src) break;
+        float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
+        const SkyPointCommon c = sky_point_common(g, rot, k);
+        {
+            const SkyDetPoint o0 = sky_det_point(g, d0, c), o1 = sky_det_point(g, d1, c);
+            float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
+            sky_det_load(o0, n_rows, c0);
+            sky_det_load(o1, n_rows, c1);
+            sky_det_finish(o0, c0, ya, yb);
+            sky_det_finish(o1, c1, ya, yb);
+        }
+        for (int X0 = 2; X0 < g.n_det; X0 += 2) {
+            const SkyDetPoint o0 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0, det_mask), c);
+            const SkyDetPoint o1 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0 + 1, det_mask), c);
+            float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
+            sky_det_load(o0, n_rows, c0);
+            sky_det_load(o1, n_rows, c1);
+            sky_det_finish(o0, c0, ya, yb);
+            sky_det_finish(o1, c1, ya, yb);
+        }
+        int off = k;
+        if (blocked) {
+            const int k1 = k >> g.log_n2, k2 = k & ((1 << g.log_n2) - 1);
+            off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
+        }
+        // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
+        Ss[off] = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
     }
-    // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
-    S[(int64_t)blockIdx.y * g.n_fft + off] = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
 }
 
 // A, B, C (eq. 8, S11): sums of w a^2, w b^2, w a b over the valid detector-frame

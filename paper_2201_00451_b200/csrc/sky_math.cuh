@@ -69,7 +69,13 @@ __device__ __forceinline__ double ssb_invert_newton(const PlanGeom &g, const Sky
 }
 
 #define SKY_THREADS 256
-#define FARROW_NC 10          // polynomial coefficients per tap (degree 9: 8e-8 max error for Dterms >= 8, 3e-7 for Dterms 1)
+// polynomial coefficients per tap weight.  Degree 7: the folded taps differ from the exact windowed-sinc weights by 2e-6
+// (root sum of squares over the taps; 7e-6 if all errors add up) for Dterms >= 8 and 2e-5 for Dterms 1, against a
+// tolerance of 1e-3 on 2F; degree 9 (10 coefficients, 80 B per sample and detector) gives 1e-8 and costs 25 % more table
+// traffic in the kernel that bounds sky-varying searches.
+#ifndef FARROW_NC
+#define FARROW_NC 8
+#endif
 
 // ---- H1 on a coarse node grid --------------------------------------------------------------------------------
 // The delay Delta(tau) = tau - T(tau) is smooth (sidereal rotation: 21 ms amplitude, one-day period; orbit: 499 s, one
@@ -94,85 +100,152 @@ __device__ __forceinline__ void timing_node(const PlanGeom &g, const SkyConst &s
     const double dp = g.omega_orb * (sc.Ps * co - sc.Pc * so) + g.omega_rot * (sc.Qs[X] * cth - sc.Qc[X] * sth);
     slope = dp / (1.0 + dp);
 }
-// H1-H5 for SSB grid point k: adds the detectors' contributions to (ya, yb) = (Fa(t), Fb(t)) before the spin-down factor.
+// ---- H1-H5 per SSB grid point, in pieces that the two forms of the sky-dependent half arrange differently ----------
+// (hoisted kernel: detector pairs outside, grid points inside, so that everything that depends on the sky position and
+// the detector only is loaded once per thread; fused kernel: one grid point at a time).
 //   nodes  : [n_det][n_nodes] double4 of this sky position (timing_nodes_kernel)
 //   rot    : [n_src] float2 from sidereal_table_kernel
 //   Y      : [n_det][FARROW_NC/2][N+1] float4, the Farrow-filtered series
 //   wslot  : [n_det][n_slots] float, 0 in gaps
-//   det_mask : bit X set = detector X contributes
-// Detectors are taken two at a time: the timing of both first, then the 2 x 80 bytes of Farrow coefficients are requested
-// together (these L2 reads are what the thread waits for), then the two Horner recurrences, phase factors and
-// antenna weights.  fp64 only for Delta, the fractional sample index and the heterodyne phase.
-__device__ __forceinline__ void sky_point(const PlanGeom &g, const SkyConst &sc, const double4 *__restrict__ nodes,
-                                          const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
-                                          int k, uint32_t det_mask, float2 &ya, float2 &yb) {
-    const int krel = k - (int)g.k_margin;
-    const double tau = (double)krel * g.dt;
-    const int nn = k >> g.log_node;
-    const double theta = (double)(k & ((1 << g.log_node) - 1)) * g.inv_node;
-    const float2 cs = __ldg(rot + k);
+// fp64 only for Delta, the fractional sample index and the heterodyne phase.  Roundings to integers are done by
+// adding 1.5 * 2^52 (fp64 pipe) or 1.5 * 2^23 (fp32) instead of the conversion instructions of the XU pipe.
+#define SKY_MAGIC64 6755399441055744.0
+#define SKY_MAGIC32 12582912.0f
+
+// what a grid point contributes to every detector
+struct SkyPointCommon {
+    int krel;           // k - K_m
+    int nn;             // timing node
+    double tau;         // SSB time - t_start
+    double theta;       // position between the nodes, [0, 1)
+    float2 cs;          // cos, sin of the Greenwich sidereal angle at tau
+    float shift_cyc;    // band placement ramp (cycles)
+};
+
+__device__ __forceinline__ SkyPointCommon sky_point_common(const PlanGeom &g, const float2 *__restrict__ rot, int k) {
+    SkyPointCommon c;
+    c.krel = k - (int)g.k_margin;
+    c.tau = (double)c.krel * g.dt;
+    c.nn = k >> g.log_node;
+    c.theta = (double)(k & ((1 << g.log_node) - 1)) * g.inv_node;
+    c.cs = __ldg(rot + k);
     // band placement: output bin q must land on FFT index q -> multiply by exp(-2 pi i s k / n_fft);
     // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32);
     // + the residual fraction of a bin when f_het is off the bin grid: |value| <= 1/2, k < 2^24 exact in fp32 (error 6e-8 cycles)
     const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
-    const float shift_cyc = fmaf((float)k, g.shift_frac_per_k, (float)tshift * (1.0f / (float)g.n_fft));
-    const int n_rows = (int)g.n_samples + 1;
-
-    for (int X0 = 0; X0 < g.n_det; X0 += 2) {
-        float w[2], d[2], fc[2], ca[2], cb[2];
-        const float4 *y[2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const int X = min(X0 + u, g.n_det - 1);
-            const double2 *np = reinterpret_cast<const double2 *>(nodes + (int64_t)X * g.n_nodes + nn);
-            const double2 n0 = __ldg(np), n1 = __ldg(np + 1);
-            const double delta = fma(theta, fma(theta, fma(theta, n1.y, n1.x), n0.y), n0.x);
-            const double T = tau - delta;                       // detector epoch - t_start
-            w[u] = 0.f;
-            // step 3: inside the data and not in a gap (det_mask: the detectors that take part -- all of them, or one
-            // for the single-detector statistic)
-            if (X0 + u < g.n_det && ((det_mask >> X) & 1u) && T >= 0.0 && T < g.span) {
-                const int slot = min((int)(T * g.inv_t_sft), g.n_slots - 1);
-                w[u] = wslot[X * g.n_slots + slot];
-            }
-            // fractional sample index u = krel - Delta/dt = j0 + d,  d in [-1/2, 1/2)
-            const double v = -delta * g.inv_dt;
-            const double vr = floor(v + 0.5);
-            d[u] = (float)(v - vr);
-            const int j0 = min(max(krel + (int)vr, 0), n_rows - 1);   // in [0, N] whenever w != 0
-            y[u] = reinterpret_cast<const float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * n_rows + j0;
-            // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
-            // (phase reduced mod 1 in fp64, then fp32)
-            const double cyc = g.f_het * delta;
-            fc[u] = (float)(cyc - floor(cyc)) + shift_cyc;
-            // sidereal angle at T: rotate the table value by e = omega_rot Delta (|e| < 0.05: Taylor to 1e-9)
-            const float e = (float)(g.omega_rot * delta), e2 = e * e;
-            const float se = e * fmaf(e2, fmaf(e2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
-            const float ce = fmaf(e2, fmaf(e2, 1.0f / 24.0f, -0.5f), 1.0f);
-            antenna_ab(sc, X, cs.x * ce + cs.y * se, cs.y * ce - cs.x * se, ca[u], cb[u]);
-        }
-        float4 c[2][FARROW_NC / 2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u)
-#pragma unroll
-            for (int p = 0; p < FARROW_NC / 2; ++p) c[u][p] = __ldg(y[u] + (int64_t)p * n_rows);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
-            const float2 dd = make_float2(d[u], d[u]);
-            float2 z = make_float2(c[u][FARROW_NC / 2 - 1].z, c[u][FARROW_NC / 2 - 1].w);
-#pragma unroll
-            for (int p = FARROW_NC / 2 - 1; p >= 0; --p) {
-                if (p < FARROW_NC / 2 - 1) z = __ffma2_rn(z, dd, make_float2(c[u][p].z, c[u][p].w));
-                z = __ffma2_rn(z, dd, make_float2(c[u][p].x, c[u][p].y));
-            }
-            float f = fc[u] - rintf(fc[u]), sp, cp;             // |arg| <= pi, where sin/cos.approx are good to 5e-7 abs
-            __sincosf(-6.283185307179586f * f, &sp, &cp);
-            const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
-            const float wa = w[u] * ca[u], wb = w[u] * cb[u];
-            ya.x = fmaf(wa, er, ya.x); ya.y = fmaf(wa, ei, ya.y);
-            yb.x = fmaf(wb, er, yb.x); yb.y = fmaf(wb, ei, yb.y);
-        }
-    }
+    c.shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
+    if (g.shift_frac_per_k != 0.f) c.shift_cyc = fmaf((float)k, g.shift_frac_per_k, c.shift_cyc);
+    return c;
 }
 
+// what depends on (sky position, detector) only
+struct SkyDetConst {
+    float cal, sal, ac[5], bc[4];
+    const double4 *nodes;   // this detector's timing nodes
+    const float4 *y;        // this detector's Farrow-filtered series
+    const float *w;         // this detector's slot weights
+    bool on;                // takes part (exists and selected by det_mask)
+};
+
+__device__ __forceinline__ SkyDetConst sky_det_const(const PlanGeom &g, const SkyConst &sc, const double4 *__restrict__ nodes,
+                                                     const float2 *__restrict__ Y, const float *__restrict__ wslot, int Xu, uint32_t det_mask) {
+    const int X = min(Xu, g.n_det - 1);
+    SkyDetConst d;
+    d.cal = sc.cal[X]; d.sal = sc.sal[X];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) d.ac[q] = sc.ac[X][q];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) d.bc[q] = sc.bc[X][q];
+    d.nodes = nodes + (int64_t)X * g.n_nodes;
+    d.y = reinterpret_cast<const float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * (g.n_samples + 1);
+    d.w = wslot + (int64_t)X * g.n_slots;
+    d.on = Xu < g.n_det && ((det_mask >> X) & 1u);
+    return d;
+}
+
+// per (grid point, detector), before the Farrow coefficients are needed
+struct SkyDetPoint {
+    float w, d, fc, ca, cb;
+    const float4 *y;        // Y_0,1 of sample j0; the other chunks follow n_rows apart
+};
+
+__device__ __forceinline__ SkyDetPoint sky_det_point(const PlanGeom &g, const SkyDetConst &dc, const SkyPointCommon &c) {
+    SkyDetPoint o;
+    const double2 *np = reinterpret_cast<const double2 *>(dc.nodes + c.nn);
+    const double2 n0 = __ldg(np), n1 = __ldg(np + 1);
+    const double delta = fma(c.theta, fma(c.theta, fma(c.theta, n1.y, n1.x), n0.y), n0.x);
+    const double T = c.tau - delta;                       // detector epoch - t_start
+    o.w = 0.f;
+    // step 3: inside the data and not in a gap (dc.on: the detectors that take part -- all of them, or one for the
+    // single-detector statistic)
+    if (dc.on && T >= 0.0 && T < g.span) {
+        const int slot = min(__double2loint(__dadd_rd(T * g.inv_t_sft, SKY_MAGIC64)), g.n_slots - 1);    // floor
+        o.w = dc.w[slot];
+    }
+    // fractional sample index u = krel - Delta/dt = j0 + d,  j0 = floor(u + 1/2), d in [-1/2, 1/2)
+    const double v = -delta * g.inv_dt;
+    const double vm = __dadd_rd(v + 0.5, SKY_MAGIC64);
+    o.d = (float)(v - (vm - SKY_MAGIC64));
+    const int n_rows = (int)g.n_samples + 1;
+    const int j0 = min(max(c.krel + __double2loint(vm), 0), n_rows - 1);   // in [0, N] whenever w != 0
+    o.y = dc.y + j0;
+    // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
+    // (phase reduced mod 1 in fp64, then fp32)
+    const double cyc = g.f_het * delta;
+    o.fc = (float)(cyc - ((cyc + SKY_MAGIC64) - SKY_MAGIC64)) + c.shift_cyc;
+    // sidereal angle at T: rotate the table value by e = omega_rot Delta (|e| < 0.05: Taylor to 1e-9)
+    const float e = (float)(g.omega_rot * delta), e2 = e * e;
+    const float se = e * fmaf(e2, fmaf(e2, 1.0f / 120.0f, -1.0f / 6.0f), 1.0f);
+    const float ce = fmaf(e2, fmaf(e2, 1.0f / 24.0f, -0.5f), 1.0f);
+    // H2: a(t), b(t) from cos/sin of the sidereal angle (fp32), as antenna_ab
+    const float cth = c.cs.x * ce + c.cs.y * se, sth = c.cs.y * ce - c.cs.x * se;
+    const float ch = dc.cal * cth + dc.sal * sth;
+    const float sh = dc.sal * cth - dc.cal * sth;
+    const float c2 = 2.f * ch * ch - 1.f, s2 = 2.f * sh * ch;
+    o.ca = dc.ac[0] + dc.ac[1] * c2 + dc.ac[2] * s2 + dc.ac[3] * ch + dc.ac[4] * sh;
+    o.cb = dc.bc[0] * c2 + dc.bc[1] * s2 + dc.bc[2] * ch + dc.bc[3] * sh;
+    return o;
+}
+
+__device__ __forceinline__ void sky_det_load(const SkyDetPoint &o, int n_rows, float4 (&c)[FARROW_NC / 2]) {
+#pragma unroll
+    for (int p = 0; p < FARROW_NC / 2; ++p) c[p] = __ldg(o.y + (int64_t)p * n_rows);
+}
+
+__device__ __forceinline__ void sky_det_finish(const SkyDetPoint &o, const float4 (&c)[FARROW_NC / 2], float2 &ya, float2 &yb) {
+    // z = sum_p d^p Y_p[j0] (Horner, packed re/im)
+    const float2 dd = make_float2(o.d, o.d);
+    float2 z = make_float2(c[FARROW_NC / 2 - 1].z, c[FARROW_NC / 2 - 1].w);
+#pragma unroll
+    for (int p = FARROW_NC / 2 - 1; p >= 0; --p) {
+        if (p < FARROW_NC / 2 - 1) z = __ffma2_rn(z, dd, make_float2(c[p].z, c[p].w));
+        z = __ffma2_rn(z, dd, make_float2(c[p].x, c[p].y));
+    }
+    float f = o.fc - ((o.fc + SKY_MAGIC32) - SKY_MAGIC32), sp, cp;      // |arg| <= pi, where sin/cos.approx are good to 5e-7 abs
+    __sincosf(-6.283185307179586f * f, &sp, &cp);
+    const float er = z.x * cp - z.y * sp, ei = z.x * sp + z.y * cp;
+    const float wa = o.w * o.ca, wb = o.w * o.cb;
+    ya.x = fmaf(wa, er, ya.x); ya.y = fmaf(wa, ei, ya.y);
+    yb.x = fmaf(wb, er, yb.x); yb.y = fmaf(wb, ei, yb.y);
+}
+
+// H1-H5 for SSB grid point k: adds the detectors' contributions to (ya, yb) = (Fa(t), Fb(t)) before the spin-down factor.
+// Detectors are taken two at a time: the timing of both first, then the 2 x 80 bytes of Farrow coefficients are requested
+// together (these L2 reads are what the thread waits for), then the two Horner recurrences, phase factors and
+// antenna weights.
+__device__ __forceinline__ void sky_point(const PlanGeom &g, const SkyConst &sc, const double4 *__restrict__ nodes,
+                                          const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
+                                          int k, uint32_t det_mask, float2 &ya, float2 &yb) {
+    const SkyPointCommon c = sky_point_common(g, rot, k);
+    const int n_rows = (int)g.n_samples + 1;
+    for (int X0 = 0; X0 < g.n_det; X0 += 2) {
+        SkyDetPoint o[2];
+        float4 cf[2][FARROW_NC / 2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) o[u] = sky_det_point(g, sky_det_const(g, sc, nodes, Y, wslot, X0 + u, det_mask), c);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) sky_det_load(o[u], n_rows, cf[u]);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) sky_det_finish(o[u], cf[u], ya, yb);
+    }
+}
