@@ -45,9 +45,11 @@ FSTAT_API int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slot
 
 /* Which path serves sky-varying banks / small FFTs: -1 = automatic (default), 0 = off, 1 = forced where supported.
  *   fused_sky : per-sky work (H1-H5) inside the FFT pass-1 prologue instead of the hoisted sky kernel + S buffer
- *               (PAPER.md:188, :293 sky-varying searches).  Automatic = off: measured slower on B200.
+ *               (PAPER.md:188, :293 sky-varying searches); needs pass 1 on tiles of >= 2^11 elements
+ *               (fstat_debug_set_geometry(-1, 11, -1, -1) where the default is the one-warp 2^10-element tile).
+ *               Automatic = off: measured slower on B200.
  *   single    : one cooperative kernel for both FFT passes of groups of templates whose four-step intermediate
- *               stays in L2 (n_fft <= 2^18, both passes on 2^11-element tiles: fstat_debug_set_geometry(-1, -1, 11, -1)).
+ *               stays in L2 (n_fft <= 2^18, both passes on 2^11-element tiles: fstat_debug_set_geometry(-1, 11, 11, -1)).
  *               Automatic = off: measured never faster than the two-launch form on B200. */
 FSTAT_API int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single);
 

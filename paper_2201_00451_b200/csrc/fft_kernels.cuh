@@ -25,6 +25,9 @@
 #ifndef FFT_CTAS11
 #define FFT_CTAS11 5
 #endif
+#ifndef FFT_CTAS_WARP
+#define FFT_CTAS_WARP 11
+#endif
 
 // Packed arithmetic.  Fa and Fb go through identical butterflies with identical twiddles, so
 // a register pair holds (Re Fa, Re Fb) or (Im Fa, Im Fb) and every add / multiply / FMA is one
@@ -109,10 +112,11 @@ __host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c
 // LOGT = 11 (128 threads, 32 KB, 4 CTAs per SM) or 12 (256 threads, 64 KB, 2 CTAs per SM); sub-FFTs of
 // length 2^12 use LOGT = 13 (two per tile, so that the other pass still gets 32-byte store runs).
 template <int LOGN, int LOGT, int E = 16> struct FftCfg {
-    static_assert(LOGT >= LOGN && LOGT >= 11 && LOGT <= 13, "tile must hold at least one sub-FFT");
+    static_assert(LOGT >= LOGN && LOGT >= 10 && LOGT <= 13, "tile must hold at least one sub-FFT");
     static constexpr int LOGW = LOGT - LOGN;
     static constexpr int W = 1 << LOGW;
-    static constexpr int MIN_CTAS = (E == 32) ? (LOGT == 13 ? 1 : 3) : (LOGT == 11) ? FFT_CTAS11 : (LOGT == 12) ? 2 : 1;
+    // LOGT = 10 with 32 elements per thread: one warp per CTA works on one 2^10-point column (no cross-warp barrier at all)
+    static constexpr int MIN_CTAS = (E == 32) ? (LOGT == 13 ? 1 : LOGT == 10 ? FFT_CTAS_WARP : 3) : (LOGT == 11) ? FFT_CTAS11 : (LOGT == 12) ? 2 : 1;
     static constexpr int N = 1 << LOGN;
     static constexpr int NT = (N * W) / E;
     // twiddle table offsets (float2 entries): pass s >= 1 holds (R_s - 1) * P_s entries, [r-1][k]
@@ -126,7 +130,9 @@ template <int LOGN, int LOGT, int E = 16> struct FftCfg {
     // shared memory: one more CTA per SM with 2^11-element tiles (measured +1 %; at 2^12 points a third CTA per SM costs
     // more in registers than it gains)
     static constexpr bool TW_LAST_GLOBAL = (RadixPlan<LOGN, E>::np > 2) && (LOGN == 11);
-    static constexpr int TW_SMEM_ENTRIES = TW_LAST_GLOBAL ? OFF2 : TW_ENTRIES;
+    // one-warp CTAs read every twiddle from global memory through L1 (the 8 KB table per warp would halve the warps per SM)
+    static constexpr bool TW_ALL_GLOBAL = (NT == 32);
+    static constexpr int TW_SMEM_ENTRIES = TW_ALL_GLOBAL ? 0 : TW_LAST_GLOBAL ? OFF2 : TW_ENTRIES;
     static constexpr int SMEM_BYTES = BUF_ELEMS * 16 + TW_SMEM_ENTRIES * 8 + 16;   // exchange buffer + twiddle table + mbarrier
     // pass 1 with a staging buffer of its own (FFT_P1_DB): the next tile's bulk copy starts as soon as the current tile's
     // inputs are in registers instead of after its last exchange
@@ -328,7 +334,8 @@ template <int LOGN, int LOGT, int E>
 __device__ __forceinline__ void tile_last_pass(float2 (&a)[E], float2 (&b)[E], const float2 *__restrict__ tw, const float2 *__restrict__ tw_g) {
     using C = FftCfg<LOGN, LOGT, E>;
     using RP = RadixPlan<LOGN, E>;
-    if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
+    if (RP::np == 2 && C::TW_ALL_GLOBAL) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false, E, true>(a, b, tw_g + C::OFF1);
+    else if (RP::np == 2) pass_compute<RP::r1, C::P1, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF1);
     else if (C::TW_LAST_GLOBAL) pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false, E, true>(a, b, tw_g + C::OFF2);
     else pass_compute<RP::r2, C::P2, LOGN, C::LOGW, C::NT, false>(a, b, tw + C::OFF2);
 }

@@ -119,9 +119,13 @@ single_launch_fn fft_find_single_kernel(int logn1, int logn2, int var) {
 fft_launch_fn FFT_CAT(fft_find_kernel_unit, FFT_UNIT)(int pass, int logn, int logt, int elems, int var) {
 #if FFT_UNIT == 0      // pass 1, sub-FFT 2^6 .. 2^9
     K1(6, 11) K1(7, 11) K1(8, 11) K1(9, 11) K1(6, 12) K1(7, 12) K1(8, 12) K1(9, 12)
+    K(1, 9, 10, 32, 0) K(1, 9, 10, 32, FFT_VAR_CUBIC)                      // one warp per two 2^9-point columns
+    K(1, 9, 10, 32, FFT_VAR_GENERIC) K(1, 9, 10, 32, FFT_VAR_GENERIC | FFT_VAR_CUBIC)
     K1G(6, 11) K1G(7, 11) K1G(8, 11) K1G(6, 12) K1G(7, 12) K1G(8, 12)
 #elif FFT_UNIT == 1    // pass 1, sub-FFT 2^10, 2^11
     K1(10, 11) K1(10, 12) K1(10, 13) K1Z(10, 11)
+    K(1, 10, 10, 32, 0) K(1, 10, 10, 32, FFT_VAR_CUBIC)                    // one warp per 2^10-point column, two radix-32 passes
+    K(1, 10, 10, 32, FFT_VAR_GENERIC) K(1, 10, 10, 32, FFT_VAR_GENERIC | FFT_VAR_CUBIC)
     K1(11, 11) K1(11, 12) K1(11, 13) K1Z(11, 11) K1Z(11, 12)
 #elif FFT_UNIT == 2    // pass 1, sub-FFT 2^12
     K1(12, 12) K1(12, 13) K1Z(12, 12) K1Z(12, 13)

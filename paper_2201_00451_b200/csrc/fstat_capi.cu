@@ -248,7 +248,7 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out, uin
 // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
 // 2^11-element tiles.
 void default_geometry(int L, PlanGeom &g) {
-    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L <= 19 ? 8 : L <= 21 ? 10 : L == 22 ? 10 : L - 12;
+    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L == 18 ? 8 : L == 19 ? 9 : L <= 21 ? 10 : L == 22 ? 10 : L - 12;
     g.log_n1 = L - g.log_n2;
     // pass 2: 2^12-element tiles; 2^13 (8 rows of 2^10 points: 128-byte runs in pass 1's transposed store, 32-byte
     // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2; likewise 4 rows
@@ -257,10 +257,12 @@ void default_geometry(int L, PlanGeom &g) {
     // pass 1: the smallest tile (most CTAs per SM) whose transposed store still writes >= 64-byte runs: a tile
     // of a single column needs >= 4 rows per pass-2 tile
     const int w2_rows = 1 << (g.log_tile2 - g.log_n2);
-    g.log_tile1 = g.log_n1 <= 10 ? 11 : (w2_rows >= 4 ? g.log_n1 : g.log_n1 + 1);
+    // 2^9 / 2^10-point columns: one warp per 2^10-element tile, 32 register elements per thread (two radix passes, no block barrier)
+    g.log_tile1 = (g.log_n1 == 9 || g.log_n1 == 10) ? 10 : g.log_n1 <= 10 ? 11 : (w2_rows >= 4 ? g.log_n1 : g.log_n1 + 1);
     // pass 2 with 32 register elements per thread (two radix-32 passes, one trip through shared memory) for
     // sub-FFTs of 2^9 and 2^10 points on 2^12-element (2^10 also 2^13-element) tiles
     g.p2_elems = (((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 == 12) || (g.log_n2 == 10 && g.log_tile2 == 13)) ? 32 : 16;
+    g.p1_elems = g.log_tile1 == 10 ? 32 : 16;
     g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
 }
 
@@ -268,20 +270,20 @@ void default_geometry(int L, PlanGeom &g) {
 // neither stages nor touches the padding (where one is instantiated); a pass-2 tile with more rows than the last radix
 // pass of pass 1 has butterflies needs the general store address; cubic = the launch holds templates with fddot != 0
 int pass1_variant(const PlanGeom &g, bool cubic) {
-    const std::vector<int> rl = radix_list(g.log_n1);
+    const std::vector<int> rl = radix_list(g.log_n1, g.p1_elems);
     const int ni_last = (1 << g.log_n1) / rl.back();
     int var = (cubic ? FFT_VAR_CUBIC : 0) | ((ni_last >> g.log_w2) == 0 ? FFT_VAR_GENERIC : 0);
-    if (2 * g.n_src <= g.n_fft && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, var | FFT_VAR_SKIPZ)) var |= FFT_VAR_SKIPZ;
+    if (2 * g.n_src <= g.n_fft && fft_find_kernel(1, g.log_n1, g.log_tile1, g.p1_elems, var | FFT_VAR_SKIPZ)) var |= FFT_VAR_SKIPZ;
     return var;
 }
 bool geometry_supported(const PlanGeom &g) {
-    return fft_find_kernel(1, g.log_n1, g.log_tile1, 16, pass1_variant(g, false)) && fft_find_kernel(1, g.log_n1, g.log_tile1, 16, pass1_variant(g, true))
+    return fft_find_kernel(1, g.log_n1, g.log_tile1, g.p1_elems, pass1_variant(g, false)) && fft_find_kernel(1, g.log_n1, g.log_tile1, g.p1_elems, pass1_variant(g, true))
         && fft_find_kernel(2, g.log_n2, g.log_tile2, g.p2_elems, 0);
 }
 
 // (re)upload the Stockham twiddle tables of the plan's current geometry
 int upload_twiddles(fstat_plan *p) {
-    const std::vector<float2> tw1 = make_twiddles(p->g.log_n1), tw2 = make_twiddles(p->g.log_n2, p->g.p2_elems);
+    const std::vector<float2> tw1 = make_twiddles(p->g.log_n1, p->g.p1_elems), tw2 = make_twiddles(p->g.log_n2, p->g.p2_elems);
     cudaFree(p->d_tw1); cudaFree(p->d_tw2); p->d_tw1 = p->d_tw2 = nullptr;
     CUDA_TRY(p, cudaMalloc(&p->d_tw1, tw1.size() * sizeof(float2)));
     CUDA_TRY(p, cudaMalloc(&p->d_tw2, tw2.size() * sizeof(float2)));
@@ -361,7 +363,7 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
         ++p->launches;
     } else {
         ProfScope ps(p, 1);
-        const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, 16, pass1_variant(p->g, cubic));
+        const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, p->g.p1_elems, pass1_variant(p->g, cubic));
         if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
         CUDA_TRY(p, f(ctx, a, tiles1, nt));
         ++p->launches;
@@ -561,7 +563,7 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     TmplDesc *h_tmpl = p->h_tmpl + (size_t)slot * p->tmpl_cap;
     int2 *h_grp = p->h_grp + (size_t)slot * p->sky_cap;
     // spacing in time of the first-pass inputs of one FFT pass-1 butterfly: (N1 / r0) rows of N2 samples
-    const double h_p1 = (double)(((int64_t)1 << p->g.log_n1) / radix_list(p->g.log_n1)[0]) * (double)((int64_t)1 << p->g.log_n2) * p->g.dt;
+    const double h_p1 = (double)(((int64_t)1 << p->g.log_n1) / radix_list(p->g.log_n1, p->g.p1_elems)[0]) * (double)((int64_t)1 << p->g.log_n2) * p->g.dt;
     for (size_t gi = 0; gi < groups.size(); ++gi) {
         fill_sky_const(p, groups[gi].alpha, groups[gi].delta, &h_sky[gi]);
         sky_abcd(p, groups[gi].alpha, groups[gi].delta, &h_abcd[gi], out.det_mask);
@@ -1078,9 +1080,10 @@ int fstat_debug_set_geometry(fstat_plan_t *plan, int32_t log_n2, int32_t log_til
     if (log_n2 >= 0) { g.log_n2 = log_n2; g.log_n1 = L - log_n2; }
     if (log_tile1 >= 0) g.log_tile1 = log_tile1;
     if (log_tile2 >= 0) g.log_tile2 = log_tile2;
-    if (log_n2 >= 0 && log_tile1 < 0) g.log_tile1 = g.log_n1 <= 10 ? 11 : g.log_n1;
+    if (log_n2 >= 0 && log_tile1 < 0) g.log_tile1 = (g.log_n1 == 9 || g.log_n1 == 10) ? 10 : g.log_n1 <= 10 ? 11 : g.log_n1;
     if (log_n2 >= 0 && log_tile2 < 0) g.log_tile2 = g.log_n2 <= 11 ? 12 : 13;
     g.p2_elems = p2_elems >= 0 ? p2_elems : ((g.log_n2 == 9 || g.log_n2 == 10) && g.log_tile2 >= 12 && !(g.log_n2 == 9 && g.log_tile2 == 13)) ? 32 : 16;
+    g.p1_elems = g.log_tile1 == 10 ? 32 : 16;
     g.log_w1 = g.log_tile1 - g.log_n1; g.log_w2 = g.log_tile2 - g.log_n2;
     if (!geometry_supported(g)) return fail(plan, FSTAT_ESIZE, "no kernel instantiated for this (sub-FFT, tile, elements) combination");
     plan->g = g;

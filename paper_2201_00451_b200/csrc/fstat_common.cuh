@@ -65,7 +65,7 @@ struct PlanGeom {
     int log_n1, log_n2;     // n_fft = 2^log_n1 * 2^log_n2 (log_n1 >= log_n2)
     int log_w1, log_w2;     // columns / rows per tile of FFT pass 1 / pass 2
     int log_tile1, log_tile2;   // log2 of the tile size of FFT pass 1 / 2 (11 or 12; sub-FFTs of length 2^12 use 13)
-    int p2_elems;           // register elements per thread of FFT pass 2 (16 or 32)
+    int p1_elems, p2_elems; // register elements per thread of FFT pass 1 / 2 (16 or 32)
     int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
     int log_node, n_nodes;  // timing nodes: every 2^log_node grid points (<= 256 s apart), n_nodes = ((n_src - 1) >> log_node) + 1
     double inv_node;        // 2^-log_node

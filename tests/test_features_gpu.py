@@ -170,6 +170,7 @@ def test_fused_sky_pass1_matches_oracle_and_hoisted_path(log_nfft, n_samples, dt
     p.templates = _sky_bank(p, 9, (-3e-9, 0.0, -1e-9), seed=5, fddot=fddot)
     cpu = O.fstat_2F_bank(p)
     with _plan(p) as plan:
+        plan.debug_set_geometry(log_tile1=11)                 # the fused kernel's tile shape (16 elements per thread)
         plan.debug_set_paths(fused_sky=0)
         hoisted = plan.compute(p.templates)
         plan.sync()
@@ -214,7 +215,7 @@ def test_single_kernel_form_matches_two_launch_form_and_oracle(log_nfft, n_sampl
     sample = sorted({0, p.injection_template, n_t - 1})
     cpu = O.fstat_2F_bank(p, sample)
     with _plan(p) as plan:
-        plan.debug_set_geometry(log_tile2=11)                     # both passes on 2^11-element tiles: the single-kernel shape
+        plan.debug_set_geometry(log_tile1=11, log_tile2=11)       # both passes on 2^11-element tiles: the single-kernel shape
         plan.debug_set_paths(single=0)
         plan.set_profile(True)
         two = plan.compute(p.templates)
