@@ -408,10 +408,12 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked, 
     ProfScope ps(p, 0);
     int rc = launch_timing_nodes(p, g0, ng);
     if (rc) return rc;
-    const int n_kblocks = (int)((g.n_src + SKY_THREADS * SKY_PTS - 1) / (SKY_THREADS * SKY_PTS));
+    // patches of 32 adjacent k2 x 32 adjacent k1 (k = N2 k1 + k2) over the rows that hold data
+    const int64_t rows_src = (g.n_src + ((int64_t)1 << g.log_n2) - 1) >> g.log_n2;
+    const int n_patches = (int)((rows_src + SKY_PATCH - 1) / SKY_PATCH) << (g.log_n2 - 5);
     // sky position fastest when the Farrow-filtered series would not stay in L2 between sky positions
     const int sky_major = ng > 1 && (size_t)g.n_det * (FARROW_NC / 2) * (size_t)(g.n_samples + 1) * sizeof(float4) > ((size_t)48 << 20);
-    sky_resample_kernel<<<(unsigned)n_kblocks * (unsigned)ng, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask, ng, n_kblocks, sky_major);
+    sky_resample_kernel<<<(unsigned)n_patches * (unsigned)ng, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask, ng, n_patches, sky_major);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return FSTAT_OK;

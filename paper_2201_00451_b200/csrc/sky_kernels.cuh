@@ -65,66 +65,90 @@ sidereal_table_kernel(PlanGeom g, float2 *__restrict__ rot) {
 }
 
 // The hoisted form of the sky-dependent half: S written once per sky position and re-read by every spin-down template
-// (long fdot banks).  A block works on SKY_PTS * 256 consecutive SSB grid points of one sky position, a thread on
-// SKY_PTS of them 256 apart (coalesced): what depends on (sky position, detector) only -- antenna coefficients, table
+// (long fdot banks).  With k = N2 k1 + k2 (the four-step index split of the FFT), a block works on a patch of 32
+// adjacent k2 x 32 adjacent k1 of one sky position: warp w takes the rows k1 = k1_0 + w + 8 i (i < 4), lane l the
+// grid point k2 = k2_0 + l of each, so that every read of the Farrow-filtered series is 32 consecutive samples
+// (512 B per coefficient pair); the 1024 results are transposed through shared memory and written in the tile-blocked
+// order FFT pass 1 bulk-loads, as runs of 512 B and more (written point by point that order scatters: one 16-byte piece
+// per line, 32 lines per warp store).  What depends on (sky position, detector) only -- antenna coefficients, table
 // bases -- is loaded once per thread for the first detector pair instead of once per grid point.
 // Block order: sky_major != 0 lets the sky position vary fastest, so that the blocks running at the same time cover
-// the same stretch of the SSB grid for all sky positions of the batch and read the same stretch (+- the spread of the
-// delays) of the Farrow-filtered series, which then comes from HBM once per batch instead of once per sky position
-// (used when that table exceeds what the L2 holds: 276 MB at config-2 size); otherwise the grid index varies fastest.
+// the same patch for all sky positions of the batch and read the same stretches (+- the spread of the delays) of the
+// Farrow-filtered series, which then comes from HBM once per batch instead of once per sky position (used when that
+// table exceeds what the L2 holds: 221 MB at config-2 size); otherwise the patch index varies fastest.
 //   S      : [n_sky][n_fft] float4 = (Re Ya0, Im Ya0, Re Yb0, Im Yb0); natural order S[k], or
-//            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: with k = N2*k1 + k2,
-//            S[k2 / W1][k1][k2 % W1]
-#ifndef SKY_PTS
+//            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: S[k2 / W1][k1][k2 % W1]
 #define SKY_PTS 4
-#endif
+#define SKY_PATCH 32
 #ifndef SKY_MIN_BLOCKS
 #define SKY_MIN_BLOCKS 4
 #endif
 __global__ void __launch_bounds__(SKY_THREADS, SKY_MIN_BLOCKS)
 sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restrict__ skies, const double4 *__restrict__ nodes,
                     const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
-                    float4 *__restrict__ S, int blocked, uint32_t det_mask, int n_sky, int n_kblocks, int sky_major) {
-    const int sky = sky_major ? (int)(blockIdx.x % (unsigned)n_sky) : (int)(blockIdx.x / (unsigned)n_kblocks);
-    const int kb = sky_major ? (int)(blockIdx.x / (unsigned)n_sky) : (int)(blockIdx.x % (unsigned)n_kblocks);
-    const int k0 = kb * (SKY_THREADS * SKY_PTS) + threadIdx.x;          // n_src <= n_fft <= 2^24
+                    float4 *__restrict__ S, int blocked, uint32_t det_mask, int n_sky, int n_patches, int sky_major) {
+    static_assert(SKY_THREADS == 8 * SKY_PATCH && SKY_PTS * 8 == SKY_PATCH, "8 warps x 4 rows = 32 rows of 32 points");
+    __shared__ float4 tile[SKY_PATCH * (SKY_PATCH + 16)];                 // row pitch 32 + W1 elements (W1 <= 16): conflict-free both ways
+    const int sky = sky_major ? (int)(blockIdx.x % (unsigned)n_sky) : (int)(blockIdx.x / (unsigned)n_patches);
+    const int pb = sky_major ? (int)(blockIdx.x / (unsigned)n_sky) : (int)(blockIdx.x % (unsigned)n_patches);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int k2_0 = (pb & ((1 << (g.log_n2 - 5)) - 1)) << 5, k1_0 = (pb >> (g.log_n2 - 5)) << 5;
     const SkyConst &sc = skies[sky];
     const double4 *nd = nodes + (int64_t)sky * g.n_det * g.n_nodes;
     const int n_rows = (int)g.n_samples + 1;
     float4 *Ss = S + (int64_t)sky * g.n_fft;
+    // through shared memory when the blocked order breaks a row of 32 adjacent k2 into pieces (W1 < 32 columns per pass-1 tile)
+    const bool transpose = blocked && g.log_w1 < 5;
+    const int pitch = SKY_PATCH + (1 << min(g.log_w1, 4));
     // the first detector pair (all there is in the two-detector configurations) hoisted out of the loop over grid points
     const SkyDetConst d0 = sky_det_const(g, sc, nd, Y, wslot, 0, det_mask);
     const SkyDetConst d1 = sky_det_const(g, sc, nd, Y, wslot, 1, det_mask);
 #pragma unroll 1
     for (int i = 0; i < SKY_PTS; ++i) {
-        const int k = k0 + i * SKY_THREADS;
-        if (k >= g.n_src) break;
+        const int k1 = k1_0 + warp + 8 * i, k2 = k2_0 + lane;
+        const int k = (k1 << g.log_n2) + k2;                              // n_src <= n_fft <= 2^24
         float2 ya = make_float2(0.f, 0.f), yb = make_float2(0.f, 0.f);
-        const SkyPointCommon c = sky_point_common(g, rot, k);
-        {
-            const SkyDetPoint o0 = sky_det_point(g, d0, c), o1 = sky_det_point(g, d1, c);
-            float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
-            sky_det_load(o0, n_rows, c0);
-            sky_det_load(o1, n_rows, c1);
-            sky_det_finish(o0, c0, ya, yb);
-            sky_det_finish(o1, c1, ya, yb);
-        }
-        for (int X0 = 2; X0 < g.n_det; X0 += 2) {
-            const SkyDetPoint o0 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0, det_mask), c);
-            const SkyDetPoint o1 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0 + 1, det_mask), c);
-            float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
-            sky_det_load(o0, n_rows, c0);
-            sky_det_load(o1, n_rows, c1);
-            sky_det_finish(o0, c0, ya, yb);
-            sky_det_finish(o1, c1, ya, yb);
-        }
-        int off = k;
-        if (blocked) {
-            const int k1 = k >> g.log_n2, k2 = k & ((1 << g.log_n2) - 1);
-            off = ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1));
+        if (k < g.n_src) {
+            const SkyPointCommon c = sky_point_common(g, rot, k);
+            {
+                const SkyDetPoint o0 = sky_det_point(g, d0, c), o1 = sky_det_point(g, d1, c);
+                float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
+                sky_det_load(o0, n_rows, c0);
+                sky_det_load(o1, n_rows, c1);
+                sky_det_finish(o0, c0, ya, yb);
+                sky_det_finish(o1, c1, ya, yb);
+            }
+            for (int X0 = 2; X0 < g.n_det; X0 += 2) {
+                const SkyDetPoint o0 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0, det_mask), c);
+                const SkyDetPoint o1 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0 + 1, det_mask), c);
+                float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
+                sky_det_load(o0, n_rows, c0);
+                sky_det_load(o1, n_rows, c1);
+                sky_det_finish(o0, c0, ya, yb);
+                sky_det_finish(o1, c1, ya, yb);
+            }
         }
         // blocked mode feeds the FFT kernels, whose element format is (Re Ya, Re Yb, Im Ya, Im Yb)
-        Ss[off] = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
+        const float4 v = blocked ? make_float4(ya.x, yb.x, ya.y, yb.y) : make_float4(ya.x, ya.y, yb.x, yb.y);
+        if (transpose) tile[(warp + 8 * i) * pitch + lane] = v;
+        else if (k < g.n_src) {                                           // rows of 32 adjacent k2 are contiguous in S
+            const int off = blocked ? ((k2 >> g.log_w1) << (g.log_n1 + g.log_w1)) + (k1 << g.log_w1) + (k2 & ((1 << g.log_w1) - 1)) : k;
+            Ss[off] = v;
+        }
+    }
+    if (!transpose) return;
+    __syncthreads();
+    // element e of the patch in output order: run e / (32 W1) = block of W1 columns, then k1, then the column within the block
+    const int lw = g.log_w1;
+#pragma unroll 1
+    for (int i = 0; i < SKY_PTS; ++i) {
+        const int e = ((warp + 8 * i) << 5) + lane;
+        const int run = e >> (5 + lw), within = e & ((32 << lw) - 1);
+        const int k1l = within >> lw, k2l = (run << lw) + (within & ((1 << lw) - 1));
+        const int k1 = k1_0 + k1l, k2 = k2_0 + k2l;
+        // rows beyond n_src are zero padding: written as zeros (the patch covers whole rows k1 < N1 only)
+        if (k1 < (1 << g.log_n1))
+            Ss[((k2 >> lw) << (g.log_n1 + lw)) + (k1 << lw) + (k2 & ((1 << lw) - 1))] = tile[k1l * pitch + k2l];
     }
 }
 
