@@ -496,6 +496,8 @@ def run_ours(args):
         plan.debug_set_paths(*[int(v) for v in args.paths.split(",")])
     if args.geometry:
         plan.debug_set_geometry(*[int(v) for v in args.geometry.split(",")])
+    if args.sky_slots:
+        plan.debug_set_max_sky_slots(args.sky_slots)
     n_t, nb = len(p.templates), plan.n_bins
     topk = args.mode == "topk"
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -583,6 +585,7 @@ def main():
     ap.add_argument("--inflight", type=int, default=0)
     ap.add_argument("--paths", default="", help="fused_sky,single overrides for fstat_debug_set_paths (-1 auto, 0 off, 1 on)")
     ap.add_argument("--geometry", default="", help="log_n2,log_tile1,log_tile2,p2_elems overrides for fstat_debug_set_geometry (-1 = default)")
+    ap.add_argument("--sky-slots", type=int, default=0, help="fstat_debug_set_max_sky_slots: sky positions resampled per batch (0 = default)")
     ap.add_argument("--mode", default="full", choices=["full", "topk"])
     ap.add_argument("--k", type=int, default=8)
     ap.add_argument("--cpu-templates-per-core", type=int, default=2)
