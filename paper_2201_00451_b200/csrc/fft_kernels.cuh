@@ -444,32 +444,39 @@ __device__ __forceinline__ void pass1_tile_loop(const FftArgs &p, float4 *sm, fl
     if (tile >= tile_end) return;
     float2 a[E], b[E];
     const int tile_mask = (1 << p.log_tiles) - 1;
-    TmplDesc td_next = p.tmpl[tile >> p.log_tiles];
+    // tile -> (template t, column block x).  Template-major (t = tile / tiles per template) by default; with p.t_fast the
+    // template varies fastest, so that the CTAs running at the same time work on the same column blocks of all templates
+    // of the launch and the series S, too large to stay in L2 for the length of a template (n_fft >= 2^22), is read from
+    // HBM once per launch instead of once per template.
+    const bool t_fast = p.t_fast != 0;
+    auto tile_t = [&](int tl) { return t_fast ? tl % p.n_tmpl : tl >> p.log_tiles; };
+    auto tile_x = [&](int tl) { return t_fast ? tl / p.n_tmpl : tl & tile_mask; };
+    TmplDesc td_next = p.tmpl[tile_t(tile)];
     // zero padding: rows k1 >= ceil(n_src / N2) of every column are zero, i.e. the inputs r >= r_nz of every first-pass
     // butterfly (k1 = i + r*NI): they are neither staged nor multiplied by the spin-down factor
     const int r_nz = !SKIPZ ? (int)RP::r0
         : min((int)RP::r0, (int)((((p.n_src + ((int64_t)1 << p.log_other) - 1) >> p.log_other) + (C::N / RP::r0) - 1) / (C::N / RP::r0)));
     const unsigned stage_bytes = (unsigned)min(r_nz * (C::N / RP::r0), (int)C::N) * C::W * 16u;
-    tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(tile & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
+    tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)tile_x(tile) * TILE_ELEMS, bar, pol_S, stage_bytes);
     for (; tile < tile_end; tile += stride) {
-        const int t = tile >> p.log_tiles, x = tile & tile_mask;
+        const int t = tile_t(tile), x = tile_x(tile);
         const TmplDesc td = td_next;
         const int k2_0 = x << LOGW;
         const int nxt = tile + stride;                  // fetch the next tile's descriptor early
-        if (nxt < tile_end) td_next = p.tmpl[nxt >> p.log_tiles];
+        if (nxt < tile_end) td_next = p.tmpl[tile_t(nxt)];
         mbar_wait(bar, parity);
         parity ^= 1;
         tile_take_inputs<LOGN, LOGT>(a, b, stage, SKIPZ ? r_nz : 32);
         if (FFT_P1_DB) {
             __syncthreads();                            // every thread has taken its inputs: the staging buffer is free
             if (nxt < tile_end)
-                tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
+                tile_prefetch<LOGN, LOGT>(stage, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)tile_x(nxt) * TILE_ELEMS, bar, pol_S, stage_bytes);
         }
         // times exp(-i Phi_s) (S9)
         spin_down<LOGN, LOGT, E, SKIPZ, CUBIC>(a, b, p, td, k2_0, r_nz);
         tile_passes<LOGN, LOGT>(a, b, sm, sm_tw);
         if (!FFT_P1_DB && nxt < tile_end)
-            tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)(nxt & tile_mask) * TILE_ELEMS, bar, pol_S, stage_bytes);
+            tile_prefetch<LOGN, LOGT>(sm, p.S + (int64_t)td_next.sky_slot * p.n_fft + (int64_t)tile_x(nxt) * TILE_ELEMS, bar, pol_S, stage_bytes);
         tile_last_pass<LOGN, LOGT>(a, b, sm_tw, p.tw);
         store_columns<LOGN, LOGT, E, AFFINE>(a, b, p, p.T + (int64_t)(t - t_off) * p.n_fft, k2_0, pol_T);
     }

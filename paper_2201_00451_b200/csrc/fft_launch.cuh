@@ -21,6 +21,8 @@ struct FftArgs {
     int log_tiles;            // log2(tiles per template) = log_other - LOGW
     int n_tiles;              // tiles per template * templates in this launch
     int accumulate;           // pass 2: add 2F to what the output row holds (semi-coherent sum over segments)
+    int n_tmpl;               // templates of this launch
+    int t_fast;               // pass 1: tile order with the template varying fastest (S read from HBM once per launch)
 };
 
 // Arguments of the fused sky + FFT pass-1 kernel (sky-varying search): the FFT arguments plus what the sky-dependent

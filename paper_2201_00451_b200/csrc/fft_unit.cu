@@ -30,6 +30,7 @@ cudaError_t launch_pass(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, in
     while ((1 << lt) < tiles_per_tmpl) ++lt;
     a.log_tiles = lt;
     a.n_tiles = tiles_per_tmpl * n_t;
+    a.n_tmpl = n_t;
     const int grid = a.n_tiles < resident ? a.n_tiles : resident;
     kern<<<grid, C::NT, SMEM, ctx.stream>>>(a);
     return cudaGetLastError();

@@ -109,6 +109,11 @@ struct ProfScope {
     ~ProfScope() { if (p->profile) { size_t e1 = prof_mark(p); p->segs.push_back({cls, e0, e1, (int)(p->launches - l0)}); } }
 };
 
+// pass 1 takes the template-fastest tile order when one sky position's series exceeds this many bytes (measured on B200)
+#ifndef FSTAT_TFAST_MIN_BYTES
+#define FSTAT_TFAST_MIN_BYTES (96ll << 20)
+#endif
+
 int ilog2(int64_t v) { int l = 0; while ((int64_t(1) << l) < v) ++l; return l; }
 
 // radix list of fft_kernels.cuh RadixPlan<LOGN>
@@ -365,8 +370,11 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
         ProfScope ps(p, 1);
         const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, p->g.p1_elems, pass1_variant(p->g, cubic));
         if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
+        // the series of one sky position no longer stays in L2 for the length of a template: template fastest in the tile order
+        a.t_fast = 16 * p->g.n_src > (int64_t)FSTAT_TFAST_MIN_BYTES;
         CUDA_TRY(p, f(ctx, a, tiles1, nt));
         ++p->launches;
+        a.t_fast = 0;
     }
     a.tw = p->d_tw2; a.log_other = l1; a.log_w_other = p->g.log_w1;
     {
