@@ -45,7 +45,7 @@ struct fstat_plan {
     void *d_tmp[3] = {nullptr, nullptr, nullptr};   // setup-time scratch (freed by destroy_impl if setup fails half-way)
     float2 *d_rot = nullptr;          // [n_src] cos, sin of the Greenwich sidereal angle per SSB grid point
     double4 *d_nodes = nullptr; size_t nodes_cap = 0;   // timing nodes of the sky positions of one batch [nodes_cap][n_det][n_nodes]
-    float2 *d_farrow = nullptr;       // [n_det][FARROW_NC/2][N+1] float4: Farrow-filtered series (sky_kernels.cuh)
+    float2 *d_farrow = nullptr;       // [n_det][y_det_stride] float4: Farrow-filtered series (sky_math.cuh farrow_index)
     float *d_wslot = nullptr;
     float2 *d_tw1 = nullptr, *d_tw2 = nullptr;
     float4 *d_S = nullptr;   int n_sky_slots = 0, max_sky_slots = 1;   // S buffers: allocated / allowed (grown on demand)
@@ -420,7 +420,7 @@ int launch_sky_batch(fstat_plan *p, int g0, int ng, float4 *S_dst, int blocked, 
     const int64_t rows_src = (g.n_src + ((int64_t)1 << g.log_n2) - 1) >> g.log_n2;
     const int n_patches = (int)((rows_src + SKY_PATCH - 1) / SKY_PATCH) << (g.log_n2 - 5);
     // sky position fastest when the Farrow-filtered series would not stay in L2 between sky positions
-    const int sky_major = ng > 1 && (size_t)g.n_det * (FARROW_NC / 2) * (size_t)(g.n_samples + 1) * sizeof(float4) > ((size_t)48 << 20);
+    const int sky_major = ng > 1 && (size_t)g.n_det * (size_t)g.y_det_stride * sizeof(float4) > ((size_t)48 << 20);
     sky_resample_kernel<<<(unsigned)n_patches * (unsigned)ng, SKY_THREADS, 0, p->stream>>>(g, p->d_sky + g0, p->d_nodes, p->d_rot, p->d_farrow, p->d_wslot, S_dst, blocked, det_mask, ng, n_patches, sky_major);
     p->launches += 1;
     CUDA_TRY(p, cudaGetLastError());
@@ -823,6 +823,8 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     while (g.log_node < 16 && (double)(2 << g.log_node) * dt <= 256.0) ++g.log_node;
     g.n_nodes = (int)((g.n_src - 1) >> g.log_node) + 1;
     g.inv_node = 1.0 / (double)(1 << g.log_node);
+    g.inv_n_fft = 1.0f / (float)n_fft;
+    g.y_det_stride = ((n_samples + 1 + FARROW_BLOCK - 1) / FARROW_BLOCK) * (int64_t)(FARROW_BLOCK * (FARROW_NC / 2));
     {   // Newton steps of the timing inversion: e <- C2 e^2 / 2 + dp^3 e until below 1e-11 s (sky_kernels.cuh)
         const double wa = fabs(eph->omega_orb * eph->au_over_c_s) + fabs(eph->omega_rot * eph->re_over_c_s);
         const double c2 = eph->omega_orb * eph->omega_orb * fabs(eph->au_over_c_s) + eph->omega_rot * eph->omega_rot * fabs(eph->re_over_c_s);
@@ -852,7 +854,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
         float *&d_fc = reinterpret_cast<float *&>(p->d_tmp[0]);
         SETUP_TRY(cudaMalloc(&d_fc, fc.size() * sizeof(float)));
         SETUP_TRY(cudaMemcpyAsync(d_fc, fc.data(), fc.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-        SETUP_TRY(cudaMalloc(&p->d_farrow, (size_t)n_det * (n_samples + 1) * FARROW_NC * sizeof(float2)));
+        SETUP_TRY(cudaMalloc(&p->d_farrow, (size_t)n_det * g.y_det_stride * sizeof(float4)));
         dim3 grid((unsigned)((n_samples + 1 + SKY_THREADS - 1) / SKY_THREADS), n_det);
         farrow_filter_kernel<<<grid, SKY_THREADS, 0, p->stream>>>(g, p->d_series, d_fc, p->d_farrow);
         ++p->launches;

@@ -69,4 +69,6 @@ struct PlanGeom {
     int n_newton;           // Newton steps of the SSB timing inversion (1 for the Earth)
     int log_node, n_nodes;  // timing nodes: every 2^log_node grid points (<= 256 s apart), n_nodes = ((n_src - 1) >> log_node) + 1
     double inv_node;        // 2^-log_node
+    float inv_n_fft;        // 1 / n_fft
+    int64_t y_det_stride;   // float4 elements of the Farrow-filtered series per detector: 128 * ceil((N + 1) / 32)
 };

@@ -12,7 +12,7 @@
 // numbers (five coalesced float4 loads) and runs one Horner recurrence instead of evaluating 2D+1 weights.
 //   series : [n_det][series_stride] float2 (data at +SERIES_PAD, zeros around it)
 //   coef   : [2D+1][FARROW_NC] float, row m+D
-//   Y      : [n_det][FARROW_NC/2][N+1] float4 = (Re Y_2c, Im Y_2c, Re Y_2c+1, Im Y_2c+1)
+//   Y      : [n_det][ceil((N+1)/32)][FARROW_NC/2][32] float4 = (Re Y_2c, Im Y_2c, Re Y_2c+1, Im Y_2c+1) (farrow_index, sky_math.cuh)
 __global__ void __launch_bounds__(SKY_THREADS)
 farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float *__restrict__ coef, float2 *__restrict__ Y) {
     __shared__ float s_coef[(2 * FSTAT_MAX_DTERMS + 1) * FARROW_NC];
@@ -31,11 +31,10 @@ farrow_filter_kernel(PlanGeom g, const float2 *__restrict__ series, const float 
 #pragma unroll
         for (int p = 0; p < FARROW_NC; ++p) acc[p] = __ffma2_rn(xv, make_float2(c[p], c[p]), acc[p]);
     }
-    // chunk-major: chunk c = (Y_2c, Y_2c+1) of all j contiguous, so that consecutive grid points read consecutive float4
-    float4 *out = reinterpret_cast<float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * (g.n_samples + 1) + j;
+    float4 *out = reinterpret_cast<float4 *>(Y) + (int64_t)X * g.y_det_stride + farrow_index((int)j);
 #pragma unroll
     for (int p = 0; p < FARROW_NC / 2; ++p)
-        out[(int64_t)p * (g.n_samples + 1)] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
+        out[FARROW_BLOCK * p] = make_float4(acc[2 * p].x, acc[2 * p].y, acc[2 * p + 1].x, acc[2 * p + 1].y);
 }
 
 __global__ void __launch_bounds__(NODE_THREADS)
@@ -80,6 +79,9 @@ sidereal_table_kernel(PlanGeom g, float2 *__restrict__ rot) {
 //            (blocked != 0) the tile-blocked order FFT pass 1 bulk-loads: S[k2 / W1][k1][k2 % W1]
 #define SKY_PTS 4
 #define SKY_PATCH 32
+#ifndef SKY_PIN_BASES
+#define SKY_PIN_BASES 1
+#endif
 #ifndef SKY_MIN_BLOCKS
 #define SKY_MIN_BLOCKS 5          // 48 registers; measured: 4 blocks +3 %, 6 blocks (40 registers, spills) +4 %
 #endif
@@ -95,14 +97,18 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
     const int k2_0 = (pb & ((1 << (g.log_n2 - 5)) - 1)) << 5, k1_0 = (pb >> (g.log_n2 - 5)) << 5;
     const SkyConst &sc = skies[sky];
     const double4 *nd = nodes + (int64_t)sky * g.n_det * g.n_nodes;
-    const int n_rows = (int)g.n_samples + 1;
     float4 *Ss = S + (int64_t)sky * g.n_fft;
     // through shared memory when the blocked order breaks a row of 32 adjacent k2 into pieces (W1 < 32 columns per pass-1 tile)
     const bool transpose = blocked && g.log_w1 < 5;
     const int pitch = SKY_PATCH + (1 << min(g.log_w1, 4));
     // the first detector pair (all there is in the two-detector configurations) hoisted out of the loop over grid points
-    const SkyDetConst d0 = sky_det_const(g, sc, nd, Y, wslot, 0, det_mask);
-    const SkyDetConst d1 = sky_det_const(g, sc, nd, Y, wslot, 1, det_mask);
+    SkyDetConst d0 = sky_det_const(g, sc, nd, Y, wslot, 0, det_mask);
+    SkyDetConst d1 = sky_det_const(g, sc, nd, Y, wslot, 1, det_mask);
+#if SKY_PIN_BASES
+    // the table bases are uniform values that ptxas would otherwise recompute in every iteration of the loop below
+    // (~40 uniform-datapath instructions per grid point): an opaque move pins them in registers
+    asm volatile("" : "+l"(d0.nodes), "+l"(d0.y), "+l"(d0.w), "+l"(d1.nodes), "+l"(d1.y), "+l"(d1.w));
+#endif
 #pragma unroll 1
     for (int i = 0; i < SKY_PTS; ++i) {
         const int k1 = k1_0 + warp + 8 * i, k2 = k2_0 + lane;
@@ -113,8 +119,8 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
             {
                 const SkyDetPoint o0 = sky_det_point(g, d0, c), o1 = sky_det_point(g, d1, c);
                 float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
-                sky_det_load(o0, n_rows, c0);
-                sky_det_load(o1, n_rows, c1);
+                sky_det_load(o0, c0);
+                sky_det_load(o1, c1);
                 sky_det_finish(o0, c0, ya, yb);
                 sky_det_finish(o1, c1, ya, yb);
             }
@@ -122,8 +128,8 @@ sky_resample_kernel(const __grid_constant__ PlanGeom g, const SkyConst *__restri
                 const SkyDetPoint o0 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0, det_mask), c);
                 const SkyDetPoint o1 = sky_det_point(g, sky_det_const(g, sc, nd, Y, wslot, X0 + 1, det_mask), c);
                 float4 c0[FARROW_NC / 2], c1[FARROW_NC / 2];
-                sky_det_load(o0, n_rows, c0);
-                sky_det_load(o1, n_rows, c1);
+                sky_det_load(o0, c0);
+                sky_det_load(o1, c1);
                 sky_det_finish(o0, c0, ya, yb);
                 sky_det_finish(o1, c1, ya, yb);
             }

@@ -112,6 +112,13 @@ __device__ __forceinline__ void timing_node(const PlanGeom &g, const SkyConst &s
 #define SKY_MAGIC64 6755399441055744.0
 #define SKY_MAGIC32 12582912.0f
 
+// Layout of the Farrow-filtered series of one detector: blocks of FARROW_BLOCK = 32 consecutive samples, within a block
+// the FARROW_NC / 2 coefficient pairs one after the other, each as 32 float4 = (Re Y_2c, Im Y_2c, Re Y_2c+1, Im Y_2c+1):
+// 32 consecutive samples of one pair are 512 contiguous bytes (coalesced for consecutive grid points), and the pairs of
+// one sample sit at compile-time offsets from each other (one address computation per sample instead of one per pair).
+#define FARROW_BLOCK 32
+__host__ __device__ __forceinline__ int farrow_index(int j) { return ((j >> 5) * (FARROW_BLOCK * (FARROW_NC / 2))) + (j & 31); }
+
 // what a grid point contributes to every detector
 struct SkyPointCommon {
     int krel;           // k - K_m
@@ -133,7 +140,7 @@ __device__ __forceinline__ SkyPointCommon sky_point_common(const PlanGeom &g, co
     // (shift * k mod n_fft) / n_fft is exact in fp32 (n_fft <= 2^24 is a power of two, uint32 wrap-around is mod 2^32);
     // + the residual fraction of a bin when f_het is off the bin grid: |value| <= 1/2, k < 2^24 exact in fp32 (error 6e-8 cycles)
     const uint32_t tshift = (g.shift_mod * (uint32_t)k) & (uint32_t)(g.n_fft - 1);
-    c.shift_cyc = (float)tshift * (1.0f / (float)g.n_fft);
+    c.shift_cyc = (float)tshift * g.inv_n_fft;
     if (g.shift_frac_per_k != 0.f) c.shift_cyc = fmaf((float)k, g.shift_frac_per_k, c.shift_cyc);
     return c;
 }
@@ -157,7 +164,7 @@ __device__ __forceinline__ SkyDetConst sky_det_const(const PlanGeom &g, const Sk
 #pragma unroll
     for (int q = 0; q < 4; ++q) d.bc[q] = sc.bc[X][q];
     d.nodes = nodes + (int64_t)X * g.n_nodes;
-    d.y = reinterpret_cast<const float4 *>(Y) + (int64_t)X * (FARROW_NC / 2) * (g.n_samples + 1);
+    d.y = reinterpret_cast<const float4 *>(Y) + (int64_t)X * g.y_det_stride;
     d.w = wslot + (int64_t)X * g.n_slots;
     d.on = Xu < g.n_det && ((det_mask >> X) & 1u);
     return d;
@@ -166,7 +173,7 @@ __device__ __forceinline__ SkyDetConst sky_det_const(const PlanGeom &g, const Sk
 // per (grid point, detector), before the Farrow coefficients are needed
 struct SkyDetPoint {
     float w, d, fc, ca, cb;
-    const float4 *y;        // Y_0,1 of sample j0; the other chunks follow n_rows apart
+    const float4 *y;        // (Y_0, Y_1) of sample j0; the other coefficient pairs follow 32 float4 apart (farrow_index)
 };
 
 __device__ __forceinline__ SkyDetPoint sky_det_point(const PlanGeom &g, const SkyDetConst &dc, const SkyPointCommon &c) {
@@ -188,7 +195,7 @@ __device__ __forceinline__ SkyDetPoint sky_det_point(const PlanGeom &g, const Sk
     o.d = (float)(v - (vm - SKY_MAGIC64));
     const int n_rows = (int)g.n_samples + 1;
     const int j0 = min(max(c.krel + __double2loint(vm), 0), n_rows - 1);   // in [0, N] whenever w != 0
-    o.y = dc.y + j0;
+    o.y = dc.y + farrow_index(j0);
     // step (iii): SSB heterodyne correction exp(-2 pi i f_het Delta), plus the band shift
     // (phase reduced mod 1 in fp64, then fp32)
     const double cyc = g.f_het * delta;
@@ -207,9 +214,9 @@ __device__ __forceinline__ SkyDetPoint sky_det_point(const PlanGeom &g, const Sk
     return o;
 }
 
-__device__ __forceinline__ void sky_det_load(const SkyDetPoint &o, int n_rows, float4 (&c)[FARROW_NC / 2]) {
+__device__ __forceinline__ void sky_det_load(const SkyDetPoint &o, float4 (&c)[FARROW_NC / 2]) {
 #pragma unroll
-    for (int p = 0; p < FARROW_NC / 2; ++p) c[p] = __ldg(o.y + (int64_t)p * n_rows);
+    for (int p = 0; p < FARROW_NC / 2; ++p) c[p] = __ldg(o.y + FARROW_BLOCK * p);
 }
 
 __device__ __forceinline__ void sky_det_finish(const SkyDetPoint &o, const float4 (&c)[FARROW_NC / 2], float2 &ya, float2 &yb) {
@@ -244,7 +251,7 @@ __device__ __forceinline__ void sky_point(const PlanGeom &g, const SkyConst &sc,
 #pragma unroll
         for (int u = 0; u < 2; ++u) o[u] = sky_det_point(g, sky_det_const(g, sc, nodes, Y, wslot, X0 + u, det_mask), c);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) sky_det_load(o[u], n_rows, cf[u]);
+        for (int u = 0; u < 2; ++u) sky_det_load(o[u], cf[u]);
 #pragma unroll
         for (int u = 0; u < 2; ++u) sky_det_finish(o[u], cf[u], ya, yb);
     }
