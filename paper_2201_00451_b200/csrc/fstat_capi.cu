@@ -299,7 +299,6 @@ int upload_twiddles(fstat_plan *p) {
 }
 
 // log2 of the tile size used for a sub-FFT of length 2^logn under the plan's tile setting
-int tile_log1(const fstat_plan *p) { return p->g.log_tile1; }
 int tile_log2(const fstat_plan *p) { return p->g.log_tile2; }
 
 // FFT + 2F for templates [t0, t0+nt) of the current call (descriptors already on the device).

@@ -244,7 +244,6 @@ __device__ __forceinline__ void sky_point(const PlanGeom &g, const SkyConst &sc,
                                           const float2 *__restrict__ rot, const float2 *__restrict__ Y, const float *__restrict__ wslot,
                                           int k, uint32_t det_mask, float2 &ya, float2 &yb) {
     const SkyPointCommon c = sky_point_common(g, rot, k);
-    const int n_rows = (int)g.n_samples + 1;
     for (int X0 = 0; X0 < g.n_det; X0 += 2) {
         SkyDetPoint o[2];
         float4 cf[2][FARROW_NC / 2];
