@@ -5,11 +5,11 @@
 
 // H3 in Farrow form.  The interpolation weight of tap m, c_m(d) = sinc(d-m) W(d-m) for d in [-1/2, 1/2)
 // (S6), is an entire function of d; fstat_setup expands it as c_m(d) = sum_p a[m][p] d^p
-// (Chebyshev interpolation of degree 9, converted to powers of d, fp64 -> fp32).  Then
+// (Chebyshev interpolation of degree FARROW_NC - 1 = 7, converted to powers of d, fp64 -> fp32).  Then
 //     z(j0 + d) = sum_m x[j0+m] c_m(d) = sum_p d^p Y_p[j0],   Y_p[j] = sum_m a[m][p] x[j+m]:
 // the 2D+1 taps are folded, once per plan and independent of the sky position, into FARROW_NC filtered
 // copies of the series (this kernel); per SSB grid point the resampler then reads FARROW_NC complex
-// numbers (five coalesced float4 loads) and runs one Horner recurrence instead of evaluating 2D+1 weights.
+// numbers (FARROW_NC / 2 = 4 coalesced float4 loads) and runs one Horner recurrence instead of evaluating 2D+1 weights.
 //   series : [n_det][series_stride] float2 (data at +SERIES_PAD, zeros around it)
 //   coef   : [2D+1][FARROW_NC] float, row m+D
 //   Y      : [n_det][ceil((N+1)/32)][FARROW_NC/2][32] float4 = (Re Y_2c, Im Y_2c, Re Y_2c+1, Im Y_2c+1) (farrow_index, sky_math.cuh)
