@@ -49,7 +49,8 @@ FSTAT_API int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slot
  *               (fstat_debug_set_geometry(-1, 11, -1, -1) where the default is the one-warp 2^10-element tile).
  *               Automatic = off: measured slower on B200.
  *   single    : one cooperative kernel for both FFT passes of groups of templates whose four-step intermediate
- *               stays in L2 (n_fft <= 2^18, both passes on 2^11-element tiles: fstat_debug_set_geometry(-1, 11, 11, -1)).
+ *               stays in L2 (n_fft <= 2^18, both passes on 2^11-element tiles and one of the splits 2^6 x 2^6, 2^7 x 2^6, 2^7 x 2^7,
+ *               2^9 x 2^6, 2^10 x 2^6 / 2^7 / 2^8: e.g. fstat_debug_set_geometry(6, 11, 11, -1) at n_fft = 2^16).
  *               Automatic = off: measured never faster than the two-launch form on B200. */
 FSTAT_API int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single);
 

@@ -253,7 +253,7 @@ void sky_abcd(const fstat_plan *p, double alpha, double delta, SkyABCD *out, uin
 // makes the runs of its transposed 2F store long (W2 x 4 bytes); pass 1 is fastest at <= 2^10 points with
 // 2^11-element tiles.
 void default_geometry(int L, PlanGeom &g) {
-    g.log_n2 = L <= 14 ? L / 2 : L <= 16 ? 6 : L == 17 ? 7 : L == 18 ? 8 : L == 19 ? 9 : L <= 21 ? 10 : L == 22 ? 10 : L - 12;
+    g.log_n2 = L <= 14 ? L / 2 : L == 15 ? 6 : L == 16 ? 7 : L <= 18 ? 8 : L == 19 ? 9 : L <= 21 ? 10 : L == 22 ? 10 : L - 12;
     g.log_n1 = L - g.log_n2;
     // pass 2: 2^12-element tiles; 2^13 (8 rows of 2^10 points: 128-byte runs in pass 1's transposed store, 32-byte
     // runs of 2F) for n_fft >= 2^21, where the gain in pass 1 outweighs the single CTA per SM in pass 2; likewise 4 rows

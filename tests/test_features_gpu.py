@@ -215,7 +215,8 @@ def test_single_kernel_form_matches_two_launch_form_and_oracle(log_nfft, n_sampl
     sample = sorted({0, p.injection_template, n_t - 1})
     cpu = O.fstat_2F_bank(p, sample)
     with _plan(p) as plan:
-        plan.debug_set_geometry(log_tile1=11, log_tile2=11)       # both passes on 2^11-element tiles: the single-kernel shape
+        # both passes on 2^11-element tiles and the split the single-kernel form is instantiated for
+        plan.debug_set_geometry(log_n2={12: 6, 13: 6, 14: 7, 15: 6, 16: 6, 17: 7, 18: 8}[log_nfft], log_tile1=11, log_tile2=11)
         plan.debug_set_paths(single=0)
         plan.set_profile(True)
         two = plan.compute(p.templates)
