@@ -701,10 +701,11 @@ int default_inflight(int64_t n_fft, int log_tile) {
     // templates per persistent launch.  Measured on B200 (profiles/r01_v3_experiments.md): every launch pair
     // costs ~35 us of ramp-up, tail and launch gap whatever its size, and keeping the four-step
     // intermediate L2-resident buys nothing (the passes are FMA-pipe bound, not DRAM bound), so
-    // launches are made large: ~64 rounds of 4096-element tiles over the 296 resident CTAs, bounded by
-    // 4 GB of intermediates (larger buffers get slower again: profiles/r01_v3_experiments.md, section 13).
+    // launches are made large: ~112 rounds of 4096-element tiles over the 296 resident CTAs (128 templates at 2^20 / 2^21:
+    // -1 % against 74, profiles/r02_experiments.md 15), bounded by 4 GB of intermediates (larger buffers get slower again:
+    // profiles/r01_v3_experiments.md, section 13).
     const int64_t tiles_per_tmpl = (n_fft >> log_tile) > 0 ? (n_fft >> log_tile) : 1;
-    int64_t want = (64 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
+    int64_t want = (112 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
     if (want < 64) want = 64;
     int64_t tb = (4096ll << 20) / (n_fft * 16);
     if (tb > want) tb = want;
