@@ -107,8 +107,8 @@ typedef struct fstat_plan fstat_plan_t;   /* opaque */
  *
  * Device memory owned by the plan: the series (8 B per sample and detector), its Farrow-filtered
  * copies (64 B per sample and detector: the interpolation taps folded once), 8 B per
- * SSB grid point (sidereal-angle table), 32 B per timing node (<= 256 s apart), detector and sky position of a batch, 16 B x n_fft per sky position of a batch (grown on demand, <= 1 GB) and up to
- * 4 GB of FFT intermediates (16 B x n_fft per template of a launch, grown on demand); scratch rows for the top-k and
+ * SSB grid point (sidereal-angle table), 32 B per timing node (<= 256 s apart), detector and sky position of a batch, 16 B x n_fft per sky position of a batch (grown on demand, <= 2 GB) and up to
+ * 8 GB of FFT intermediates (16 B x n_fft per template of a launch, grown on demand); scratch rows for the top-k and
  * host-output modes on first use.
  */
 FSTAT_API int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det,

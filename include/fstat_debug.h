@@ -39,7 +39,7 @@ FSTAT_API int fstat_get_profile(fstat_plan_t *plan, double *ms, int64_t *launche
  * fp32 rounding order. */
 FSTAT_API int fstat_debug_set_geometry(fstat_plan_t *plan, int32_t log_n2, int32_t log_tile1, int32_t log_tile2, int32_t p2_elems);
 
-/* Upper bound on the sky positions resampled per batch (default: 1 GB of resampled series); lets a test reach
+/* Upper bound on the sky positions resampled per batch (default: 2 GB of resampled series); lets a test reach
  * the multi-batch path with a handful of sky positions.  0 = default. */
 FSTAT_API int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slots);
 

@@ -702,12 +702,13 @@ int default_inflight(int64_t n_fft, int log_tile) {
     // costs ~35 us of ramp-up, tail and launch gap whatever its size, and keeping the four-step
     // intermediate L2-resident buys nothing (the passes are FMA-pipe bound, not DRAM bound), so
     // launches are made large: ~112 rounds of 4096-element tiles over the 296 resident CTAs (128 templates at 2^20 / 2^21:
-    // -1 % against 74, profiles/r02_experiments.md 15), bounded by 4 GB of intermediates (larger buffers get slower again:
+    // -1 % against 74, profiles/r02_experiments.md 15), bounded by 8 GB of intermediates (128 templates at 2^22, 64 at 2^23: -1..-2 % against 4 GB, mostly fewer top-k
+    // launches; profiles/r02_experiments.md 16; much larger buffers get slower again:
     // profiles/r01_v3_experiments.md, section 13).
     const int64_t tiles_per_tmpl = (n_fft >> log_tile) > 0 ? (n_fft >> log_tile) : 1;
     int64_t want = (112 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
     if (want < 64) want = 64;
-    int64_t tb = (4096ll << 20) / (n_fft * 16);
+    int64_t tb = (8192ll << 20) / (n_fft * 16);
     if (tb > want) tb = want;
     if (tb < 1) tb = 1;
     return (int)tb;
@@ -715,8 +716,8 @@ int default_inflight(int64_t n_fft, int log_tile) {
 
 int max_sky_slots_for(int64_t n_fft) {
     // sky positions resampled per batch: a search over the sky wants large batches (every FFT launch pair costs
-    // ~35 us whatever its size, profiles/r01_v3_experiments.md), bounded by 1 GB of resampled series
-    int64_t s = (1024ll << 20) / (n_fft * 16);
+    // ~35 us whatever its size, profiles/r01_v3_experiments.md), bounded by 2 GB of resampled series
+    int64_t s = (2048ll << 20) / (n_fft * 16);
     if (s < 1) s = 1;
     if (s > 1024) s = 1024;
     return (int)s;
