@@ -707,7 +707,7 @@ int default_inflight(int64_t n_fft, int log_tile) {
     // profiles/r01_v3_experiments.md, section 13).
     const int64_t tiles_per_tmpl = (n_fft >> log_tile) > 0 ? (n_fft >> log_tile) : 1;
     int64_t want = (112 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
-    if (want < 64) want = 64;
+    if (want < 128) want = 128;
     int64_t tb = (8192ll << 20) / (n_fft * 16);
     if (tb > want) tb = want;
     if (tb < 1) tb = 1;
