@@ -57,6 +57,7 @@ struct fstat_plan {
     double mom[FSTAT_MAX_DET][MOM_TERMS];                   // antenna moment matrices M_X (sky_kernels.cuh)
     bool pending_edom = false;                              // a template since the last sync had D <= 0
     int force_fused_sky = -1, force_single = -1;            // fstat_debug_set_paths
+    bool chunk_one_sky = false;                             // the launch being issued holds templates of one sky position only
     unsigned *d_counter = nullptr;                          // grid barrier of the single-kernel form
     TmplDesc *d_tmpl = nullptr; size_t tmpl_cap = 0;
     float *d_rows = nullptr;          // top-k scratch rows [n_inflight][n_bins]
@@ -370,7 +371,7 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
         const fft_launch_fn f = fft_find_kernel(1, l1, p->g.log_tile1, p->g.p1_elems, pass1_variant(p->g, cubic));
         if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 1");
         // the series of one sky position no longer stays in L2 for the length of a template: template fastest in the tile order
-        a.t_fast = 16 * p->g.n_src > (int64_t)FSTAT_TFAST_MIN_BYTES;
+        a.t_fast = p->chunk_one_sky && 16 * p->g.n_src > (int64_t)FSTAT_TFAST_MIN_BYTES;
         CUDA_TRY(p, f(ctx, a, tiles1, nt));
         ++p->launches;
         a.t_fast = 0;
@@ -621,6 +622,9 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
     auto run_chunk = [&](int g0, int t0, int nt, int fused_ng) -> int {
         bool cubic = false;                      // second spin-down anywhere in this launch?
         for (int t = t0; t < t0 + nt && !cubic; ++t) cubic = (tm[t].fddot != 0.0);
+        // one sky position for the whole launch?  (only then does the template-fastest tile order of pass 1 share anything)
+        p->chunk_one_sky = true;
+        for (int t = t0 + 1; t < t0 + nt && p->chunk_one_sky; ++t) p->chunk_one_sky = tm[t].alpha == tm[t0].alpha && tm[t].delta == tm[t0].delta;
         int r;
         if (out.mode == OUT_DEV_ROWS) {
             r = launch_fft_chunk(p, g0, t0, nt, out.rows + (int64_t)t0 * nb, nb, cubic, nullptr, out.accumulate, fused_ng, out.det_mask);
