@@ -166,6 +166,40 @@ FSTAT_API int fstat_select_topk(fstat_plan_t *plan, const float *twoF_dev, int32
 FSTAT_API int fstat_select_threshold(fstat_plan_t *plan, const float *twoF_dev, int32_t n_rows, float threshold, int32_t k,
                            float *val_dev, int32_t *bin_dev, int32_t *count_dev);
 
+/* fstat_select_topk_noalloc -- fstat_select_topk for callers that must not allocate device memory.
+ *
+ * Who needs it.  Two kinds of caller cannot let this library call cudaMalloc on their behalf:
+ *  (1) a search pipeline that has handed the whole GPU to its own arena or pool at start-up (the summed 2F rows of a
+ *      semi-coherent search, are typically held in such an arena): nothing is left for cudaMalloc to
+ *      give, so the plan-based calls, which create their scratch on first use, fail with an allocation error;
+ *  (2) a follow-up stage inside a latency-bound loop: cudaMalloc and cudaFree synchronise the whole device and stall
+ *      every other stream while they run.
+ * This call needs no plan (fstat_setup allocates) and calls no cudaMalloc, cudaFree or other allocating routine.  Its
+ * only scratch -- one uint32 maximum per group of 512 bins, the table the selection kernel reads to find the groups
+ * that can hold a top-k bin -- is a fixed array of FSTAT_NOALLOC_MAX_GROUPS entries (1 MiB) inside the library image.
+ * Every GPU that loads the library carries that 1 MiB until the process exits, whether or not this call is used.
+ *
+ *  twoF_dev   caller-owned DEVICE memory float32[n_rows][n_bins], row-major, read only.
+ *  n_bins     1 .. 2^24 bins per row (any value: rows need not be a multiple of 512).
+ *  n_rows     >= 0;  n_rows * ceil(n_bins / 512) must not exceed FSTAT_NOALLOC_MAX_GROUPS: e.g. 64 rows of 2^22 bins
+ *             or 4096 rows of 2^16 bins per call.  Larger requests are rejected with FSTAT_ESIZE and nothing is
+ *             launched; split them over several calls on the same stream.
+ *  k          1 .. min(64, n_bins).
+ *  val_dev float32[n_rows][k], bin_dev int32[n_rows][k]: caller-owned DEVICE memory; same order, tie rule and values
+ *             (bit for bit) as fstat_select_topk.
+ *  cuda_stream  a cudaStream_t (0 = legacy default stream); the call returns without waiting for the GPU.
+ *
+ * The device that holds the rows must be current.  The FIRST call on each device does a one-time set-up (it looks up
+ * the device address of the scratch array and raises the selection kernel's shared-memory limit); make that first call
+ * before any stream capture begins.  All calls on a device share the one array and it keeps whatever the last call
+ * left in it: the call overwrites every entry it reads, so nothing has to be cleared, but two calls whose GPU work
+ * overlaps (different streams, different host threads) race on it -- keep them on one stream or order them with
+ * events.  Errors: FSTAT_EINVAL (null pointer, k out of range, n_rows < 0), FSTAT_ESIZE (limits above), FSTAT_ECUDA;
+ * the text is available from fstat_last_error(NULL) on the calling thread. */
+#define FSTAT_NOALLOC_MAX_GROUPS 262144
+FSTAT_API int fstat_select_topk_noalloc(const float *twoF_dev, int64_t n_bins, int32_t n_rows, int32_t k,
+                              float *val_dev, int32_t *bin_dev, void *cuda_stream);
+
 /* Host-buffer variants (the end-to-end entry points): outputs are HOST memory (pinned
  * memory makes the copies asynchronous and overlapped); they return after the data
  * has landed and report FSTAT_EDOM if a template had D <= 0. */

@@ -20,7 +20,7 @@ FSTAT_OK, FSTAT_EINVAL, FSTAT_ESIZE, FSTAT_EDOM, FSTAT_ECUDA, FSTAT_ENOMEM = 0, 
 EXPORTS = [
     "fstat_setup", "fstat_get_layout", "fstat_compute", "fstat_compute_topk", "fstat_compute_threshold", "fstat_compute_host",
     "fstat_compute_topk_host", "fstat_compute_accumulate", "fstat_compute_per_detector", "fstat_select_topk",
-    "fstat_select_threshold", "fstat_resample_sky", "fstat_sync", "fstat_destroy", "fstat_strerror", "fstat_last_error",
+    "fstat_select_threshold", "fstat_select_topk_noalloc", "fstat_resample_sky", "fstat_sync", "fstat_destroy", "fstat_strerror", "fstat_last_error",
     # include/fstat_debug.h: measurement / experiment hooks
     "fstat_launch_count", "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile",
     "fstat_debug_set_geometry", "fstat_debug_set_max_sky_slots", "fstat_debug_set_paths",
@@ -86,6 +86,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_select_topk.argtypes = [vp, vp, i32, i32, vp, vp]
     lib.fstat_select_threshold.restype = C.c_int
     lib.fstat_select_threshold.argtypes = [vp, vp, i32, C.c_float, i32, vp, vp, vp]
+    lib.fstat_select_topk_noalloc.restype = C.c_int
+    lib.fstat_select_topk_noalloc.argtypes = [vp, i64, i32, i32, vp, vp, vp]
     lib.fstat_resample_sky.restype = C.c_int
     lib.fstat_resample_sky.argtypes = [vp, dbl, dbl, vp, C.POINTER(dbl)]
     lib.fstat_sync.restype = C.c_int
@@ -112,6 +114,33 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_last_error.argtypes = [vp]
     _lib = lib
     return lib
+
+
+NOALLOC_MAX_GROUPS = 262144          # FSTAT_NOALLOC_MAX_GROUPS of include/fstat.h
+
+
+def select_topk_noalloc(rows, k: int, out: Tuple, stream=None):
+    """fstat_select_topk_noalloc: the k loudest bins of every row of `rows` (float32[n_rows][n_bins] on the GPU), written
+    into the caller's `out = (val float32[n_rows][k], bin int32[n_rows][k])` device tensors.
+
+    For callers that cannot allocate device memory -- a pipeline whose own arena already owns the whole GPU, or a
+    latency-bound loop that cannot take the device-wide stall of cudaMalloc -- so, unlike `FstatPlan.select_topk`, it
+    takes no plan, creates no tensor and the library allocates nothing: the per-group maxima it needs live in a fixed
+    1 MiB array inside the library.  Hence `n_rows * ceil(n_bins / 512) <= NOALLOC_MAX_GROUPS` per call (FSTAT_ESIZE
+    otherwise), and calls whose GPU work overlaps race on that array: keep them on one stream.  The first call on a
+    device does a one-time set-up and should come before any stream capture.  Returns `out`."""
+    import torch
+    val, idx = out
+    assert rows.is_cuda and rows.dtype == torch.float32 and rows.is_contiguous() and rows.dim() == 2
+    assert val.is_cuda and val.dtype == torch.float32 and val.is_contiguous() and tuple(val.shape) == (rows.shape[0], k)
+    assert idx.is_cuda and idx.dtype == torch.int32 and idx.is_contiguous() and tuple(idx.shape) == (rows.shape[0], k)
+    lib = load_library()
+    s = torch.cuda.current_stream() if stream is None else stream
+    rc = lib.fstat_select_topk_noalloc(rows.data_ptr(), rows.shape[1], rows.shape[0], k, val.data_ptr(), idx.data_ptr(),
+                                       C.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise FstatError(rc, (lib.fstat_last_error(None) or lib.fstat_strerror(rc)).decode())
+    return out
 
 
 def _templates_array(templates) -> np.ndarray:

@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -743,6 +744,48 @@ int ensure_sky_slots(fstat_plan *p, size_t want) {
 
 }  // namespace
 
+// ---- fstat_select_topk_noalloc (include/fstat.h): scratch that is part of the library image -------------------------
+// The group maxima of the caller's rows, one uint32 per 512 bins.  A fixed array instead of a cudaMalloc, for callers
+// that cannot allocate (a pipeline whose arena owns the whole GPU; a latency-bound loop that cannot take the
+// device-wide stall of cudaMalloc / cudaFree).  1 MiB on every device that loads the library, until the process exits.
+// In HOST code this name is only a handle for the runtime's symbol table, not a device address: host code must go
+// through noalloc_scratch() below, which asks cudaGetSymbolAddress for the address on the current device.
+static __device__ __align__(256) uint32_t g_noalloc_gmax[FSTAT_NOALLOC_MAX_GROUPS];
+
+namespace {
+
+#define NOALLOC_MAX_DEVICES 64
+std::mutex g_noalloc_mu;
+uint32_t *g_noalloc_ptr[NOALLOC_MAX_DEVICES];      // device address of g_noalloc_gmax per device ordinal; null = not set up yet
+
+// One-time set-up per device, with that device current: the array's device address and the dynamic shared-memory
+// limit of the selection kernel (128 KB of group keys at 2^24 bins).  Neither call allocates device memory.
+int noalloc_scratch(uint32_t **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, FSTAT_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(nullptr, FSTAT_ECUDA, "device ordinal beyond the no-alloc set-up table");
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        uint32_t *ptr = nullptr;
+        e = cudaGetSymbolAddress((void **)&ptr, g_noalloc_gmax);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return fail(nullptr, FSTAT_ECUDA, std::string("cudaGetSymbolAddress(g_noalloc_gmax): ") + cudaGetErrorString(e));
+        }
+        e = cudaFuncSetAttribute(topk_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TOPK_MAX_GROUPS * (int)sizeof(uint32_t));
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(nullptr, FSTAT_ECUDA, std::string("cudaFuncSetAttribute(topk_select_kernel): ") + cudaGetErrorString(e));
+        }
+        g_noalloc_ptr[dev] = ptr;
+    }
+    *out = g_noalloc_ptr[dev];
+    return FSTAT_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char *fstat_strerror(int code) {
@@ -984,6 +1027,43 @@ int fstat_select_threshold(fstat_plan_t *plan, const float *twoF_dev, int32_t n_
     if (!std::isfinite(threshold)) return fail(plan, FSTAT_EINVAL, "non-finite threshold");
     if (n_rows > 0 && !count_dev) return fail(plan, FSTAT_EINVAL, "null count output");
     return select_rows(plan, twoF_dev, n_rows, k, val_dev, bin_dev, threshold, count_dev);
+}
+
+// fstat_select_topk without a plan and without any allocation: the two kernels of select_rows, with the group maxima
+// in the library's own g_noalloc_gmax (shared by every call on the device; group_max_kernel rewrites each entry the
+// selection reads, so stale contents of an earlier call are never seen).
+int fstat_select_topk_noalloc(const float *twoF_dev, int64_t n_bins, int32_t n_rows, int32_t k, float *val_dev, int32_t *bin_dev,
+                              void *cuda_stream) {
+    if (n_rows < 0 || (n_rows > 0 && (!twoF_dev || !val_dev || !bin_dev))) return fail(nullptr, FSTAT_EINVAL, "null argument or negative row count");
+    if (n_bins < 1 || n_bins > (int64_t(1) << 24)) return fail(nullptr, FSTAT_ESIZE, "n_bins outside [1, 2^24]");
+    if (k < 1 || k > FSTAT_MAX_TOPK || k > n_bins) return fail(nullptr, FSTAT_EINVAL, "k outside [1, min(64, n_bins)]");
+    const int64_t n_groups = (n_bins + 511) / 512;
+    if ((int64_t)n_rows * n_groups > FSTAT_NOALLOC_MAX_GROUPS) {
+        char msg[200];
+        snprintf(msg, sizeof msg, "n_rows * ceil(n_bins / 512) = %lld exceeds the fixed scratch of %d groups: split the rows over several calls",
+                 (long long)n_rows * (long long)n_groups, FSTAT_NOALLOC_MAX_GROUPS);
+        return fail(nullptr, FSTAT_ESIZE, msg);
+    }
+    if (n_rows == 0) return FSTAT_OK;
+    uint32_t *gmax = nullptr;
+    const int rc = noalloc_scratch(&gmax);
+    if (rc) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    TopkGeom tg{};
+    tg.elems = 16; tg.linear = 1; tg.n_groups = (int)n_groups;
+    const int chunk = 32768;                                   // rows per launch pair (grid.y limit of group_max_kernel)
+    for (int r0 = 0; r0 < n_rows; r0 += chunk) {
+        const int nr = std::min(chunk, n_rows - r0);
+        const float *rp = twoF_dev + (int64_t)r0 * n_bins;
+        uint32_t *gp = gmax + (int64_t)r0 * tg.n_groups;
+        group_max_kernel<<<dim3((tg.n_groups + TOPK_THREADS / 32 - 1) / (TOPK_THREADS / 32), nr), TOPK_THREADS, 0, stream>>>(
+            rp, n_bins, n_bins, tg.n_groups, gp);
+        topk_select_kernel<<<nr, TOPK_THREADS, tg.n_groups * sizeof(uint32_t), stream>>>(
+            rp, n_bins, n_bins, k, gp, tg, val_dev + (int64_t)r0 * k, bin_dev + (int64_t)r0 * k, 0.f, nullptr);
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, FSTAT_ECUDA, std::string("fstat_select_topk_noalloc launch: ") + cudaGetErrorString(e));
+    return FSTAT_OK;
 }
 
 int fstat_compute_host(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *twoF_host) {
