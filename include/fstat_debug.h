@@ -17,8 +17,10 @@ extern "C" {
 /* Number of kernels this plan has launched since setup (bench.py's `gpu_launches`). */
 FSTAT_API int fstat_launch_count(const fstat_plan_t *plan, int64_t *count);
 
-/* How many templates' four-step intermediates are kept in flight per launch (0 = default); bounds the
- * L2 / HBM footprint of the FFT. */
+/* How many templates' four-step intermediates are kept in flight per launch (0 = the plan's default, which depends on
+ * n_fft, the SM count and the device's memory; 1 .. FSTAT_MAX_INFLIGHT otherwise, FSTAT_EINVAL beyond); bounds the
+ * L2 / HBM footprint of the FFT (16 B x n_fft per template, allocated on demand). */
+#define FSTAT_MAX_INFLIGHT 65536
 FSTAT_API int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight);
 
 /* Per-kernel-class device timing with CUDA events on the plan's stream (for the roofline report,

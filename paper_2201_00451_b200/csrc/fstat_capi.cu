@@ -41,6 +41,7 @@ struct fstat_plan {
     double f_min = 0, band = 0, df = 0;
     int device = 0;
     int n_sm = 148;
+    size_t mem_total = 0;                            // device memory (cudaMemGetInfo at setup): scales the default buffer caps
     // device memory
     float2 *d_series = nullptr;
     void *d_tmp[3] = {nullptr, nullptr, nullptr};   // setup-time scratch (freed by destroy_impl if setup fails half-way)
@@ -702,27 +703,32 @@ void destroy_impl(fstat_plan *p) {
     delete p;
 }
 
-int default_inflight(int64_t n_fft, int log_tile) {
-    // templates per persistent launch.  Measured on B200 (profiles/r01_v3_experiments.md): every launch pair
+int default_inflight(const fstat_plan *p) {
+    // templates per persistent launch.  Measured on B200: every launch pair
     // costs ~35 us of ramp-up, tail and launch gap whatever its size, and keeping the four-step
     // intermediate L2-resident buys nothing (the passes are FMA-pipe bound, not DRAM bound), so
-    // launches are made large: ~112 rounds of 4096-element tiles over the 296 resident CTAs (128 templates at 2^20 / 2^21:
-    // -1 % against 74, profiles/r02_experiments.md 15), bounded by 8 GB of intermediates (128 templates at 2^22, 64 at 2^23: -1..-2 % against 4 GB, mostly fewer top-k
-    // launches; profiles/r02_experiments.md 16; much larger buffers get slower again:
-    // profiles/r01_v3_experiments.md, section 13).
+    // launches are made large: ~112 rounds of 4096-element tiles over the 2 resident CTAs of every SM (128 templates at
+    // 2^20 / 2^21: -1 % against 74), bounded by 8 GB of intermediates -- or 1/16 of the device's memory if that is
+    // less (180 GB on a B200: the 8 GB cap binds) -- i.e. 128 templates at 2^22, 64 at 2^23: -1..-2 % against 4 GB, mostly
+    // fewer top-k launches; much larger buffers get slower again.
+    const int64_t n_fft = p->g.n_fft;
+    const int log_tile = p->g.log_tile2;
     const int64_t tiles_per_tmpl = (n_fft >> log_tile) > 0 ? (n_fft >> log_tile) : 1;
-    int64_t want = (112 * (log_tile == 11 ? 4 : 2) * 148 + tiles_per_tmpl - 1) / tiles_per_tmpl;
+    int64_t want = (112 * (log_tile == 11 ? 4 : 2) * (int64_t)p->n_sm + tiles_per_tmpl - 1) / tiles_per_tmpl;
     if (want < 128) want = 128;
-    int64_t tb = (8192ll << 20) / (n_fft * 16);
+    const int64_t cap_bytes = std::min<int64_t>(8192ll << 20, (int64_t)(p->mem_total / 16));
+    int64_t tb = cap_bytes / (n_fft * 16);
     if (tb > want) tb = want;
+    if (tb > FSTAT_MAX_INFLIGHT) tb = FSTAT_MAX_INFLIGHT;
     if (tb < 1) tb = 1;
     return (int)tb;
 }
 
-int max_sky_slots_for(int64_t n_fft) {
+int max_sky_slots_for(const fstat_plan *p) {
     // sky positions resampled per batch: a search over the sky wants large batches (every FFT launch pair costs
-    // ~35 us whatever its size, profiles/r01_v3_experiments.md), bounded by 2 GB of resampled series
-    int64_t s = (2048ll << 20) / (n_fft * 16);
+    // ~35 us whatever its size), bounded by 2 GB of resampled series (1/64 of the device's memory if less)
+    const int64_t cap_bytes = std::min<int64_t>(2048ll << 20, (int64_t)(p->mem_total / 64));
+    int64_t s = cap_bytes / (p->g.n_fft * 16);
     if (s < 1) s = 1;
     if (s > 1024) s = 1024;
     return (int)s;
@@ -853,6 +859,7 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
 #define SETUP_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { p->err = std::string(#expr) + ": " + cudaGetErrorString(e__); return bail(e__ == cudaErrorMemoryAllocation ? FSTAT_ENOMEM : FSTAT_ECUDA); } } while (0)
     SETUP_TRY(cudaGetDevice(&p->device));
     SETUP_TRY(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device));
+    { size_t mem_free = 0; SETUP_TRY(cudaMemGetInfo(&mem_free, &p->mem_total)); }
     p->stream = (cudaStream_t)cuda_stream;
     PlanGeom &g = p->g;
     g.n_det = n_det; g.dterms = dterms; g.n_samples = n_samples; g.k_margin = km; g.n_src = n_samples + 2 * km;
@@ -869,6 +876,13 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
     // timing nodes (sky_kernels.cuh): the largest power of two of grid points that spans at most 256 s
     g.log_node = 0;
     while (g.log_node < 16 && (double)(2 << g.log_node) * dt <= 256.0) ++g.log_node;
+    {   // ... and small enough for THIS ephemeris: the cubic Hermite interpolant between nodes h apart is off by at most
+        // h^4 / 384 max|Delta''''| ~ h^4 / 384 (re w_rot^4 + au w_orb^4) (7e-12 s for the Earth at h = 256 s).  Halve the
+        // spacing until that is below 1e-9 s (needed: <~ 3e-8 s); at log_node = 0 every grid point is a node
+        // and the inversion is exact everywhere, so any ephemeris the omega * delay check above admits is handled.
+        const double d4 = fabs(eph->re_over_c_s) * pow(eph->omega_rot, 4) + fabs(eph->au_over_c_s) * pow(eph->omega_orb, 4);
+        while (g.log_node > 0 && pow((double)(1 << g.log_node) * dt, 4) / 384.0 * d4 > 1e-9) --g.log_node;
+    }
     g.n_nodes = (int)((g.n_src - 1) >> g.log_node) + 1;
     g.inv_node = 1.0 / (double)(1 << g.log_node);
     g.inv_n_fft = 1.0f / (float)n_fft;
@@ -893,10 +907,12 @@ int fstat_setup(fstat_plan_t **out, int32_t n_det, const fstat_detector_t *det, 
                                   cudaMemcpyDefault, p->stream));
     SETUP_TRY(cudaMalloc(&p->d_wslot, wslot.size() * sizeof(float)));
     SETUP_TRY(cudaMemcpyAsync(p->d_wslot, wslot.data(), wslot.size() * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-    if (upload_twiddles(p) != FSTAT_OK) return bail(FSTAT_ECUDA);
-    p->n_inflight = default_inflight(n_fft, g.log_tile2);
-    p->max_sky_slots = max_sky_slots_for(n_fft);
-    if (ensure_sky_slots(p, 1) != FSTAT_OK) return bail(FSTAT_ENOMEM);
+    // the default launch shape must be one fft_unit.cu instantiates: fail here, not in the first fstat_compute
+    if (!geometry_supported(g)) { p->err = "no FFT kernel instantiated for the default geometry of this n_fft"; return bail(FSTAT_ESIZE); }
+    { const int rc = upload_twiddles(p); if (rc != FSTAT_OK) return bail(rc); }
+    p->n_inflight = default_inflight(p);
+    p->max_sky_slots = max_sky_slots_for(p);
+    { const int rc = ensure_sky_slots(p, 1); if (rc != FSTAT_OK) return bail(rc); }
     {   // Farrow-filtered copies of the series (sky_kernels.cuh), once per plan
         const std::vector<float> fc = farrow_coefficients(dterms);
         float *&d_fc = reinterpret_cast<float *&>(p->d_tmp[0]);
@@ -1132,10 +1148,10 @@ int fstat_launch_count(const fstat_plan_t *plan, int64_t *count) {
 }
 
 int fstat_set_inflight(fstat_plan_t *plan, int32_t n_inflight) {
-    if (!plan || n_inflight < 0 || n_inflight > 4096) return FSTAT_EINVAL;
+    if (!plan || n_inflight < 0 || n_inflight > FSTAT_MAX_INFLIGHT) return FSTAT_EINVAL;
     CUDA_TRY(plan, cudaSetDevice(plan->device));
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
-    const int tb = n_inflight == 0 ? default_inflight(plan->g.n_fft, plan->g.log_tile2) : n_inflight;
+    const int tb = n_inflight == 0 ? default_inflight(plan) : n_inflight;
     if (tb == plan->n_inflight) return FSTAT_OK;
     cudaFree(plan->d_T); plan->d_T = nullptr; plan->t_cap = 0;
     cudaFree(plan->d_rows); plan->d_rows = nullptr;
@@ -1194,7 +1210,7 @@ int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slots) {
     if (!plan || max_slots < 0) return FSTAT_EINVAL;
     CUDA_TRY(plan, cudaSetDevice(plan->device));
     CUDA_TRY(plan, cudaStreamSynchronize(plan->stream));
-    plan->max_sky_slots = max_slots == 0 ? max_sky_slots_for(plan->g.n_fft) : max_slots;
+    plan->max_sky_slots = max_slots == 0 ? max_sky_slots_for(plan) : max_slots;
     if (plan->n_sky_slots > plan->max_sky_slots) {            // shrink: reallocate on the next call
         cudaFree(plan->d_S); plan->d_S = nullptr; plan->n_sky_slots = 0;
         return ensure_sky_slots(plan, 1);

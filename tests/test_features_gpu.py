@@ -87,6 +87,61 @@ def test_per_detector_statistic_matches_oracle():
     assert rel_err(coh, O.fstat_2F_bank(p)).max() <= TOL          # the coherent path is untouched by the masked runs
 
 
+def test_per_detector_with_an_all_gap_detector_gives_nan_rows_and_edom():
+    # detector 1 has no data segment at all: D_1 <= 0, its rows are NaN and fstat_sync reports FSTAT_EDOM; the rows of the
+    # detectors that do have data are unaffected
+    from paper_2201_00451_b200.binding import FstatError, FSTAT_EDOM
+    p = synth.small_problem(seed=97, n_det=3, rho=14.0, n_samples=30000, n_fft=1 << 16, n_templates=2, gap_frac=0.3)
+    p.timestamps[1] = p.timestamps[1][:0]
+    p.weights[1] = p.weights[1][:0]
+    p.series[1] = np.zeros_like(p.series[1])
+    with _plan(p) as plan:
+        gpu = plan.compute_per_detector(p.templates)
+        with pytest.raises(FstatError) as ei:
+            plan.sync()
+        assert ei.value.code == FSTAT_EDOM
+        gpu = gpu.cpu().numpy()
+        coh = plan.compute(p.templates)                 # the coherent statistic over the two live detectors is fine
+        plan.sync()
+        coh = coh.cpu().numpy()
+    assert np.isnan(gpu[1]).all()
+    for X in (0, 2):
+        cpu = np.stack([O.fstat_2F(O.single_detector_view(p, X), t) for t in p.templates])
+        assert rel_err(gpu[X], cpu).max() <= TOL
+    assert rel_err(coh, O.fstat_2F_bank(p)).max() <= TOL
+
+
+def test_accumulate_with_bin_offsets_across_several_launches():
+    # n_tmpl > templates per launch: the per-template bin offsets must follow their templates through the chunking
+    # (fstat_set_inflight(4), 11 templates of 3 sky positions -> 3+ launches); bit-identical to the one-launch result and
+    # equal to the oracle's shifted rows
+    import torch
+    p = synth.small_problem(seed=98, n_samples=9000, n_fft=1 << 14, n_templates=3, rho=9.0)
+    sky = [(3.52, -0.83), (1.1, 0.4), (5.0, 1.0)]
+    tm = [(a, d, p.f_min, fd, 0.0) for (a, d) in sky for fd in (-2e-9, -1e-9, 0.0, 1e-9)][:11]
+    p.templates = np.array(tm)
+    n_t, nb = len(tm), p.n_bins
+    offs = np.array([0, 5, -3, 17, -40, 0, 1, -1, nb - 1, -(nb - 1), 250], dtype=np.int32)
+    cpu = O.fstat_2F_bank(p)
+    want = np.zeros_like(cpu)
+    for t in range(n_t):
+        q = np.arange(nb) - offs[t]                       # bin q of the plan lands on output bin q - off
+        ok = (q >= 0) & (q < nb)
+        want[t, q[ok]] = cpu[t, ok]
+    with _plan(p) as plan:
+        one = torch.zeros((n_t, nb), dtype=torch.float32, device="cuda")
+        plan.compute_accumulate(p.templates, one, offs)
+        plan.sync()
+        plan.set_inflight(4)
+        many = torch.zeros((n_t, nb), dtype=torch.float32, device="cuda")
+        plan.compute_accumulate(p.templates, many, offs)
+        plan.compute_accumulate(p.templates, many, offs)             # twice: the second pass adds to the first
+        plan.sync()
+        one, many = one.cpu().numpy(), many.cpu().numpy()
+    assert (np.abs(one - want) / np.maximum(want, 4.0)).max() <= TOL
+    np.testing.assert_array_equal(many, one + one)
+
+
 def test_two_live_topk_plans_of_different_size():
     # the dynamic shared memory attribute of the selection kernel is per function, not per plan
     big = synth.small_problem(seed=96, n_samples=int(0.7 * (1 << 20)), dt=0.5, n_fft=1 << 20, n_templates=2, rho=10.0)

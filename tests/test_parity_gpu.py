@@ -86,9 +86,36 @@ def test_parity_three_detectors():
     assert int(np.argmax(gpu.max(axis=1))) == int(np.argmax(cpu.max(axis=1))) == p.injection_template
 
 
-def test_resampled_series_and_antenna_sums_match_oracle():
-    p = synth.small_problem(seed=9, n_samples=30000, n_fft=1 << 15, n_templates=1)
-    al, de = synth.SKY0
+@pytest.mark.parametrize("n_det", [4, 5])
+def test_parity_four_and_five_detectors(n_det):
+    # more than one full detector pair in the sky kernel's pair loop (4: two pairs; 5: two pairs and one alone)
+    q = synth.small_problem(seed=50 + n_det, n_det=3, n_samples=30000, n_fft=1 << 16, n_templates=2, gap_frac=0.3, rho=14.0)
+    extra = [dict(lat_rad=36.41 * synth.DEG, lon_east_rad=137.31 * synth.DEG, xarm_azimuth_rad=60.4 * synth.DEG),
+             dict(lat_rad=19.61 * synth.DEG, lon_east_rad=77.03 * synth.DEG, xarm_azimuth_rad=207.0 * synth.DEG)]
+    dets = (q.detectors + extra)[:n_det]
+    p = synth.make_problem(f"det{n_det}", dets, q.n_samples, q.dt, q.f_min, q.band, q.f_het, q.n_fft, q.dterms, q.templates,
+                           seed=q.seed, gap_frac=0.3, weight_range=(0.5, 2.0), injection=q.injection,
+                           injection_template=q.injection_template, snap_injection_to_bin=True)
+    assert p.n_det == n_det
+    gpu, cpu = _check_bank(p)
+    assert int(np.argmax(gpu.max(axis=1))) == int(np.argmax(cpu.max(axis=1))) == p.injection_template
+
+
+@pytest.mark.parametrize("omega_rot", [1e-2, 0.5])
+def test_parity_fast_rotation_ephemeris_without_orbit(omega_rot):
+    # an ephemeris fstat_setup admits (omega * delay < 0.05 rad) that is nothing like the Earth: no orbit, a rotation
+    # period of 10 minutes / 13 s.  The timing nodes (<= 256 s apart for the Earth) must move closer together for the
+    # cubic Hermite interpolant of the delay to hold: fstat_setup bounds h^4/384 (re w_rot^4 + au w_orb^4) <= 1e-9 s
+    # (at 0.5 rad/s every grid point becomes a node).  With 256 s nodes the delay would be off by milliseconds.
+    eph = dict(synth.EPHEM_DEFAULT, au_over_c_s=0.0, omega_rot=omega_rot)
+    p = synth.small_problem(seed=77, n_samples=20000, n_fft=1 << 15, n_templates=2, rho=12.0, ephem=eph)
+    gpu, cpu = _check_bank(p)
+    assert int(gpu[p.injection_template].argmax()) == int(cpu[p.injection_template].argmax())
+    # and the resampled series itself (the delay enters through the sample index and the heterodyne phase)
+    _check_resampled_series(p, float(p.templates[0, 0]), float(p.templates[0, 1]))
+
+
+def _check_resampled_series(p, al, de):
     sky = O.per_sky(p, al, de)
     n_src = p.n_samples + 2 * O.k_margin(p)
     ya = np.zeros(n_src, dtype=np.complex128)
@@ -110,6 +137,11 @@ def test_resampled_series_and_antenna_sums_match_oracle():
     assert np.abs(S[:n_src, 2] + 1j * S[:n_src, 3] - yb).max() <= 2e-5 * scale
     assert np.all(S[n_src:] == 0)
     np.testing.assert_allclose(abcd, np.array(sky["ABCD"]), rtol=2e-6)
+
+
+def test_resampled_series_and_antenna_sums_match_oracle():
+    p = synth.small_problem(seed=9, n_samples=30000, n_fft=1 << 15, n_templates=1)
+    _check_resampled_series(p, *synth.SKY0)
 
 
 def test_multiple_sky_positions_in_one_call():
