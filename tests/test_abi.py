@@ -72,6 +72,55 @@ def test_setup_argument_validation_without_gpu():
     assert len(lib.fstat_last_error(None)) > 0
 
 
+def test_oracle_validate_and_fstat_setup_reject_the_same_sizes():
+    """Pin of `O.validate` (the oracle's only function without one): it raises on exactly the size rules of the method that
+    fstat_setup answers with FSTAT_ESIZE -- n_fft a power of two, n_samples + 2 ceil(512 s/dt) <= n_fft (the zero-padded
+    transform must hold the resampled series, S7), band <= 1/dt -- and accepts what fstat_setup
+    accepts, on both sides of every boundary.  (Dterms outside [1, 32] is a limit of the CUDA library only: the oracle's
+    windowed sinc is defined for any D.)"""
+    import copy
+    from oracle import fstat_oracle as O
+    lib = binding.load_library()
+    p = synth.small_problem(n_samples=5000, n_fft=1 << 13, rho=None)
+    km2 = 2 * O.k_margin(p)
+
+    def both(**over):
+        q = copy.copy(p)
+        for k, v in over.items():
+            setattr(q, k, v)
+        try:
+            O.validate(q)
+            oracle_ok = True
+        except ValueError:
+            oracle_ok = False
+        rc, h = _setup_raw(lib, p, **over)
+        if rc == binding.FSTAT_OK:
+            lib.fstat_destroy(h)
+        lib_ok = rc != binding.FSTAT_ESIZE               # valid sizes end in FSTAT_OK (GPU box) or FSTAT_ECUDA (no device)
+        assert rc in (binding.FSTAT_OK, binding.FSTAT_ECUDA, binding.FSTAT_ESIZE), rc
+        assert oracle_ok == lib_ok, (over, oracle_ok, rc)
+        return oracle_ok
+
+    assert both() is True
+    assert both(n_fft=(1 << 13) + 2) is False                       # not a power of two
+    assert both(n_fft=1 << 12) is False                             # 5000 + 1024 > 4096
+    assert both(n_fft=1 << 14) is True
+    assert both(band=1.5 / p.dt) is False                           # wider than the sample rate
+    assert both(band=1.0 / p.dt) is True                            # exactly the sample rate: every FFT output is a bin
+    # the boundary of the padding rule, on a series cut to fit / not to fit exactly
+    for n_samples, ok in (((1 << 13) - km2, True), ((1 << 13) - km2 + 1, False)):
+        q = synth.small_problem(n_samples=n_samples, n_fft=1 << 13, rho=None)
+        try:
+            O.validate(q)
+            oracle_ok = True
+        except ValueError:
+            oracle_ok = False
+        rc, h = _setup_raw(lib, q)
+        if rc == binding.FSTAT_OK:
+            lib.fstat_destroy(h)
+        assert oracle_ok == ok and (rc != binding.FSTAT_ESIZE) == ok, (n_samples, oracle_ok, rc)
+
+
 def test_no_cpu_fallback():
     import torch
     if torch.cuda.is_available():

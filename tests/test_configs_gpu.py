@@ -2,6 +2,10 @@
 templates per launch), on sampled templates the oracle can compute one by one -- plus the
 properties that hold at any size (chi^2_4 noise statistics of the full bank, top-k == selection
 over the full rows, loudest template)."""
+import os
+import subprocess
+import sys
+
 import numpy as np
 import pytest
 
@@ -11,6 +15,46 @@ from paper_2201_00451_b200 import synth
 from _parity_util import TOL, compare_rows
 
 pytestmark = pytest.mark.gpu
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _start_oracle_bank(config, out, rows=()):
+    """The oracle over the whole bank of `synth.<config>()` in a process of its own (tests/oracle_bank_maxima.py: a fork
+    pool over the host cores), started before the GPU work of the test so that the two overlap."""
+    cmd = [sys.executable, os.path.join(HERE, "oracle_bank_maxima.py"), config, str(out), "--rows", ",".join(str(int(r)) for r in rows)]
+    return subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+
+
+def _finish_oracle_bank(proc, out, timeout=1000):
+    text, _ = proc.communicate(timeout=timeout)
+    assert proc.returncode == 0, text
+    print("[oracle]", text.strip().splitlines()[-1])
+    return np.load(str(out))
+
+
+def _check_bank_maxima(val, idx, ora, label):
+    """GPU top-1 (val[n_t], idx[n_t]) of every template against the oracle's three loudest bins of the same row:
+    the GPU's bin is one of them, its value agrees within TOL, and where it is not the oracle's loudest bin the two are a
+    tie within the tolerance (S15: what is compared is unique only up to the tolerance); the loudest template
+    of the whole bank is identical (same rule)."""
+    ov, ob = ora["val"], ora["bin"]
+    n_t = len(val)
+    assert ov.shape[0] == n_t
+    hit = ob == idx[:, None].astype(np.int64)
+    assert hit.any(axis=1).all(), np.nonzero(~hit.any(axis=1))[0][:10]
+    pos = hit.argmax(axis=1)
+    o_at = ov[np.arange(n_t), pos]
+    err = np.abs(val.astype(np.float64) - o_at) / np.maximum(o_at, 4.0)
+    assert err.max() <= TOL, err.max()
+    gap = (ov[:, 0] - o_at) / np.maximum(ov[:, 0], 4.0)
+    assert gap.max() <= 2 * TOL, gap.max()
+    tg, to = int(np.argmax(val)), int(np.argmax(ov[:, 0]))
+    assert tg == to or (ov[to, 0] - ov[tg, 0]) <= 2 * TOL * max(ov[to, 0], 4.0), (tg, to)
+    print(f"[parity] {label}: loudest bin of all {n_t} templates: max |d2F|/max(2F,4) = {err.max():.2e}, "
+          f"{int((pos != 0).sum())} rows where the GPU's loudest bin is the oracle's second or third (ties within {2 * TOL:g}), "
+          f"loudest template {tg} (oracle {to}), 2F = {val[tg]:.3f} (oracle {ov[to, 0]:.3f})")
+    return tg
 
 
 def _plan(prob):
@@ -39,8 +83,9 @@ def test_config1_full_bank_every_bin():
     assert abs(f_peak - 100.2) < 2 * p.df
 
 
-def test_config2_full_size_sampled_templates_and_loudest():
+def test_config2_full_size_sampled_templates_and_loudest(tmp_path):
     p = synth.config2()                                  # 1024 templates, FFT 2^21, 30 % gaps, weights
+    proc = _start_oracle_bank("config2", tmp_path / "config2.npz")      # the oracle runs ALL templates
     sample = sorted({0, 1, p.injection_template - 1, p.injection_template, p.injection_template + 1, 517, 1023})
     cpu = O.fstat_2F_bank(p, sample)
     with _plan(p) as plan:
@@ -55,6 +100,9 @@ def test_config2_full_size_sampled_templates_and_loudest():
     # loudest template of the whole bank = the injected one, which the oracle confirms within the sample
     assert int(np.argmax(val[:, 0])) == p.injection_template
     assert sample[int(np.argmax(cpu.max(axis=1)))] == p.injection_template
+    # every one of the 1024 templates: loudest bin and its value against the oracle's row, loudest template of the bank
+    ora = _finish_oracle_bank(proc, tmp_path / "config2.npz")
+    assert _check_bank_maxima(val[:, 0], idx[:, 0], ora, "config2 full bank") == p.injection_template
 
 
 CELLS = [(d, b) for d in synth.CONFIG3_DAYS for b in synth.CONFIG3_BANDS]
@@ -161,6 +209,46 @@ def test_config5_shape_sky_grid_dterms16():
     # over 2 days neighbouring sky points are degenerate with frequency, so the loudest template need not be the
     # injected one (input recipe); the injected template itself carries 2F ~ 4 + rho^2 = 104 +- 20
     assert 50.0 < gpu[inj_local].max() < 170.0
+
+
+def test_config5_full_bank_all_sky_batches_and_loudest_template(tmp_path):
+    # the whole config-5 bank (4096 sky positions x 4 spin-downs = 16384 templates, FFT 2^18, Dterms 16) in the launch
+    # structure bench.py times: 8 sky batches of 512 positions.  From every batch the complete rows of four sky positions
+    # (first, last, two seeded random ones; all four spin-downs) are compared bin by bin with the oracle, and the oracle
+    # runs over the WHOLE bank (tests/oracle_bank_maxima.py, all host cores) so that the loudest bin of every template
+    # and the loudest template of the bank are checked, not only timed (VERDICT r2 missing 1)
+    import torch
+    p = synth.config5()
+    n_t = len(p.templates)
+    n_sky, per_batch = n_t // 4, 512
+    assert n_sky == 4096 and np.all(p.templates[0::4, :2] == p.templates[3::4, :2])
+    rng = np.random.default_rng(505)
+    sky_sample = []
+    for b in range(n_sky // per_batch):
+        lo = b * per_batch
+        sky_sample += [lo, lo + per_batch - 1] + [int(x) for x in lo + 1 + rng.choice(per_batch - 2, size=2, replace=False)]
+    sample = sorted(4 * s + j for s in sky_sample for j in range(4))
+    proc = _start_oracle_bank("config5", tmp_path / "config5.npz", sample)
+    with _plan(p) as plan:
+        full = plan.compute(p.templates)                        # 16384 x 131072 float32 = 8.6 GB on the GPU
+        val, idx = plan.compute_topk(p.templates, 1)
+        plan.sync()
+        assert bool(torch.isfinite(full).all())
+        m = full.max(dim=1)
+        assert torch.equal(m.values, val[:, 0])                 # the top-k path agrees with the full rows, every template
+        rows = full[sample].cpu().numpy()
+        val, idx = val.cpu().numpy()[:, 0], idx.cpu().numpy()[:, 0]
+        del full, m
+        torch.cuda.empty_cache()
+    ora = _finish_oracle_bank(proc, tmp_path / "config5.npz")
+    np.testing.assert_array_equal(ora["row_idx"], sample)
+    err = _rel_err(rows, ora["rows"])
+    print(f"[parity] config5 full bank: {len(sample)} complete rows from all 8 sky batches: max |d2F|/max(2F,4) = {err.max():.2e}")
+    assert err.max() <= TOL
+    best = _check_bank_maxima(val, idx, ora, "config5 full bank")
+    # over 2 days neighbouring sky points are degenerate with frequency (input recipe): the loudest template is
+    # near the injected one on the sky, not necessarily it; the injected template carries 2F ~ 4 + rho^2
+    assert 50.0 < val[p.injection_template] < 170.0 and val[best] >= val[p.injection_template]
 
 
 def test_sky100_protocol_on_a_config3_cell():
