@@ -101,21 +101,20 @@ def algorithmic_bytes(p):
 
 
 def ncu_traffic_table():
-    """{(class, n_fft): dram bytes per template} from the newest committed `profiles/r*_traffic.csv`
-    (ncu dram__bytes_read.sum + dram__bytes_write.sum per launch / templates per launch)."""
-    pdir = os.path.join(ROOT, "profiles")
+    """{(class, n_fft): dram bytes per template} from `paper_2201_00451_b200/traffic_table.csv` (ncu dram__bytes_read.sum +
+    dram__bytes_write.sum per launch / templates per launch, written by `python -m paper_2201_00451_b200.capture_traffic`),
+    and a description that names the commit the table was captured on."""
+    path = os.path.join(ROOT, "paper_2201_00451_b200", "traffic_table.csv")
+    tab, commits = {}, set()
     try:
-        files = sorted(f for f in os.listdir(pdir) if f.endswith("_traffic.csv"))
+        for line in open(path):
+            f = [c.strip() for c in line.split(",")]
+            if len(f) >= 5 and f[1].isdigit():
+                tab[(f[0], int(f[1]))] = float(f[2]) + float(f[3])
+                commits.add(f[4])
     except OSError:
         return {}, None
-    if not files:
-        return {}, None
-    tab = {}
-    for line in open(os.path.join(pdir, files[-1])):
-        f = [c.strip() for c in line.split(",")]
-        if len(f) >= 4 and f[1].isdigit():
-            tab[(f[0], int(f[1]))] = float(f[2]) + float(f[3])
-    return tab, "profiles/" + files[-1]
+    return tab, f"paper_2201_00451_b200/traffic_table.csv, captured on commit {'/'.join(sorted(commits))}"
 
 
 def measured_peaks():
@@ -278,7 +277,10 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------
 def time_bank(plan, p, steps, warmup, topk, k, flush, barrier=None, sampler=None):
     """W warm-up steps, then K timed steps of the whole bank (CUDA events on the plan's stream, L2 flushed between
-    steps, per-kernel-class events inside the library).  Returns (per-step ms, class profile, launches, clocks)."""
+    steps) with the library's per-class event recording OFF, then a separate repetition of the same K steps with it ON,
+    from which only the split of the time over the kernel classes is taken (its event pairs per launch group would
+    otherwise sit inside the steps whose launch overhead decides the small cells).
+    Returns (per-step ms, class profile of the profiled repetition, its total ms, launches, clocks)."""
     import torch
     n_t, nb = len(p.templates), plan.n_bins
     if topk:
@@ -293,37 +295,46 @@ def time_bank(plan, p, steps, warmup, topk, k, flush, barrier=None, sampler=None
         else:
             plan.compute(p.templates, out=out)
 
+    def timed(n):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for s in range(n):
+            flush.zero_()
+            ev[s][0].record(stream)
+            step()
+            ev[s][1].record(stream)
+        return ev
+
     for _ in range(warmup):
         step()
     plan.sync()
-    plan.set_profile(True)
+    plan.set_profile(False)
     l0 = plan.launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     if barrier:
         barrier()
     if sampler:
         sampler.start()
     t_wall0 = time.time()
-    for s in range(steps):
-        flush.zero_()
-        ev[s][0].record(stream)
-        step()
-        ev[s][1].record(stream)
+    ev = timed(steps)
     if barrier:
         barrier()
     else:
         torch.cuda.synchronize()
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
-    prof = plan.get_profile()
-    plan.set_profile(False)
     launches = plan.launch_count() - l0
     step_ms = [a.elapsed_time(b) for a, b in ev]
+    # class split: the same steps again, profiled
+    plan.set_profile(True)
+    evp = timed(steps)
+    torch.cuda.synchronize()
+    prof = plan.get_profile()
+    plan.set_profile(False)
+    prof_ms = float(sum(a.elapsed_time(b) for a, b in evp))
     del out
-    return step_ms, prof, launches, clocks
+    return step_ms, prof, prof_ms, launches, clocks
 
 
-def roofline_report(p, prof, total_ms, steps, n_t, world, traffic_tab, traffic_src, peak, peak_src):
+def roofline_report(p, prof, total_ms, steps, n_t, world, traffic_tab, traffic_src, peak, peak_src, prof_ms=None):
     """Roofline of the dominant FFT kernel and of the pair, on SURVEY.md 8(d)'s algorithmic bytes, plus the DRAM-only
     view: which of those bytes are served by HBM and which by L2 (the resampled series S is re-read by every template
     of a sky position out of L2), and the fraction of the measured HBM peak that the ncu-measured DRAM traffic makes."""
@@ -355,11 +366,20 @@ def roofline_report(p, prof, total_ms, steps, n_t, world, traffic_tab, traffic_s
     n_groups = len({(float(a), float(d)) for a, d in p.templates[:, :2]})
     s_from_hbm = ab["S_read"] * n_groups / n_t            # S is read from HBM once per sky position, then from L2
     hbm_alg = s_from_hbm + (0 if single else ab["T_write"] + ab["T_read"]) + ab["twoF_write"]
+    prof_ms = total_ms if prof_ms is None else prof_ms          # duration of the profiled repetition the class times come from
     return {"bound": "hbm", "kernel": dom + "_kernel", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
             "traffic": tr * per_launch if tr is not None else None,
             "traffic_source": ((traffic_src or "") + " (ncu dram__bytes_read.sum + dram__bytes_write.sum per template x templates per launch)") if tr is not None else None,
             "peak_source": peak_src,
+            "conventions": "frac / fft_pair_frac: SURVEY 8(d) algorithmic bytes (B_2pass, INCLUDING the per-template re-read of the "
+                           "resampled series that L2 serves) over FFT KERNEL time; hbm_algorithmic_frac: the HBM-only part of those bytes "
+                           "over kernel time; dram_frac: ncu-measured DRAM bytes over kernel time; step_frac / hbm_algorithmic_step_frac / "
+                           "dram_step_frac: the same three over the WHOLE timed step (SURVEY 8(d): t = the timed fstat_compute call, "
+                           "class profiling off)",
             "fft_pair_achieved": pair, "fft_pair_frac": pair / peak,
+            "step_frac": (b1 + b2) * n_t * steps / (total_ms * 1e-3) / 1e9 / peak,
+            "hbm_algorithmic_step_frac": hbm_alg * n_t * steps / (total_ms * 1e-3) / 1e9 / peak,
+            "dram_step_frac": dram_pair * n_t * steps / (total_ms * 1e-3) / 1e9 / peak if dram_pair is not None else None,
             # which of the algorithmic bytes are HBM traffic and which are L2 hits (per template)
             "algorithmic_bytes_per_template": {"total_B_2pass": b1 + b2, "hbm": hbm_alg, "l2_served_S_reread": ab["S_read"] - s_from_hbm,
                                                "on_chip_T": (ab["T_write"] + ab["T_read"]) if single else 0},
@@ -371,7 +391,7 @@ def roofline_report(p, prof, total_ms, steps, n_t, world, traffic_tab, traffic_s
             "r_min_frac": (8 * p.n_samples * p.n_det + 4 * p.n_bins) * n_t * steps / (total_ms * 1e-3) / 1e9 / peak,
             "alu_tflops": flops / (fft_ms * 1e-3) / 1e12, "alu_peak_tflops": ALU_PEAK_TFLOPS,
             "alu_frac": flops / (fft_ms * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
-            "share_of_step": prof[dom][0] / total_ms if world == 1 else None}, kernels
+            "share_of_step": prof[dom][0] / prof_ms if world == 1 else None}, kernels
 
 
 def cufft_variant(plan, p, ours_us_per_template):
@@ -425,37 +445,78 @@ def cufft_variant(plan, p, ours_us_per_template):
     plan.sync()
     dev = float(((ours - ref).abs() / torch.clamp(ref, min=4.0)).max().item())
     return {"us_per_template_cufft_path": us_path, "us_per_template_two_ffts_only": us_fft,
-            "ours_us_per_template_whole_path": ours_us_per_template,
+            "ours_us_per_template_fft_classes": ours_us_per_template,
             "speedup_vs_cufft_path": us_path / ours_us_per_template,
+            "speedup_vs_two_ffts_only": us_fft / ours_us_per_template,
             "max_rel_dev_ours_vs_cufft_path": dev, "templates": len(same_sky),
             "note": "comparison baseline only, never on the product path: our resampled series S, then torch ops per step "
-                    "(fp64 spin-down phase -> complex64 factor, two torch.fft.fft = cuFFT, 2F expression); the sky-dependent "
-                    "work is excluded from both sides' per-template figure"}
+                    "(fp64 spin-down phase -> complex64 factor, two torch.fft.fft = cuFFT, 2F expression).  The torch path is "
+                    "dominated by its unfused fp64 elementwise phase; the fairer floor for a cuFFT-based design is "
+                    "us_per_template_two_ffts_only (two bare cuFFT transforms, no phase factor, no 2F map), which a fused "
+                    "custom phase / 2F kernel pair could approach but not beat.  ours_us_per_template_fft_classes = our two FFT "
+                    "kernel classes (spin-down prologue + FFT + 2F epilogue); the sky-dependent work is excluded on both sides"}
+
+
+def bounded_cell(p, flush, traffic_tab, peak, warmup, topk=False, k=8, steps=3):
+    """One bounded measurement of a workload for the blocks the default line carries besides its headline: W warm-up +
+    3 timed steps (class profiling off) + 3 profiled steps for the class split, with every roofline convention."""
+    from paper_2201_00451_b200.binding import FstatPlan
+    with FstatPlan(p) as plan:
+        step_ms, prof, prof_ms, launches, _ = time_bank(plan, p, steps, max(3, warmup), topk, k, flush)
+        nb = plan.n_bins
+    n_t = len(p.templates)
+    total_ms = float(sum(step_ms))
+    roof, _ = roofline_report(p, prof, total_ms, steps, n_t, 1, traffic_tab, None, peak, None, prof_ms)
+    ms = total_ms / steps
+    return {"log2_n_fft": int(np.log2(p.n_fft)), "n_det": p.n_det, "n_templates": n_t,
+            "n_sky": len({(float(a), float(d)) for a, d in p.templates[:, :2]}), "dterms": p.dterms,
+            "output": f"top-{k}" if topk else "full 2F",
+            "ms_per_step": ms, "ms_per_step_profiled": prof_ms / steps,
+            "bins_per_s": n_t * nb / (ms * 1e-3), "templates_per_s": n_t / (ms * 1e-3),
+            "tau_eff_s_per_bin_per_detector": ms * 1e-3 / (n_t * nb * p.n_det),
+            "pair_frac": roof["fft_pair_frac"], "step_frac": roof["step_frac"],
+            "dom_kernel": roof["kernel"], "dom_frac": roof["frac"],
+            "hbm_algorithmic_frac": roof["hbm_algorithmic_frac"], "hbm_algorithmic_step_frac": roof["hbm_algorithmic_step_frac"],
+            "dram_frac": roof["dram_frac"], "dram_step_frac": roof["dram_step_frac"],
+            "launches_per_step": launches // steps,
+            "class_ms_per_step": {c: prof[c][0] / steps for c in prof if prof[c][1] > 0}}
 
 
 def config3_block(args, flush, traffic_tab, peak):
-    """Bounded config-3 sweep carried by the default line: one cell per FFT length 2^15 .. 2^23 (256 fdot templates,
-    W warm-up + 3 timed steps each), with the pair / dominant-kernel / DRAM fractions per cell."""
-    from paper_2201_00451_b200.binding import FstatPlan
+    """Bounded config-3 sweep carried by the default line: one cell per FFT length 2^15 .. 2^23 (256 fdot templates)."""
     cells = []
     for days, band in CONFIG3_SWEEP:
         p = synth.config3(days, band)
-        with FstatPlan(p) as plan:
-            step_ms, prof, launches, _ = time_bank(plan, p, 3, max(3, args.warmup), False, 0, flush)
-        n_t = len(p.templates)
-        total_ms = float(sum(step_ms))
-        roof, kern = roofline_report(p, prof, total_ms, 3, n_t, 1, traffic_tab, None, peak, None)
-        cells.append({"days": days, "band_hz": band, "log2_n_fft": int(np.log2(p.n_fft)), "n_templates": n_t,
-                      "ms_per_step": total_ms / 3, "bins_per_s": n_t * p.n_bins / (total_ms / 3 * 1e-3),
-                      "pair_frac": roof["fft_pair_frac"], "dom_kernel": roof["kernel"], "dom_frac": roof["frac"],
-                      "hbm_algorithmic_frac": roof["hbm_algorithmic_frac"], "dram_frac": roof["dram_frac"],
-                      "launches_per_step": launches // 3,
-                      "class_ms_per_step": {c: prof[c][0] / 3 for c in prof if prof[c][1] > 0}})
+        cell = {"days": days, "band_hz": band}
+        cell.update(bounded_cell(p, flush, traffic_tab, peak, args.warmup))
+        cells.append(cell)
         del p
     return {"cells": cells, "min_pair_frac": min(c["pair_frac"] for c in cells),
             "min_pair_cell": min(cells, key=lambda c: c["pair_frac"])["log2_n_fft"],
+            "min_step_frac": min(c["step_frac"] for c in cells),
+            "min_step_cell": min(cells, key=lambda c: c["step_frac"])["log2_n_fft"],
+            "min_hbm_algorithmic_step_frac": min(c["hbm_algorithmic_step_frac"] for c in cells),
             "note": "config 3 (2 detectors, 50 % gaps, 256 fdot templates, full 2F output), one cell per FFT length; "
-                    "pair_frac = B_2pass / (FFT kernel time) / measured HBM peak (SURVEY.md 8(d) R_hbm)"}
+                    "pair_frac = B_2pass / (FFT kernel time) / measured HBM peak; step_frac = B_2pass / (time of the whole "
+                    "fstat_compute step, class profiling off) / peak = SURVEY.md 8(d) R_hbm on its own t; the hbm_algorithmic_* "
+                    "and dram_* figures leave out the re-reads of the resampled series that L2 serves"}
+
+
+# the other BASELINE.json configs and the paper's own timing protocol, bounded (3 timed steps each)
+EXTRA_BLOCKS = [("config1", False), ("config4:0:256", True), ("config5:512", False), ("sky100:10:1", False), ("sky100:1:0.5", False)]
+
+
+def extra_blocks(args, flush, traffic_tab, peak):
+    out = {}
+    for name, topk in EXTRA_BLOCKS:
+        p = make_workload(name)
+        out[name] = bounded_cell(p, flush, traffic_tab, peak, args.warmup, topk=topk, k=8)
+        del p
+    out["note"] = ("config1: 16 templates, FFT 2^17; config4:0:256: 256 of target 0's 16384 fdot x fddot templates, FFT 2^22, top-8 "
+                   "retention (the bank's time is 64 x this step); config5:512: 512 of the 4096 sky positions x 4 spin-downs, FFT 2^18, "
+                   "Dterms 16 (one sky batch; the bank is 8 of these); sky100:<days>:<band>: the paper's timing protocol "
+                   "(PAPER.md:188), 100 sky positions x 1 template on a config-3 cell")
+    return out
 
 
 def run_ours(args):
@@ -501,17 +562,17 @@ def run_ours(args):
     n_t, nb = len(p.templates), plan.n_bins
     topk = args.mode == "topk"
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    step_ms, prof, launches, clocks = time_bank(plan, p, args.steps, args.warmup, topk, args.k, flush, barrier, ClockSampler(local))
+    step_ms, prof, prof_ms, launches, clocks = time_bank(plan, p, args.steps, args.warmup, topk, args.k, flush, barrier, ClockSampler(local))
     total_ms = float(sum(step_ms))
     value, ms_per_step = aggregate_ranks(total_ms, n_t * nb, args.steps, dist if world > 1 else None, "cuda")
     total_ms = ms_per_step * args.steps
 
     peak, peak_src = measured_peaks()
     traffic_tab, traffic_src = ncu_traffic_table()
-    roofline, kernels = roofline_report(p, prof, total_ms, args.steps, n_t, world, traffic_tab, traffic_src or "", peak, peak_src)
+    roofline, kernels = roofline_report(p, prof, total_ms, args.steps, n_t, world, traffic_tab, traffic_src or "", peak, peak_src, prof_ms)
 
     # ---- end to end through the host-buffer entry point (pinned host 2F, D2H inside the timed region)
-    e2e = None
+    e2e = e2e_topk = None
     if not args.no_e2e:
         if topk:
             def e2e_step():
@@ -542,6 +603,23 @@ def run_ours(args):
                "api": api + "; the series is uploaded once by fstat_setup (PAPER.md:93) and is not part of a step"}
         if not topk:
             del host_out
+            # the same bank through fstat_compute_topk_host: only the k loudest bins per template cross PCIe
+            # (retain candidates on the GPU instead of copying every 2F value back)
+            plan.compute_topk_host(p.templates, args.k)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(n_e2e):
+                plan.compute_topk_host(p.templates, args.k)
+            torch.cuda.synchronize()
+            k_ms = 1e3 * (time.perf_counter() - t0) / n_e2e
+            if world > 1:
+                t = torch.tensor([k_ms], device="cuda", dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                k_ms = float(t.item())
+            e2e_topk = {"value": world * n_t * nb / (k_ms * 1e-3), "unit": UNIT, "ms_per_step": k_ms, "steps": n_e2e,
+                        "h2d_bytes_per_step": int(p.templates.nbytes), "d2h_bytes_per_step": int(n_t * args.k * 8),
+                        "api": f"fstat_compute_topk_host (host templates in, host top-{args.k} values + bins out): every bin is "
+                               "searched, only the candidates leave the GPU"}
 
     cufft = None
     if not args.no_cufft_compare and rank == 0:
@@ -554,6 +632,12 @@ def run_ours(args):
         del p.series
         torch.cuda.empty_cache()
         c3 = config3_block(args, flush, traffic_tab, peak)
+    extra = None
+    if rank == 0 and world == 1 and not args.no_extra and args.workload == "config2":
+        if hasattr(p, "series"):
+            del p.series
+        torch.cuda.empty_cache()
+        extra = extra_blocks(args, flush, traffic_tab, peak)
 
     if rank == 0:
         from paper_2201_00451_b200 import build as _b
@@ -567,8 +651,8 @@ def run_ours(args):
                            "output": f"top-{args.k} per template" if topk else "full 2F[n_templates][n_bins]", "multi_gpu": "independent replicas, no collective",
                            "l2": "256 MiB flush buffer written between timed steps; each step also writes "
                                  f"{n_t * nb * 4 / 1e9:.2f} GB of 2F (> L2)"},
-                "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "kernels": kernels,
-                "config3": c3, "cpu_baseline": cpu, "cufft_compare": cufft, "nccl": nccl,
+                "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "e2e_topk": e2e_topk, "roofline": roofline, "kernels": kernels,
+                "config3": c3, "other_workloads": extra, "cpu_baseline": cpu, "cufft_compare": cufft, "nccl": nccl,
                 "library": {"path": os.path.relpath(_b.LIB_PATH, ROOT), "mtime": int(os.path.getmtime(_b.LIB_PATH))}}
         print(json.dumps(line))
     if world > 1:
@@ -593,6 +677,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft-compare", action="store_true")
     ap.add_argument("--no-config3", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the bounded config1 / config4 / config5 / sky100 blocks")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
