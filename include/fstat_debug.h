@@ -56,6 +56,16 @@ FSTAT_API int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slot
  *               Automatic = off: measured never faster than the two-launch form on B200. */
 FSTAT_API int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single);
 
+/* fstat_debug_compute_fafb -- the path of fstat_compute, but the pass-2 epilogue stores the two spectra instead of
+ * combining them with eq. 8: the paper's accuracy tooling compares "the output for F, Fa, and Fb" (Fig. 4),
+ * and 2F alone cannot see a slip that leaves the quadratic form unchanged (Fa <-> conj Fa, a common phase).
+ *  fafb_dev  caller-owned DEVICE memory float32[n_tmpl][n_bins][4] = (Re Fa, Im Fa, Re Fb, Im Fb) of bin q = f_min + q df,
+ *            on the grid convention of DESIGN.md S7 (SSB grid index 0 at t_start - K_m dt: compare with another
+ *            implementation only up to the common factor exp(+2 pi i (f - f_het) K_m dt)).
+ * For accuracy checks on small banks: 16 B per bin, and only for the default launch shapes of n_fft <= 2^22
+ * (FSTAT_ESIZE otherwise). */
+FSTAT_API int fstat_debug_compute_fafb(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *fafb_dev);
+
 #ifdef __cplusplus
 }
 #endif

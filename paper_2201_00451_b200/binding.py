@@ -23,7 +23,7 @@ EXPORTS = [
     "fstat_select_threshold", "fstat_select_topk_noalloc", "fstat_resample_sky", "fstat_sync", "fstat_destroy", "fstat_strerror", "fstat_last_error",
     # include/fstat_debug.h: measurement / experiment hooks
     "fstat_launch_count", "fstat_set_inflight", "fstat_set_profile", "fstat_get_profile",
-    "fstat_debug_set_geometry", "fstat_debug_set_max_sky_slots", "fstat_debug_set_paths",
+    "fstat_debug_set_geometry", "fstat_debug_set_max_sky_slots", "fstat_debug_set_paths", "fstat_debug_compute_fafb",
 ]
 
 
@@ -106,6 +106,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.fstat_debug_set_max_sky_slots.argtypes = [vp, i32]
     lib.fstat_debug_set_paths.restype = C.c_int
     lib.fstat_debug_set_paths.argtypes = [vp, i32, i32]
+    lib.fstat_debug_compute_fafb.restype = C.c_int
+    lib.fstat_debug_compute_fafb.argtypes = [vp, vp, i32, vp]
     lib.fstat_destroy.restype = None
     lib.fstat_destroy.argtypes = [vp]
     lib.fstat_strerror.restype = C.c_char_p
@@ -336,6 +338,14 @@ class FstatPlan:
 
     def debug_set_max_sky_slots(self, n: int):
         self._check(self.lib.fstat_debug_set_max_sky_slots(self.handle, n))
+
+    def debug_compute_fafb(self, templates):
+        """fstat_debug_compute_fafb: (Fa, Fb) as two complex64 device tensors [n_tmpl][n_bins]."""
+        t = _templates_array(templates)
+        torch = self._torch
+        out = torch.empty((t.shape[0], self.n_bins, 4), dtype=torch.float32, device="cuda")
+        self._check(self.lib.fstat_debug_compute_fafb(self.handle, t.ctypes.data, t.shape[0], out.data_ptr()))
+        return torch.complex(out[..., 0], out[..., 1]), torch.complex(out[..., 2], out[..., 3])
 
     def debug_set_paths(self, fused_sky: int = -1, single: int = -1):
         self._check(self.lib.fstat_debug_set_paths(self.handle, fused_sky, single))

@@ -572,7 +572,10 @@ fft_sky_pass1_kernel(const __grid_constant__ FusedArgs q) {
 // ---------------------------------------------------------------------------------------
 // E = register elements per thread: 16, or 32 for the two-pass radix-32 plans (sub-FFT 2^9, 2^10: one trip through
 // shared memory instead of two).
-template <int LOGN, int LOGT, int E>
+// FAFB (debug entry point fstat_debug_compute_fafb only): instead of eq. 8 the epilogue stores the spectra themselves,
+// (Re Fa, Im Fa, Re Fb, Im Fb) per bin as one float4 -- the vectors the paper's accuracy tooling compares next to 2F
+// (PAPER.md:236); p.twoF then points to float4[n_tmpl][n_bins].  A compile-time variant: the product kernels are unchanged.
+template <int LOGN, int LOGT, int E, bool FAFB = false>
 __device__ __forceinline__ void pass2_tile_loop(const FftArgs &p, float4 *sm, const float2 *sm_tw, uint64_t *bar, unsigned &parity,
                                                 int tile, int tile_end, int stride, int t_off, uint64_t pol_T) {
     using C = FftCfg<LOGN, LOGT, E>;
@@ -618,7 +621,11 @@ __device__ __forceinline__ void pass2_tile_loop(const FftArgs &p, float4 *sm, co
                 int q = (PI::out_idx(i, 0) << p.log_other) + m1_0 + w;
 #pragma unroll
                 for (int r = 0; r < RL; ++r, q += q_step) {
-                    if ((unsigned)(q - lo) < span) {
+                    if constexpr (FAFB) {
+                        if (q < nb)
+                            __stcs(reinterpret_cast<float4 *>(p.twoF) + (int64_t)t * nb + q,
+                                   make_float4(a[bb * RL + r].x, b[bb * RL + r].x, a[bb * RL + r].y, b[bb * RL + r].y));
+                    } else if ((unsigned)(q - lo) < span) {
                         const float2 fa = make_float2(a[bb * RL + r].x, b[bb * RL + r].x);    // unpack (re, im) of Fa, Fb
                         const float2 fb = make_float2(a[bb * RL + r].y, b[bb * RL + r].y);
                         float twoF = b_over_d * (fa.x * fa.x + fa.y * fa.y) + a_over_d * (fb.x * fb.x + fb.y * fb.y)
@@ -645,6 +652,16 @@ fft_pass2_kernel(const __grid_constant__ FftArgs p) {
     pass_smem_setup<LOGN, LOGT, E>(p, sm, sm_tw, bar);
     unsigned parity = 0;
     pass2_tile_loop<LOGN, LOGT, E>(p, sm, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_first());
+}
+
+template <int LOGN, int LOGT, int E>
+__global__ void __launch_bounds__(FftCfg<LOGN, LOGT, E>::NT, FftCfg<LOGN, LOGT, E>::MIN_CTAS)
+fft_pass2_fafb_kernel(const __grid_constant__ FftArgs p) {
+    extern __shared__ float4 sm[];
+    float2 *sm_tw; uint64_t *bar;
+    pass_smem_setup<LOGN, LOGT, E>(p, sm, sm_tw, bar);
+    unsigned parity = 0;
+    pass2_tile_loop<LOGN, LOGT, E, true>(p, sm, sm_tw, bar, parity, blockIdx.x, p.n_tiles, gridDim.x, 0, l2_policy_evict_first());
 }
 
 // ---------------------------------------------------------------------------------------
@@ -705,6 +722,7 @@ fft_single_kernel(const __grid_constant__ SingleArgs q) {
 // kernel pointer by (sub-FFT, tile, pass, elements, padding variant)
 template <int LOGN, int LOGT, bool P2, int E, int VAR>
 inline void (*fft_kernel_ptr())(const FftArgs) {
-    if constexpr (P2) return fft_pass2_kernel<LOGN, LOGT, E>;
+    if constexpr (P2 && (VAR & FFT_VAR_FAFB) != 0) return fft_pass2_fafb_kernel<LOGN, LOGT, E>;
+    else if constexpr (P2) return fft_pass2_kernel<LOGN, LOGT, E>;
     else return fft_pass1_kernel<LOGN, LOGT, E, VAR>;
 }

@@ -58,10 +58,11 @@ struct LaunchCtx {
 typedef cudaError_t (*fft_launch_fn)(const LaunchCtx &ctx, FftArgs &a, int tiles_per_tmpl, int n_t);
 
 // pass: 1 or 2; logn: log2 of the sub-FFT length; logt: log2 of the tile size; elems: register elements per thread (16
-// or 32); var: FFT_VAR_* bits of the pass-1 variant (0 for pass 2).  Null when the unit has no such kernel.
+// or 32); var: FFT_VAR_* bits of the pass-1 variant (pass 2: 0 or FFT_VAR_FAFB).  Null when the unit has no such kernel.
 #define FFT_VAR_SKIPZ 1      // neither stage nor touch the zero padding
 #define FFT_VAR_CUBIC 2      // templates with fddot != 0 in the launch
 #define FFT_VAR_GENERIC 4    // general (non-affine) address of the transposed store
+#define FFT_VAR_FAFB 8       // pass 2 only: store (Fa, Fb) per bin instead of 2F (fstat_debug_compute_fafb; default shapes up to n_fft 2^22)
 typedef cudaError_t (*fused_launch_fn)(const LaunchCtx &ctx, FusedArgs &a, int tiles_per_tmpl, int n_groups);
 fused_launch_fn fft_find_fused_kernel(int logn, int logt, int var);      // unit 6
 

@@ -133,9 +133,11 @@ fft_launch_fn FFT_CAT(fft_find_kernel_unit, FFT_UNIT)(int pass, int logn, int lo
 #elif FFT_UNIT == 3    // pass 2, sub-FFT 2^6 .. 2^9
     K(2, 6, 11, 16, 0) K(2, 7, 11, 16, 0) K(2, 8, 11, 16, 0) K(2, 9, 11, 16, 0)
     K(2, 6, 12, 16, 0) K(2, 7, 12, 16, 0) K(2, 8, 12, 16, 0) K(2, 9, 12, 16, 0) K(2, 9, 12, 32, 0)
+    K(2, 6, 12, 16, FFT_VAR_FAFB) K(2, 7, 12, 16, FFT_VAR_FAFB) K(2, 8, 12, 16, FFT_VAR_FAFB) K(2, 9, 12, 32, FFT_VAR_FAFB)   // debug: Fa, Fb out
 #elif FFT_UNIT == 4    // pass 2, sub-FFT 2^10, 2^11
     K(2, 10, 11, 16, 0) K(2, 10, 12, 16, 0) K(2, 10, 13, 16, 0) K(2, 10, 12, 32, 0) K(2, 10, 13, 32, 0)
     K(2, 11, 11, 16, 0) K(2, 11, 12, 16, 0) K(2, 11, 13, 16, 0)
+    K(2, 10, 12, 32, FFT_VAR_FAFB) K(2, 10, 13, 32, FFT_VAR_FAFB)                                                             // debug: Fa, Fb out
 #elif FFT_UNIT == 5    // pass 2, sub-FFT 2^12
     K(2, 12, 12, 16, 0) K(2, 12, 13, 16, 0)
 #endif

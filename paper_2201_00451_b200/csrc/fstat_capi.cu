@@ -323,8 +323,8 @@ int single_group_size(fstat_plan *p, int nt, bool cubic) {
 }
 
 int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t row_stride, bool cubic, uint32_t *gmax = nullptr,
-                     bool accumulate = false, int fused_ng = 0, uint32_t det_mask = 0xffffffffu) {
-    const int single_group = fused_ng > 0 ? 0 : single_group_size(p, nt, cubic);
+                     bool accumulate = false, int fused_ng = 0, uint32_t det_mask = 0xffffffffu, bool fafb = false) {
+    const int single_group = (fused_ng > 0 || fafb) ? 0 : single_group_size(p, nt, cubic);
     const int t_need = single_group > 0 ? std::min(nt, 2 * single_group) : nt;
     if (t_need > p->t_cap) {       // grow the intermediate buffer to the launch size actually used
         CUDA_TRY(p, cudaStreamSynchronize(p->stream));
@@ -382,8 +382,9 @@ int launch_fft_chunk(fstat_plan *p, int g0, int t0, int nt, float *rows, int64_t
     {
         ProfScope ps(p, 2);
         const int tiles2 = 1 << (l1 - p->g.log_w2);
-        const fft_launch_fn f = fft_find_kernel(2, l2, p->g.log_tile2, p->g.p2_elems, 0);
-        if (!f) return fail(p, FSTAT_ESIZE, "unsupported (sub-FFT, tile) combination in FFT pass 2");
+        const fft_launch_fn f = fft_find_kernel(2, l2, p->g.log_tile2, p->g.p2_elems, fafb ? FFT_VAR_FAFB : 0);
+        if (!f) return fail(p, FSTAT_ESIZE, fafb ? "no (Fa, Fb) variant of FFT pass 2 for this geometry (default shapes up to n_fft 2^22 only)"
+                                                 : "unsupported (sub-FFT, tile) combination in FFT pass 2");
         CUDA_TRY(p, f(ctx, a, tiles2, nt));
         ++p->launches;
     }
@@ -473,6 +474,7 @@ struct OutSpec {
     bool accumulate = false;     // OUT_DEV_ROWS: rows += 2F (semi-coherent sum)
     const int32_t *bin_off = nullptr;   // accumulate: host [n_tmpl] bin offsets (null = 0)
     uint32_t det_mask = 0xffffffffu;    // detectors that take part
+    bool fafb = false;           // OUT_DEV_ROWS: rows is float4[n_tmpl][n_bins] = (Fa, Fb) per bin instead of 2F (debug)
 };
 
 // groups of 512 bins (one warp of a pass-2 tile each) per row, and how pass 2 maps them to bins
@@ -629,7 +631,8 @@ int compute_impl(fstat_plan *p, const fstat_template_t *tm, int32_t n_tmpl, cons
         for (int t = t0 + 1; t < t0 + nt && p->chunk_one_sky; ++t) p->chunk_one_sky = tm[t].alpha == tm[t0].alpha && tm[t].delta == tm[t0].delta;
         int r;
         if (out.mode == OUT_DEV_ROWS) {
-            r = launch_fft_chunk(p, g0, t0, nt, out.rows + (int64_t)t0 * nb, nb, cubic, nullptr, out.accumulate, fused_ng, out.det_mask);
+            r = launch_fft_chunk(p, g0, t0, nt, out.rows + (int64_t)t0 * nb * (out.fafb ? 4 : 1), nb, cubic, nullptr, out.accumulate, fused_ng,
+                                 out.det_mask, out.fafb);
             if (r) return r;
         } else if (out.mode == OUT_HOST_ROWS) {
             if (ring_fill + nt > p->ring.rows) { r = flush_ring(); if (r) return r; }
@@ -1216,6 +1219,11 @@ int fstat_debug_set_max_sky_slots(fstat_plan_t *plan, int32_t max_slots) {
         return ensure_sky_slots(plan, 1);
     }
     return FSTAT_OK;
+}
+
+int fstat_debug_compute_fafb(fstat_plan_t *plan, const fstat_template_t *tmpl_host, int32_t n_tmpl, float *fafb_dev) {
+    OutSpec o; o.mode = OUT_DEV_ROWS; o.rows = fafb_dev; o.fafb = true;
+    return compute_impl(plan, tmpl_host, n_tmpl, o);
 }
 
 int fstat_debug_set_paths(fstat_plan_t *plan, int32_t fused_sky, int32_t single) {

@@ -142,6 +142,36 @@ def test_accumulate_with_bin_offsets_across_several_launches():
     np.testing.assert_array_equal(many, one + one)
 
 
+@pytest.mark.parametrize("log_nfft,n_samples,dt,noise,rho", [
+    (15, 20000, 1.0, False, 30.0), (17, 100003, 1.0, True, 8.0), (19, 400001, 0.5, True, 8.0), (20, 700000, 0.5, False, 30.0),
+    (21, 1500000, 0.5, True, 8.0)])
+def test_fa_fb_spectra_match_oracle(log_nfft, n_samples, dt, noise, rho):
+    # the paper's accuracy tooling compares three vectors, "the output for F, Fa, and Fb" (Fig. 4: L2
+    # relative errors up to ~1e-5): 2F alone cannot see a slip that leaves the quadratic form of eq. 8 unchanged
+    # (Fa <-> conj Fa, a phase common to Fa and Fb).  Signal-dominated (no noise) and noisy cases; the oracle and the
+    # library share the SSB grid convention (index 0 at t_start - K_m dt), so the spectra compare directly.
+    p = synth.small_problem(seed=300 + log_nfft, rho=rho, noise=noise, n_templates=2, n_samples=n_samples, dt=dt,
+                            n_fft=1 << log_nfft, fddot=1e-16 if log_nfft == 17 else 0.0)
+    with _plan(p) as plan:
+        fa, fb = plan.debug_compute_fafb(p.templates)
+        twoF = plan.compute(p.templates)
+        plan.sync()
+        fa, fb, twoF = fa.cpu().numpy(), fb.cpu().numpy(), twoF.cpu().numpy()
+    for t in range(len(p.templates)):
+        Fa, Fb, (A, B, C, D) = O.fstat_FaFb(p, p.templates[t])
+        cpu2F = O.twoF_from_FaFb(Fa, Fb, A, B, C, D)
+        for name, g, c in (("Fa", fa[t], Fa), ("Fb", fb[t], Fb), ("2F", twoF[t], cpu2F)):
+            r1, r2, th = O.comparison_metrics(g.astype(np.complex128 if name != "2F" else np.float64), c)
+            print(f"[parity] n_fft 2^{log_nfft}, template {t}, {name}: r1 = {r1:.2e}, r2 = {r2:.2e}, theta = {th:.2e} rad (eq. 9-10)")
+            assert r2 <= 1e-5 and th <= 1e-3, (name, r1, r2, th)
+        # bin by bin, against the largest magnitude of the row (fp32 FFT: errors scale with the row's norm, not the bin's)
+        scale = max(np.abs(Fa).max(), np.abs(Fb).max())
+        assert np.abs(fa[t] - Fa).max() <= 2e-5 * scale and np.abs(fb[t] - Fb).max() <= 2e-5 * scale
+        # and eq. 8 applied to the library's own spectra reproduces its 2F (same registers, fp64 combination here)
+        own = O.twoF_from_FaFb(fa[t].astype(np.complex128), fb[t].astype(np.complex128), A, B, C, D)
+        assert rel_err(twoF[t], own).max() <= 1e-4
+
+
 def test_two_live_topk_plans_of_different_size():
     # the dynamic shared memory attribute of the selection kernel is per function, not per plan
     big = synth.small_problem(seed=96, n_samples=int(0.7 * (1 << 20)), dt=0.5, n_fft=1 << 20, n_templates=2, rho=10.0)
