@@ -16,7 +16,7 @@
 #pragma once
 #include "fstat_common.cuh"
 #include "fft_launch.cuh"
-// Experiment switch (profiles/r02_experiments.md): FFT pass 1 with a staging buffer of its own, so that the next tile's
+// Experiment switch ('Tried, not kept'): FFT pass 1 with a staging buffer of its own, so that the next tile's
 // bulk copy starts as soon as the current tile's inputs are in registers.  Measured slower (3 instead of 5 CTAs per SM).
 #ifndef FFT_P1_DB
 #define FFT_P1_DB 0
