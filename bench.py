@@ -512,7 +512,7 @@ def extra_blocks(args, flush, traffic_tab, peak):
         p = make_workload(name)
         out[name] = bounded_cell(p, flush, traffic_tab, peak, args.warmup, topk=topk, k=8)
         del p
-    out["note"] = ("config1: 16 templates, FFT 2^17; config4:0:256: 256 fdot x 4 fddot = 1024 of target 0's 16384 templates, FFT 2^22, top-8 "
+    out["note"] = ("config1: 16 templates, FFT 2^18; config4:0:256: 256 fdot x 4 fddot = 1024 of target 0's 16384 templates, FFT 2^22, top-8 "
                    "retention (the bank's time is 16 x this step); config5:512: 512 of the 4096 sky positions x 4 spin-downs, FFT 2^18, "
                    "Dterms 16 (one sky batch; the bank is 8 of these); sky100:<days>:<band>: the paper's timing protocol "
                    "(PAPER.md:188), 100 sky positions x 1 template on a config-3 cell")
